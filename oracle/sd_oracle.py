@@ -1,0 +1,144 @@
+"""ctypes binding of the CPU oracle (oracle/sd_oracle.c).
+
+TEST INFRASTRUCTURE, NOT THE PRODUCT: only tests/, __graft_entry__.smoke() and bench.py's
+cpu_baseline / --impl reference legs may import this module.  It does not import, and is not
+imported by, the CUDA package paper_1205_6333_b200.
+
+The oracle evaluates Eq. (7a) of the paper as a plain double loop in fp64 with
+long-double row accumulation; see the header of sd_oracle.c for the readings.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "sd_oracle.c")
+_LIB = os.path.join(_HERE, "libsd_oracle.so")
+
+TENSOR_RPY = 0      # Eq. (7b) + RPY overlap branch for r < 2a
+TENSOR_OSEEN = 1    # Eq. (4)
+TENSOR_RP_FAR = 2   # Eq. (7b) as printed for every r (negative control)
+INT_EULER = 0
+INT_MIDPOINT = 1
+
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile sd_oracle.c with gcc into oracle/libsd_oracle.so (no-op when up to date)."""
+    if (not force and os.path.exists(_LIB)
+            and os.path.getmtime(_LIB) >= os.path.getmtime(_SRC)):
+        return _LIB
+    cmd = ["gcc", "-O2", "-std=c11", "-fPIC", "-shared", "-fopenmp", "-o", _LIB, _SRC, "-lm"]
+    subprocess.run(cmd, check=True)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is not None:
+        return _lib
+    build()
+    lib = ctypes.CDLL(_LIB)
+    dp = ctypes.POINTER(ctypes.c_double)
+    lp = ctypes.POINTER(ctypes.c_longlong)
+    ll, dbl, ci = ctypes.c_longlong, ctypes.c_double, ctypes.c_int
+    lib.sdo_mu0.restype = dbl
+    lib.sdo_mu0.argtypes = [dbl, dbl]
+    lib.sdo_apply_rows.restype = ci
+    lib.sdo_apply_rows.argtypes = [dp, dp, ll, dbl, dbl, ci, lp, ll, dp]
+    lib.sdo_apply.restype = ci
+    lib.sdo_apply.argtypes = [dp, dp, ll, dbl, dbl, ci, dp]
+    lib.sdo_assemble.restype = ci
+    lib.sdo_assemble.argtypes = [dp, ll, dbl, dbl, ci, dp]
+    lib.sdo_step.restype = ci
+    lib.sdo_step.argtypes = [dp, dp, ll, dbl, dbl, ci, dbl, ll, ci, dp, ll, dp]
+    lib.sdo_num_threads.restype = ci
+    lib.sdo_set_num_threads.argtypes = [ci]
+    _lib = lib
+    return lib
+
+
+def _as3(x, name):
+    x = np.ascontiguousarray(np.asarray(x, dtype=np.float64))
+    if x.ndim != 2 or x.shape[1] != 3:
+        raise ValueError(f"{name} must have shape [N, 3], got {x.shape}")
+    return x
+
+
+def _dp(x):
+    return x.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
+
+
+def _check(rc, what):
+    if rc != 0:
+        raise ValueError(f"{what} failed with status {rc}")
+
+
+def mu0(a: float, eta: float) -> float:
+    return float(_load().sdo_mu0(a, eta))
+
+
+def apply(pos, force, a: float, eta: float, tensor: int = TENSOR_RPY) -> np.ndarray:
+    """All rows of Eq. (7a).  pos, force: [N, 3] -> vel [N, 3] (fp64)."""
+    pos, force = _as3(pos, "pos"), _as3(force, "force")
+    if pos.shape != force.shape:
+        raise ValueError("pos and force must have the same shape")
+    vel = np.empty_like(pos)
+    _check(_load().sdo_apply(_dp(pos), _dp(force), pos.shape[0], a, eta, tensor, _dp(vel)),
+           "sdo_apply")
+    return vel
+
+
+def apply_rows(pos, force, rows, a: float, eta: float, tensor: int = TENSOR_RPY) -> np.ndarray:
+    """Rows `rows` of Eq. (7a): returns [len(rows), 3]."""
+    pos, force = _as3(pos, "pos"), _as3(force, "force")
+    if pos.shape != force.shape:
+        raise ValueError("pos and force must have the same shape")
+    rows = np.ascontiguousarray(np.asarray(rows, dtype=np.int64))
+    out = np.empty((rows.shape[0], 3), dtype=np.float64)
+    rc = _load().sdo_apply_rows(_dp(pos), _dp(force), pos.shape[0], a, eta, tensor,
+                                rows.ctypes.data_as(ctypes.POINTER(ctypes.c_longlong)),
+                                rows.shape[0], _dp(out))
+    _check(rc, "sdo_apply_rows")
+    return out
+
+
+def assemble(pos, a: float, eta: float, tensor: int = TENSOR_RPY) -> np.ndarray:
+    """Dense 3N x 3N mobility matrix (small N only)."""
+    pos = _as3(pos, "pos")
+    n = pos.shape[0]
+    M = np.empty((3 * n, 3 * n), dtype=np.float64)
+    _check(_load().sdo_assemble(_dp(pos), n, a, eta, tensor, _dp(M)), "sdo_assemble")
+    return M
+
+
+def step(pos, force, a: float, eta: float, dt: float, n_steps: int, integrator: int,
+         tensor: int = TENSOR_RPY, rec_stride: int = 0):
+    """Integrate n_steps with constant forces.  Returns (pos_final, vel_last, traj|None);
+    traj[k] = positions after (k+1)*rec_stride steps when rec_stride > 0."""
+    pos = _as3(pos, "pos").copy()
+    force = _as3(force, "force")
+    n = pos.shape[0]
+    traj = None
+    tp = None
+    if rec_stride > 0:
+        traj = np.empty((n_steps // rec_stride, n, 3), dtype=np.float64)
+        tp = _dp(traj)
+    vel = np.zeros_like(pos)
+    rc = _load().sdo_step(_dp(pos), _dp(force), n, a, eta, tensor, dt, n_steps, integrator,
+                          tp, max(rec_stride, 1), _dp(vel))
+    _check(rc, "sdo_step")
+    return pos, vel, traj
+
+
+def num_threads() -> int:
+    return int(_load().sdo_num_threads())
+
+
+def set_num_threads(n: int) -> None:
+    _load().sdo_set_num_threads(int(n))
