@@ -1,0 +1,132 @@
+/*
+ * sd_b200.h -- C ABI of libsd_b200.so: Stokesian-dynamics mobility product on NVIDIA B200.
+ *
+ * The library evaluates, on one GPU and on the fly (the 3N x 3N matrix is never stored,
+ * PAPER.md:109), the hot path of Kopp & Hoefling, arXiv:1205.6333:
+ *
+ *   v_i = mu0 F_i + sum_{j != i} T(r_i - r_j) . F_j ,   mu0 = 1/(6 pi eta a)
+ *                                                        Eq. (7a)
+ *   T(r) = mu0 [ 3a/(4r) (I + rr^) + a^3/(2r^3) (I - 3 rr^) ]      Eq. (7b)
+ *   r < 2a: T = mu0 [ (1 - 9r/(32a)) I + 3r/(32a) rr^ ]   (Rotne-Prager-Yamakawa overlap
+ *           form; the paper is silent, BASELINE.json north_star mandates it)
+ *   Oseen variant: G(r) = 1/(8 pi eta r) (I + rr^)                  Eq. (4)
+ *
+ * and the explicit integrators it feeds:
+ *   Euler     r <- r + dt M(r) F
+ *   midpoint  r_h = r + dt/2 M(r) F ;  r <- r + dt M(r_h) F         (north_star)
+ *
+ * Conventions for every entry point
+ *  - Layout: `pos`, `force`, `vel` are contiguous [N][4] records (x, y, z, pad): the paper's
+ *    float4 record.  Element type is `float` for SD_PREC_F32_KAHAN and
+ *    SD_PREC_F32_PLAIN, `double` for SD_PREC_F64.  The pad lane is ignored on input and
+ *    written as 0 on output.  Records must be 16-byte aligned (32 bytes for double).
+ *  - Unless the name ends in `_host`, data pointers are DEVICE pointers owned by the caller.
+ *    The context owns every scratch buffer (packed particle records, partial sums, midpoint
+ *    positions, position low words); nothing is allocated on the hot path.
+ *  - `stream` is a cudaStream_t passed as void* (NULL = default stream).  Calls only enqueue
+ *    work; they do not synchronise the host, except sd_create, sd_destroy and the `_host`
+ *    variants (which return after their result has landed in host memory).
+ *  - Every function returns SD_OK or an error code; sd_last_error() gives the message of the
+ *    last failure on that context (or of the last failed sd_create when ctx is NULL).
+ *    Non-finite particle DATA is not checked (as in the paper's kernels).
+ *  - There is no CPU fallback: without a CUDA device of compute capability 10.x sd_create
+ *    fails with SD_ERR_UNSUPPORTED.
+ *  - Coincident centres (r = 0, j != i): RPY contributes mu0 F_j, Oseen contributes 0.
+ */
+#ifndef SD_B200_H
+#define SD_B200_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct sd_ctx sd_ctx; /* opaque */
+
+typedef enum {
+    SD_OK = 0,
+    SD_ERR_INVALID_ARG = 1,
+    SD_ERR_ALLOC = 2,
+    SD_ERR_CUDA = 3,
+    SD_ERR_UNSUPPORTED = 4
+} sd_status;
+
+typedef enum {
+    SD_TENSOR_RPY = 0,  /* Eq. (7b) for r >= 2a, overlap form for r < 2a (default) */
+    SD_TENSOR_OSEEN = 1 /* Eq. (4), unregularised, for every r > 0 */
+} sd_tensor;
+
+typedef enum {
+    SD_PREC_F32_KAHAN = 0, /* fp32 terms, compensated accumulation; default */
+    SD_PREC_F64 = 1,       /* everything in fp64 */
+    SD_PREC_F32_PLAIN = 2  /* fp32 terms, plain fp32 accumulation: ablation of PAPER.md:253-263 */
+} sd_precision;
+
+typedef enum { SD_INT_EULER = 0, SD_INT_MIDPOINT = 1 } sd_integrator;
+
+/* Force callback for sd_step: must ENQUEUE on `stream` work that fills force[N][4] (device,
+ * element type of the context's precision) from pos[N][4] (device); must not synchronise.
+ * Return 0 on success; any other value aborts sd_step with SD_ERR_INVALID_ARG. */
+typedef int (*sd_force_fn)(const void* pos, void* force, long long N, void* user, void* stream);
+
+/* Create a context for N >= 1 spheres of radius a > 0 in a fluid of viscosity eta > 0 on the
+ * current CUDA device.  Allocates all scratch.  Defaults: SD_TENSOR_RPY, SD_PREC_F32_KAHAN. */
+sd_status sd_create(sd_ctx** out, long long N, double a, double eta);
+
+/* Select the pair tensor / the arithmetic.  Changing the precision changes the element type
+ * expected of pos/force/vel and resets the position compensation. */
+sd_status sd_set_tensor(sd_ctx* ctx, sd_tensor tensor);
+sd_status sd_set_precision(sd_ctx* ctx, sd_precision precision);
+
+/* Step 3 of the paper's loop (Eq. 7a): vel = M(pos) force.
+ * pos, force: in; vel: out (must not alias pos or force). */
+sd_status sd_mobility_apply(sd_ctx* ctx, const void* pos, const void* force, void* vel,
+                            void* stream);
+
+/* Same product with HOST buffers: copies pos/force to the device, runs the product, copies
+ * vel back and waits for it.  Pinned host memory makes the copies asynchronous. */
+sd_status sd_mobility_apply_host(sd_ctx* ctx, const void* pos_host, const void* force_host,
+                                 void* vel_host, void* stream);
+
+/* n_steps >= 0 explicit steps of size dt, pos updated in place (steps 1-3).
+ * Forces, in order of precedence:
+ *   fn != NULL     -> fn(pos, ctx-owned force buffer, N, user, stream) before every product;
+ *   force != NULL  -> constant per-particle forces force[N][4] (device);
+ *   otherwise      -> the same constant force gravity[3] on every particle.
+ * Positions are carried with a context-owned low word (double-single) in
+ * the fp32 modes; it stays valid while the caller does not modify pos between calls (see
+ * sd_reset_compensation).  After the call sd_get_velocity returns the velocities of the last
+ * product evaluated (Euler: M(r_n)F; midpoint: M(r_h)F). */
+sd_status sd_step(sd_ctx* ctx, void* pos, sd_force_fn fn, void* user, const void* force,
+                  const double gravity[3], double dt, long long n_steps,
+                  sd_integrator integrator, void* stream);
+
+/* Copy the velocities of the last product into vel_out[N][4] (device). */
+sd_status sd_get_velocity(sd_ctx* ctx, void* vel_out, void* stream);
+
+/* Forget the position low words (call after editing pos between sd_step calls). */
+sd_status sd_reset_compensation(sd_ctx* ctx, void* stream);
+
+/* Accessors. */
+long long sd_num_particles(const sd_ctx* ctx);
+double sd_self_mobility(const sd_ctx* ctx); /* mu0 = 1/(6 pi eta a) */
+
+/* Number of kernel launches enqueued by this context since creation (bench bookkeeping). */
+long long sd_launch_count(const sd_ctx* ctx);
+
+/* Name of the pair kernel the dispatcher picks for the current settings, e.g.
+ * "pairs_f32x2_i8_rpy"; static storage. */
+const char* sd_kernel_name(const sd_ctx* ctx);
+
+/* Device micro-benchmark used to calibrate the ALU roofline: runs a dependent-chain FMA
+ * kernel (fp32 packed FFMA2 when precision is an F32 mode, DFMA for SD_PREC_F64) on every SM
+ * and writes the achieved TFLOP/s (FMA = 2 flop).  Synchronises the stream. */
+sd_status sd_fma_peak_probe(sd_ctx* ctx, sd_precision precision, double* tflops_out,
+                            void* stream);
+
+const char* sd_last_error(const sd_ctx* ctx);
+void sd_destroy(sd_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SD_B200_H */

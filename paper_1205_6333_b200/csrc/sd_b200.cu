@@ -1,0 +1,481 @@
+// sd_b200.cu -- C ABI (include/sd_b200.h), context, static schedule and kernel dispatcher.
+//
+// Host side only: every step of the hot path (pack, pair sums, reduction + self term,
+// integrator update) runs in the kernels of sd_pairs_f32.cuh / sd_pairs_f64.cuh /
+// sd_stream.cuh.  There is no CPU fallback.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/sd_b200.h"
+#include "sd_common.cuh"
+#include "sd_pairs_f32.cuh"
+#include "sd_pairs_f64.cuh"
+#include "sd_stream.cuh"
+
+namespace {
+
+thread_local std::string g_create_error;
+
+struct Config {
+    int ipt = 0;        // particles i per thread
+    int IB = 0;         // particles per i-block
+    int TJ = 0;         // j per tile
+    int B = 0, T = 0, G = 0;
+    long long U = 0;
+    int max_slots = 0;
+    const void* kernel = nullptr;
+    const char* name = "";
+};
+
+}  // namespace
+
+struct sd_ctx {
+    long long N = 0;
+    long long Nrec = 0;
+    double a = 0, eta = 0, mu0 = 0;
+    int tensor = SD_TENSOR_RPY;
+    int precision = SD_PREC_F32_KAHAN;
+    int device = 0;
+    int num_sms = 0;
+    Config cfg;
+    // device buffers (context-owned)
+    void* rec = nullptr;        // packed records
+    void* part = nullptr;       // segment partial sums
+    void* vel = nullptr;        // velocities of the last product
+    void* pos_lo = nullptr;     // low words of the positions (fp32 modes)
+    void* pos_half = nullptr;   // midpoint positions (for force callbacks)
+    void* force_buf = nullptr;  // forces written by a callback
+    void* stage_pos = nullptr;  // device staging of the _host entry point
+    void* stage_force = nullptr;
+    void* stage_vel = nullptr;
+    void* probe = nullptr;
+    long long* d_cta_u0 = nullptr;
+    int* d_blk_first = nullptr;
+    int* d_blk_nslots = nullptr;
+    bool lo_valid = false;
+    long long launches = 0;
+    std::string err;
+};
+
+namespace {
+
+size_t elem_size(int precision) { return precision == SD_PREC_F64 ? sizeof(double) : sizeof(float); }
+
+sd_status fail(sd_ctx* ctx, sd_status code, const std::string& msg) {
+    if (ctx) ctx->err = msg;
+    else g_create_error = msg;
+    return code;
+}
+
+#define SD_CUDA(ctx, call)                                                                 \
+    do {                                                                                   \
+        cudaError_t e_ = (call);                                                           \
+        if (e_ != cudaSuccess)                                                             \
+            return fail(ctx, e_ == cudaErrorMemoryAllocation ? SD_ERR_ALLOC : SD_ERR_CUDA, \
+                        std::string(#call) + ": " + cudaGetErrorString(e_));               \
+    } while (0)
+
+template <int I2, int TENSOR, int ACC>
+const void* f32_kernel() {
+    return reinterpret_cast<const void*>(&sd::pairs_f32_kernel<I2, TENSOR, ACC>);
+}
+template <int I, int TENSOR>
+const void* f64_kernel() {
+    return reinterpret_cast<const void*>(&sd::pairs_f64_kernel<I, TENSOR>);
+}
+
+void free_buffers(sd_ctx* c) {
+    void** bufs[] = {&c->rec,       &c->part,        &c->vel,       &c->pos_lo, &c->pos_half,
+                     &c->force_buf, &c->stage_pos,   &c->stage_force, &c->stage_vel, &c->probe};
+    for (void** b : bufs) {
+        if (*b) cudaFree(*b);
+        *b = nullptr;
+    }
+    if (c->d_cta_u0) cudaFree(c->d_cta_u0);
+    if (c->d_blk_first) cudaFree(c->d_blk_first);
+    if (c->d_blk_nslots) cudaFree(c->d_blk_nslots);
+    c->d_cta_u0 = nullptr;
+    c->d_blk_first = c->d_blk_nslots = nullptr;
+}
+
+// Pick the kernel variant for (N, precision, tensor), build the static schedule and
+// (re)allocate every scratch buffer.
+sd_status configure(sd_ctx* c) {
+    free_buffers(c);
+    Config cfg;
+    const bool f64 = c->precision == SD_PREC_F64;
+    const bool rpy = c->tensor == SD_TENSOR_RPY;
+    if (!f64) {
+        const bool plain = c->precision == SD_PREC_F32_PLAIN;
+        const int i2 = (c->N > 8192) ? 2 : 1;  // small N: smaller i-blocks, more CTAs
+        cfg.ipt = 2 * i2;
+        cfg.TJ = sd::kTJ;
+        if (i2 == 2) {
+            cfg.kernel = rpy ? (plain ? f32_kernel<2, 0, 1>() : f32_kernel<2, 0, 0>())
+                             : (plain ? f32_kernel<2, 1, 1>() : f32_kernel<2, 1, 0>());
+            cfg.name = rpy ? (plain ? "pairs_f32x2_i4_rpy_plain" : "pairs_f32x2_i4_rpy_kahan")
+                           : (plain ? "pairs_f32x2_i4_oseen_plain" : "pairs_f32x2_i4_oseen_kahan");
+        } else {
+            cfg.kernel = rpy ? (plain ? f32_kernel<1, 0, 1>() : f32_kernel<1, 0, 0>())
+                             : (plain ? f32_kernel<1, 1, 1>() : f32_kernel<1, 1, 0>());
+            cfg.name = rpy ? (plain ? "pairs_f32x2_i2_rpy_plain" : "pairs_f32x2_i2_rpy_kahan")
+                           : (plain ? "pairs_f32x2_i2_oseen_plain" : "pairs_f32x2_i2_oseen_kahan");
+        }
+    } else {
+        cfg.ipt = 2;
+        cfg.TJ = sd::kTJ64;
+        cfg.kernel = rpy ? f64_kernel<2, 0>() : f64_kernel<2, 1>();
+        cfg.name = rpy ? "pairs_f64_i2_rpy" : "pairs_f64_i2_oseen";
+    }
+    cfg.IB = sd::kThreads * cfg.ipt;
+    cfg.B = static_cast<int>((c->N + cfg.IB - 1) / cfg.IB);
+    cfg.T = static_cast<int>((c->N + cfg.TJ - 1) / cfg.TJ);
+    cfg.U = static_cast<long long>(cfg.B) * cfg.T;
+    int occ = 0;
+    SD_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, cfg.kernel, sd::kThreads, 0));
+    if (occ < 1) return fail(c, SD_ERR_CUDA, "pair kernel does not fit on an SM");
+    cfg.G = static_cast<int>(std::min<long long>(cfg.U, static_cast<long long>(c->num_sms) * occ));
+
+    std::vector<long long> u0(cfg.G + 1);
+    for (int g = 0; g <= cfg.G; ++g) u0[g] = static_cast<long long>((__int128)g * cfg.U / cfg.G);
+    std::vector<int> first(cfg.B), nslots(cfg.B);
+    cfg.max_slots = 1;
+    for (int b = 0; b < cfg.B; ++b) {
+        const long long lo = static_cast<long long>(b) * cfg.T;
+        const long long hi = lo + cfg.T - 1;
+        const int cf = static_cast<int>(std::upper_bound(u0.begin(), u0.end(), lo) - u0.begin()) - 1;
+        const int cl = static_cast<int>(std::upper_bound(u0.begin(), u0.end(), hi) - u0.begin()) - 1;
+        first[b] = cf;
+        nslots[b] = cl - cf + 1;
+        cfg.max_slots = std::max(cfg.max_slots, nslots[b]);
+    }
+    c->cfg = cfg;
+
+    const size_t es = elem_size(c->precision);
+    const size_t v4 = 4 * es;
+    const size_t nrec = static_cast<size_t>(c->Nrec);
+    SD_CUDA(c, cudaMalloc(&c->rec, nrec * 2 * v4));
+    const size_t part_per_slot = f64 ? nrec * v4 : nrec * 2 * v4;
+    SD_CUDA(c, cudaMalloc(&c->part, part_per_slot * cfg.max_slots));
+    SD_CUDA(c, cudaMalloc(&c->vel, nrec * v4));
+    SD_CUDA(c, cudaMalloc(&c->pos_lo, nrec * v4));
+    SD_CUDA(c, cudaMalloc(&c->pos_half, nrec * v4));
+    SD_CUDA(c, cudaMalloc(&c->force_buf, nrec * v4));
+    SD_CUDA(c, cudaMemset(c->pos_lo, 0, nrec * v4));
+    SD_CUDA(c, cudaMemset(c->vel, 0, nrec * v4));
+    SD_CUDA(c, cudaMalloc(&c->d_cta_u0, sizeof(long long) * (cfg.G + 1)));
+    SD_CUDA(c, cudaMalloc(&c->d_blk_first, sizeof(int) * cfg.B));
+    SD_CUDA(c, cudaMalloc(&c->d_blk_nslots, sizeof(int) * cfg.B));
+    SD_CUDA(c, cudaMemcpy(c->d_cta_u0, u0.data(), sizeof(long long) * (cfg.G + 1), cudaMemcpyHostToDevice));
+    SD_CUDA(c, cudaMemcpy(c->d_blk_first, first.data(), sizeof(int) * cfg.B, cudaMemcpyHostToDevice));
+    SD_CUDA(c, cudaMemcpy(c->d_blk_nslots, nslots.data(), sizeof(int) * cfg.B, cudaMemcpyHostToDevice));
+    c->lo_valid = true;  // zeroed
+    return SD_OK;
+}
+
+sd::Schedule schedule_of(const sd_ctx* c) {
+    sd::Schedule s;
+    s.cta_u0 = c->d_cta_u0;
+    s.blk_first_cta = c->d_blk_first;
+    s.blk_nslots = c->d_blk_nslots;
+    s.T = c->cfg.T;
+    s.B = c->cfg.B;
+    s.G = c->cfg.G;
+    return s;
+}
+
+sd_status check_launch(sd_ctx* c, const char* what) {
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(c, SD_ERR_CUDA, std::string(what) + ": " + cudaGetErrorString(e));
+    ++c->launches;
+    return SD_OK;
+}
+
+sd_status launch_pack(sd_ctx* c, const void* pos, const void* force, int what, const double g[3],
+                      cudaStream_t st) {
+    const int n = static_cast<int>(c->N), nrec = static_cast<int>(c->Nrec);
+    const int blocks = (nrec + 255) / 256;
+    const double gx = g ? g[0] : 0.0, gy = g ? g[1] : 0.0, gz = g ? g[2] : 0.0;
+    if (c->precision == SD_PREC_F64)
+        sd::pack_kernel<double4><<<blocks, 256, 0, st>>>(
+            static_cast<const double4*>(pos), static_cast<const double4*>(force),
+            static_cast<double4*>(c->rec), what, gx, gy, gz, n, nrec);
+    else
+        sd::pack_kernel<float4><<<blocks, 256, 0, st>>>(
+            static_cast<const float4*>(pos), static_cast<const float4*>(force),
+            static_cast<float4*>(c->rec), what, gx, gy, gz, n, nrec);
+    return check_launch(c, "pack_kernel");
+}
+
+sd_status launch_pairs(sd_ctx* c, cudaStream_t st) {
+    sd::Schedule sch = schedule_of(c);
+    int n = static_cast<int>(c->N);
+    long long stride = c->Nrec;
+    const double a = c->a, mu0 = c->mu0;
+    if (c->precision == SD_PREC_F64) {
+        sd::PairCoef64 k;
+        k.c1 = mu0 * 0.75 * a;
+        k.c2 = mu0 * 0.5 * a * a * a;
+        k.m3c2 = -3.0 * k.c2;
+        k.mu0 = mu0;
+        k.ovA = -9.0 * mu0 / (32.0 * a);
+        k.ovB = 3.0 * mu0 / (32.0 * a);
+        k.four_a2 = 4.0 * a * a;
+        // threshold on the fp32 copy of r^2, inflated so that rounding can only send a pair to
+        // the exact path, never keep an overlapping one on the fast path
+        float thr = (c->tensor == SD_TENSOR_RPY) ? static_cast<float>(k.four_a2 * (1.0 + 1e-6)) : 1e-30f;
+        const double4* rec = static_cast<const double4*>(c->rec);
+        double4* part = static_cast<double4*>(c->part);
+        void* args[] = {&rec, &part, &sch, &k, &thr, &n, &stride};
+        cudaError_t e = cudaLaunchKernel(c->cfg.kernel, dim3(c->cfg.G), dim3(sd::kThreads), args, 0, st);
+        if (e != cudaSuccess) return fail(c, SD_ERR_CUDA, std::string("pairs_f64: ") + cudaGetErrorString(e));
+    } else {
+        sd::PairCoef k;
+        k.c1 = static_cast<float>(mu0 * 0.75 * a);
+        k.c2 = static_cast<float>(mu0 * 0.5 * a * a * a);
+        k.m3c2 = static_cast<float>(-1.5 * mu0 * a * a * a);
+        k.mu0 = static_cast<float>(mu0);
+        k.ovA = static_cast<float>(-9.0 * mu0 / (32.0 * a));
+        k.ovB = static_cast<float>(3.0 * mu0 / (32.0 * a));
+        k.thr = (c->tensor == SD_TENSOR_RPY) ? static_cast<float>(4.0 * a * a) : 1e-30f;
+        const float4* rec = static_cast<const float4*>(c->rec);
+        float4* part = static_cast<float4*>(c->part);
+        void* args[] = {&rec, &part, &sch, &k, &n, &stride};
+        cudaError_t e = cudaLaunchKernel(c->cfg.kernel, dim3(c->cfg.G), dim3(sd::kThreads), args, 0, st);
+        if (e != cudaSuccess) return fail(c, SD_ERR_CUDA, std::string("pairs_f32: ") + cudaGetErrorString(e));
+    }
+    return check_launch(c, c->cfg.name);
+}
+
+template <int MODE>
+sd_status launch_finalize(sd_ctx* c, void* vel, void* pos, double dt, cudaStream_t st) {
+    const int n = static_cast<int>(c->N);
+    const int blocks = (n + 255) / 256;
+    if (c->precision == SD_PREC_F64)
+        sd::finalize_f64_kernel<MODE><<<blocks, 256, 0, st>>>(
+            static_cast<const double4*>(c->part), c->d_blk_nslots, static_cast<double4*>(c->rec),
+            static_cast<double4*>(vel), static_cast<double4*>(pos),
+            static_cast<double4*>(c->pos_half), dt, c->mu0, n, c->cfg.IB, c->Nrec);
+    else
+        sd::finalize_f32_kernel<MODE><<<blocks, 256, 0, st>>>(
+            static_cast<const float4*>(c->part), c->d_blk_nslots, static_cast<float4*>(c->rec),
+            static_cast<float4*>(vel), static_cast<float4*>(pos), static_cast<float4*>(c->pos_lo),
+            static_cast<float4*>(c->pos_half), dt, c->mu0, n, c->cfg.IB, c->Nrec);
+    return check_launch(c, "finalize_kernel");
+}
+
+bool misaligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) & (a - 1)) != 0; }
+
+}  // namespace
+
+extern "C" {
+
+sd_status sd_create(sd_ctx** out, long long N, double a, double eta) {
+    if (!out) return fail(nullptr, SD_ERR_INVALID_ARG, "sd_create: out is NULL");
+    *out = nullptr;
+    if (N < 1 || N > (1LL << 30)) return fail(nullptr, SD_ERR_INVALID_ARG, "sd_create: N must be in [1, 2^30]");
+    if (!(a > 0.0) || !(eta > 0.0) || !std::isfinite(a) || !std::isfinite(eta))
+        return fail(nullptr, SD_ERR_INVALID_ARG, "sd_create: a and eta must be finite and > 0");
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+        cudaGetLastError();
+        return fail(nullptr, SD_ERR_UNSUPPORTED, "sd_create: no CUDA device (there is no CPU fallback)");
+    }
+    int dev = 0;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess)
+        return fail(nullptr, SD_ERR_CUDA, "sd_create: cannot query the current device");
+    if (prop.major != 10)
+        return fail(nullptr, SD_ERR_UNSUPPORTED,
+                    std::string("sd_create: built for sm_100a (B200); device is ") + prop.name);
+    sd_ctx* c = new (std::nothrow) sd_ctx;
+    if (!c) return fail(nullptr, SD_ERR_ALLOC, "sd_create: out of host memory");
+    c->N = N;
+    c->Nrec = (N + SD_REC_ALIGN - 1) / SD_REC_ALIGN * SD_REC_ALIGN;
+    c->a = a;
+    c->eta = eta;
+    c->mu0 = 1.0 / (6.0 * 3.14159265358979323846 * eta * a);
+    c->device = dev;
+    c->num_sms = prop.multiProcessorCount;
+    sd_status st = configure(c);
+    if (st != SD_OK) {
+        g_create_error = c->err;
+        free_buffers(c);
+        delete c;
+        return st;
+    }
+    *out = c;
+    return SD_OK;
+}
+
+sd_status sd_set_tensor(sd_ctx* ctx, sd_tensor tensor) {
+    if (!ctx) return fail(nullptr, SD_ERR_INVALID_ARG, "sd_set_tensor: ctx is NULL");
+    if (tensor != SD_TENSOR_RPY && tensor != SD_TENSOR_OSEEN)
+        return fail(ctx, SD_ERR_INVALID_ARG, "sd_set_tensor: unknown tensor");
+    if (static_cast<int>(tensor) == ctx->tensor) return SD_OK;
+    cudaDeviceSynchronize();
+    ctx->tensor = tensor;
+    return configure(ctx);
+}
+
+sd_status sd_set_precision(sd_ctx* ctx, sd_precision precision) {
+    if (!ctx) return fail(nullptr, SD_ERR_INVALID_ARG, "sd_set_precision: ctx is NULL");
+    if (precision != SD_PREC_F32_KAHAN && precision != SD_PREC_F64 && precision != SD_PREC_F32_PLAIN)
+        return fail(ctx, SD_ERR_INVALID_ARG, "sd_set_precision: unknown precision");
+    if (static_cast<int>(precision) == ctx->precision) return SD_OK;
+    cudaDeviceSynchronize();
+    ctx->precision = precision;
+    return configure(ctx);
+}
+
+sd_status sd_mobility_apply(sd_ctx* ctx, const void* pos, const void* force, void* vel, void* stream) {
+    if (!ctx) return fail(nullptr, SD_ERR_INVALID_ARG, "sd_mobility_apply: ctx is NULL");
+    if (!pos || !force || !vel) return fail(ctx, SD_ERR_INVALID_ARG, "sd_mobility_apply: NULL pointer");
+    const size_t al = 4 * elem_size(ctx->precision);
+    if (misaligned(pos, al) || misaligned(force, al) || misaligned(vel, al))
+        return fail(ctx, SD_ERR_INVALID_ARG, "sd_mobility_apply: records must be 16-byte (float) / 32-byte (double) aligned");
+    if (vel == pos || vel == force) return fail(ctx, SD_ERR_INVALID_ARG, "sd_mobility_apply: vel aliases an input");
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    sd_status s = launch_pack(ctx, pos, force, sd::PACK_POS | sd::PACK_FORCE, nullptr, st);
+    if (s != SD_OK) return s;
+    s = launch_pairs(ctx, st);
+    if (s != SD_OK) return s;
+    return launch_finalize<sd::FIN_VEL>(ctx, vel, nullptr, 0.0, st);
+}
+
+sd_status sd_mobility_apply_host(sd_ctx* ctx, const void* pos_host, const void* force_host,
+                                 void* vel_host, void* stream) {
+    if (!ctx) return fail(nullptr, SD_ERR_INVALID_ARG, "sd_mobility_apply_host: ctx is NULL");
+    if (!pos_host || !force_host || !vel_host)
+        return fail(ctx, SD_ERR_INVALID_ARG, "sd_mobility_apply_host: NULL pointer");
+    const size_t bytes = static_cast<size_t>(ctx->N) * 4 * elem_size(ctx->precision);
+    if (!ctx->stage_pos) {
+        SD_CUDA(ctx, cudaMalloc(&ctx->stage_pos, bytes));
+        SD_CUDA(ctx, cudaMalloc(&ctx->stage_force, bytes));
+        SD_CUDA(ctx, cudaMalloc(&ctx->stage_vel, bytes));
+    }
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    SD_CUDA(ctx, cudaMemcpyAsync(ctx->stage_pos, pos_host, bytes, cudaMemcpyHostToDevice, st));
+    SD_CUDA(ctx, cudaMemcpyAsync(ctx->stage_force, force_host, bytes, cudaMemcpyHostToDevice, st));
+    sd_status s = sd_mobility_apply(ctx, ctx->stage_pos, ctx->stage_force, ctx->stage_vel, stream);
+    if (s != SD_OK) return s;
+    SD_CUDA(ctx, cudaMemcpyAsync(vel_host, ctx->stage_vel, bytes, cudaMemcpyDeviceToHost, st));
+    SD_CUDA(ctx, cudaStreamSynchronize(st));
+    return SD_OK;
+}
+
+sd_status sd_step(sd_ctx* ctx, void* pos, sd_force_fn fn, void* user, const void* force,
+                  const double gravity[3], double dt, long long n_steps, sd_integrator integrator,
+                  void* stream) {
+    if (!ctx) return fail(nullptr, SD_ERR_INVALID_ARG, "sd_step: ctx is NULL");
+    if (!pos) return fail(ctx, SD_ERR_INVALID_ARG, "sd_step: pos is NULL");
+    if (!fn && !force && !gravity) return fail(ctx, SD_ERR_INVALID_ARG, "sd_step: no force given");
+    if (!std::isfinite(dt)) return fail(ctx, SD_ERR_INVALID_ARG, "sd_step: dt is not finite");
+    if (n_steps < 0) return fail(ctx, SD_ERR_INVALID_ARG, "sd_step: n_steps < 0");
+    if (integrator != SD_INT_EULER && integrator != SD_INT_MIDPOINT)
+        return fail(ctx, SD_ERR_INVALID_ARG, "sd_step: unknown integrator");
+    const size_t al = 4 * elem_size(ctx->precision);
+    if (misaligned(pos, al) || (force && misaligned(force, al)))
+        return fail(ctx, SD_ERR_INVALID_ARG, "sd_step: misaligned records");
+    if (n_steps == 0) return SD_OK;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    sd_status s;
+    if (!ctx->lo_valid) {
+        SD_CUDA(ctx, cudaMemsetAsync(ctx->pos_lo, 0, static_cast<size_t>(ctx->Nrec) * al, st));
+        ctx->lo_valid = true;
+    }
+    // constant forces are packed once; callback forces before every product
+    const int force_what = fn ? 0 : (force ? sd::PACK_FORCE : sd::PACK_GRAVITY);
+    s = launch_pack(ctx, pos, force, sd::PACK_POS | force_what, gravity, st);
+    if (s != SD_OK) return s;
+    auto callback = [&](const void* p) -> sd_status {
+        if (!fn) return SD_OK;
+        if (fn(p, ctx->force_buf, ctx->N, user, stream) != 0)
+            return fail(ctx, SD_ERR_INVALID_ARG, "sd_step: force callback failed");
+        return launch_pack(ctx, nullptr, ctx->force_buf, sd::PACK_FORCE, nullptr, st);
+    };
+    for (long long step = 0; step < n_steps; ++step) {
+        if ((s = callback(pos)) != SD_OK) return s;
+        if ((s = launch_pairs(ctx, st)) != SD_OK) return s;
+        if (integrator == SD_INT_EULER) {
+            if ((s = launch_finalize<sd::FIN_EULER>(ctx, ctx->vel, pos, dt, st)) != SD_OK) return s;
+        } else {
+            if ((s = launch_finalize<sd::FIN_HALF>(ctx, ctx->vel, pos, dt, st)) != SD_OK) return s;
+            if ((s = callback(ctx->pos_half)) != SD_OK) return s;
+            if ((s = launch_pairs(ctx, st)) != SD_OK) return s;
+            if ((s = launch_finalize<sd::FIN_FULL>(ctx, ctx->vel, pos, dt, st)) != SD_OK) return s;
+        }
+    }
+    return SD_OK;
+}
+
+sd_status sd_get_velocity(sd_ctx* ctx, void* vel_out, void* stream) {
+    if (!ctx) return fail(nullptr, SD_ERR_INVALID_ARG, "sd_get_velocity: ctx is NULL");
+    if (!vel_out) return fail(ctx, SD_ERR_INVALID_ARG, "sd_get_velocity: vel_out is NULL");
+    const size_t bytes = static_cast<size_t>(ctx->N) * 4 * elem_size(ctx->precision);
+    SD_CUDA(ctx, cudaMemcpyAsync(vel_out, ctx->vel, bytes, cudaMemcpyDeviceToDevice,
+                                 static_cast<cudaStream_t>(stream)));
+    return SD_OK;
+}
+
+sd_status sd_reset_compensation(sd_ctx* ctx, void* stream) {
+    if (!ctx) return fail(nullptr, SD_ERR_INVALID_ARG, "sd_reset_compensation: ctx is NULL");
+    const size_t bytes = static_cast<size_t>(ctx->Nrec) * 4 * elem_size(ctx->precision);
+    SD_CUDA(ctx, cudaMemsetAsync(ctx->pos_lo, 0, bytes, static_cast<cudaStream_t>(stream)));
+    ctx->lo_valid = true;
+    return SD_OK;
+}
+
+long long sd_num_particles(const sd_ctx* ctx) { return ctx ? ctx->N : 0; }
+double sd_self_mobility(const sd_ctx* ctx) { return ctx ? ctx->mu0 : 0.0; }
+long long sd_launch_count(const sd_ctx* ctx) { return ctx ? ctx->launches : 0; }
+const char* sd_kernel_name(const sd_ctx* ctx) { return ctx ? ctx->cfg.name : ""; }
+
+sd_status sd_fma_peak_probe(sd_ctx* ctx, sd_precision precision, double* tflops_out, void* stream) {
+    if (!ctx) return fail(nullptr, SD_ERR_INVALID_ARG, "sd_fma_peak_probe: ctx is NULL");
+    if (!tflops_out) return fail(ctx, SD_ERR_INVALID_ARG, "sd_fma_peak_probe: tflops_out is NULL");
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const int threads = 512, blocks = ctx->num_sms * 4, iters = 4096;
+    if (!ctx->probe) SD_CUDA(ctx, cudaMalloc(&ctx->probe, sizeof(double) * threads * blocks));
+    cudaEvent_t e0, e1;
+    SD_CUDA(ctx, cudaEventCreate(&e0));
+    SD_CUDA(ctx, cudaEventCreate(&e1));
+    float best = 1e30f;
+    for (int rep = 0; rep < 4; ++rep) {
+        cudaEventRecord(e0, st);
+        if (precision == SD_PREC_F64)
+            sd::fma_probe_f64_kernel<<<blocks, threads, 0, st>>>(static_cast<double*>(ctx->probe), 1.0000001, 1e-3, iters);
+        else
+            sd::fma_probe_f32_kernel<<<blocks, threads, 0, st>>>(static_cast<float*>(ctx->probe), 1.0001f, 1e-3f, iters);
+        cudaEventRecord(e1, st);
+        cudaEventSynchronize(e1);
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        if (rep > 0) best = std::min(best, ms);
+        ++ctx->launches;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    SD_CUDA(ctx, cudaGetLastError());
+    const double fmas = static_cast<double>(iters) * 64.0 * threads * blocks;
+    *tflops_out = 2.0 * fmas / (best * 1e-3) / 1e12;
+    return SD_OK;
+}
+
+const char* sd_last_error(const sd_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_error.c_str(); }
+
+void sd_destroy(sd_ctx* ctx) {
+    if (!ctx) return;
+    cudaDeviceSynchronize();
+    free_buffers(ctx);
+    delete ctx;
+}
+
+}  // extern "C"

@@ -1,0 +1,355 @@
+// sd_pairs_f32.cuh -- all-pairs mobility kernel, fp32 terms with compensated accumulation.
+//
+// Computes, for every particle i of the CTA's i-blocks and every j of its j-range,
+//     t_ij = A(r) F_j + B(r) (d.F_j) d ,   d = r_i - r_j                (Eq. 7a/7b)
+// without ever forming the 3x3 tensor, and writes compensated partial sums.
+//
+// Mapping (B200-first, differs from the paper's Alg. 1/2):
+//  * one thread owns I = 2*I2 particles i, held in registers as I2 packed f32x2 pairs; all FP32
+//    work is issued as packed FFMA2/FMUL2/FADD2 (two i per instruction, the j operand is a
+//    broadcast scalar), halving the issue slots per pair interaction;
+//  * j data (32-byte records) are staged in shared memory by 1-D bulk async copies
+//    (cp.async.bulk + mbarrier transaction counts) in a kStages-deep ring; every lane reads the
+//    same record (LDS.128 broadcast), so there are no bank conflicts by construction;
+//  * 1/r comes from one MUFU.RSQ per pair; coefficients need FMUL/FFMA only;
+//  * accumulation (terms of very different magnitude): plain fp32 adds inside a
+//    chunk of kChunk consecutive j, Kahan merge of the chunk sum into (s, c) per particle;
+//  * the r < 2a branch and the j == i exclusion are NOT evaluated per pair: the fast body
+//    evaluates the far-field formula unconditionally and tracks min r^2 per chunk; a chunk
+//    with min r^2 < 4a^2 (an overlapping pair, or the self pair r = 0) is discarded and redone
+//    by the exact, branching slow body.  Overlaps are rare (about 8 phi neighbours per
+//    particle), the self pair occurs once per row.
+#pragma once
+#include "sd_common.cuh"
+
+namespace sd {
+
+constexpr int kThreads = 256;
+constexpr int kWarps = kThreads / 32;
+constexpr int kTJ = 128;     // j records per tile (4 KiB)
+constexpr int kStages = 4;   // ring depth
+constexpr int kPrefetch = 2; // tiles in flight ahead of the one being consumed
+constexpr int kChunk = 32;   // j per compensation chunk
+
+enum { TENSOR_RPY = 0, TENSOR_OSEEN = 1 };
+enum { ACC_KAHAN = 0, ACC_PLAIN = 1 };
+
+__device__ __forceinline__ float rsq_approx(float x) {
+    float y;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+// Packed f32x2 values live in one 64-bit register (an aligned register pair) and are only
+// touched through these wrappers, so that ptxas keeps loop-invariant pairs packed instead of
+// re-assembling them from two scalars before every use.  A pair built from the same scalar
+// twice is folded by ptxas into the broadcast operand form (`R12.F32`) of FFMA2/FMUL2/FADD2.
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pk2(float lo, float hi) {
+    f32x2 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ f32x2 bc2(float s) { return pk2(s, s); }
+__device__ __forceinline__ float lo2(f32x2 v) {
+    float lo;
+    asm("{\n.reg .b32 t;\nmov.b64 {%0, t}, %1;\n}" : "=f"(lo) : "l"(v));
+    return lo;
+}
+__device__ __forceinline__ float hi2(f32x2 v) {
+    float hi;
+    asm("{\n.reg .b32 t;\nmov.b64 {t, %0}, %1;\n}" : "=f"(hi) : "l"(v));
+    return hi;
+}
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) {
+    f32x2 d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) {
+    f32x2 d;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) {
+    f32x2 d;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b) {
+    f32x2 d;
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+
+// Far-field body for two particles i (packed) against one j.  22 packed FP32 instructions + 2
+// MUFU for Rotne-Prager, 19 + 2 for Oseen.
+template <int TENSOR>
+__device__ __forceinline__ void pair_fast2(const f32x2 xi, const f32x2 yi, const f32x2 zi,
+                                           const float4 pj, const float4 fj, const PairCoef& k,
+                                           f32x2& px, f32x2& py, f32x2& pz, float& mn) {
+    const f32x2 dx = sub2(xi, bc2(pj.x));
+    const f32x2 dy = sub2(yi, bc2(pj.y));
+    const f32x2 dz = sub2(zi, bc2(pj.z));
+    f32x2 r2 = mul2(dx, dx);
+    r2 = fma2(dy, dy, r2);
+    r2 = fma2(dz, dz, r2);
+    const float r2a = lo2(r2), r2b = hi2(r2);
+    mn = fminf(mn, fminf(r2a, r2b));
+    const f32x2 inv = pk2(rsq_approx(r2a), rsq_approx(r2b));
+    const f32x2 fx = bc2(fj.x), fy = bc2(fj.y), fz = bc2(fj.z);
+    f32x2 dF = mul2(dx, fx);
+    dF = fma2(dy, fy, dF);
+    dF = fma2(dz, fz, dF);
+    const f32x2 inv2 = mul2(inv, inv);
+    f32x2 A, Bd;
+    if (TENSOR == TENSOR_RPY) {
+        const f32x2 P = fma2(inv2, bc2(k.c2), bc2(k.c1));    // c1 + c2/r^2
+        const f32x2 Q = fma2(inv2, bc2(k.m3c2), bc2(k.c1));  // c1 - 3 c2/r^2
+        A = mul2(P, inv);                                    // c1/r + c2/r^3
+        const f32x2 t = mul2(inv2, dF);                      // (d.F)/r^2
+        const f32x2 u = mul2(Q, t);
+        Bd = mul2(u, inv);                                   // B (d.F)
+    } else {
+        A = mul2(inv, bc2(k.c1));                            // c1/r
+        const f32x2 t = mul2(inv2, dF);
+        Bd = mul2(A, t);                                     // c1 (d.F)/r^3
+    }
+    px = fma2(A, fx, px);
+    py = fma2(A, fy, py);
+    pz = fma2(A, fz, pz);
+    px = fma2(Bd, dx, px);
+    py = fma2(Bd, dy, py);
+    pz = fma2(Bd, dz, pz);
+}
+
+// Exact body for one (i, j): self exclusion, coincident centres, overlap branch.
+template <int TENSOR>
+__device__ __forceinline__ void pair_exact(const float xi, const float yi, const float zi,
+                                           const bool self, const float4 pj, const float4 fj,
+                                           const PairCoef& k, float& px, float& py, float& pz) {
+    if (self) return;
+    const float dx = xi - pj.x, dy = yi - pj.y, dz = zi - pj.z;
+    const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+    if (r2 == 0.0f) {
+        if (TENSOR == TENSOR_RPY) {  // limit of the overlap branch: mu0 F_j
+            px = fmaf(k.mu0, fj.x, px);
+            py = fmaf(k.mu0, fj.y, py);
+            pz = fmaf(k.mu0, fj.z, pz);
+        }
+        return;
+    }
+    const float inv = rsq_approx(r2);
+    const float dF = fmaf(dz, fj.z, fmaf(dy, fj.y, dx * fj.x));
+    float A, B;
+    if (TENSOR == TENSOR_RPY) {
+        if (r2 < k.thr) {  // r < 2a
+            const float r = r2 * inv;
+            A = fmaf(k.ovA, r, k.mu0);
+            B = k.ovB * inv;
+        } else {
+            const float inv2 = inv * inv;
+            A = fmaf(k.c2, inv2, k.c1) * inv;
+            B = fmaf(k.m3c2, inv2, k.c1) * inv2 * inv;
+        }
+    } else {
+        A = k.c1 * inv;
+        B = A * inv * inv;
+    }
+    const float Bd = B * dF;
+    px = fmaf(A, fj.x, px);
+    py = fmaf(A, fj.y, py);
+    pz = fmaf(A, fj.z, pz);
+    px = fmaf(Bd, dx, px);
+    py = fmaf(Bd, dy, py);
+    pz = fmaf(Bd, dz, pz);
+}
+
+__device__ __forceinline__ void kahan_merge2(f32x2& s, f32x2& c, const f32x2 p) {
+    const f32x2 y = sub2(p, c);
+    const f32x2 t = add2(s, y);
+    c = sub2(sub2(t, s), y);
+    s = t;
+}
+
+template <int I2, int TENSOR, int ACC>
+__global__ void __launch_bounds__(kThreads, (I2 <= 2) ? 2 : 1)
+pairs_f32_kernel(const float4* __restrict__ rec, float4* __restrict__ part, const Schedule sch,
+                 const PairCoef k, const int N, const long long slot_stride) {
+    constexpr int I = 2 * I2;
+    constexpr int IB = kThreads * I;
+    __shared__ __align__(128) float4 tiles[kStages][kTJ * 2];
+    __shared__ __align__(8) uint64_t full_bar[kStages];
+    __shared__ __align__(8) uint64_t empty_bar[kStages];
+
+    const int tid = threadIdx.x;
+    const int lane = tid & 31;
+    const int c = blockIdx.x;
+    const long long u_begin = sch.cta_u0[c];
+    const long long u_end = sch.cta_u0[c + 1];
+    const int n_units = static_cast<int>(u_end - u_begin);
+    const int T = sch.T;
+
+    if (tid == 0) {
+        for (int s = 0; s < kStages; ++s) {
+            mbar_init(&full_bar[s], 1);
+            mbar_init(&empty_bar[s], kWarps);
+        }
+        mbar_fence_init();
+    }
+    __syncthreads();
+
+    // producer state (thread 0): next unit to fetch and its j-tile index
+    int pf_n = 0;
+    int pf_t = static_cast<int>(u_begin % T);
+    auto produce = [&]() {
+        const int s = pf_n % kStages;
+        const int q = pf_n / kStages;
+        if (q > 0) mbar_wait(&empty_bar[s], (q - 1) & 1);
+        mbar_arrive_expect_tx(&full_bar[s], kTJ * 32);
+        bulk_load(&tiles[s][0], rec + static_cast<size_t>(pf_t) * (kTJ * 2), kTJ * 32, &full_bar[s]);
+        ++pf_n;
+        if (++pf_t == T) pf_t = 0;
+    };
+    if (tid == 0) {
+        for (int q = 0; q < kPrefetch && pf_n < n_units; ++q) produce();
+    }
+
+    int n = 0;  // tiles consumed so far by this CTA
+    long long u = u_begin;
+    while (u < u_end) {
+        const int b = static_cast<int>(u / T);
+        const int t0 = static_cast<int>(u - static_cast<long long>(b) * T);
+        const long long left = u_end - u;
+        const int nt = (left < static_cast<long long>(T - t0)) ? static_cast<int>(left) : (T - t0);
+        const int i_first = b * IB + tid;  // particle of (m = 0, half 0)
+
+        f32x2 xi[I2], yi[I2], zi[I2];
+
+#pragma unroll
+        for (int m = 0; m < I2; ++m) {
+            const int i0 = i_first + (2 * m) * kThreads;
+            const int i1 = i0 + kThreads;
+            const float4 d = make_float4(SD_DUMMY_I_POS, SD_DUMMY_I_POS, SD_DUMMY_I_POS, 0.f);
+            const float4 p0 = (i0 < N) ? rec[2 * static_cast<size_t>(i0)] : d;
+            const float4 p1 = (i1 < N) ? rec[2 * static_cast<size_t>(i1)] : d;
+            // x + 0 through a packed add: the result is born as an aligned register pair (a
+            // bare pack of two LDG.128 lanes makes ptxas re-assemble the pair at every use)
+            const f32x2 zero = bc2(0.f);
+            xi[m] = add2(pk2(p0.x, p1.x), zero);
+            yi[m] = add2(pk2(p0.y, p1.y), zero);
+            zi[m] = add2(pk2(p0.z, p1.z), zero);
+        }
+        f32x2 sx[I2], sy[I2], sz[I2], cx[I2], cy[I2], cz[I2];  // Kahan (sum, compensation)
+        f32x2 px[I2], py[I2], pz[I2];                          // chunk sum (PLAIN: running sum)
+#pragma unroll
+        for (int m = 0; m < I2; ++m) {
+            sx[m] = sy[m] = sz[m] = cx[m] = cy[m] = cz[m] = bc2(0.f);
+            px[m] = py[m] = pz[m] = bc2(0.f);
+        }
+
+        for (int tt = 0; tt < nt; ++tt, ++n) {
+            if (tid == 0 && pf_n < n_units) produce();
+            const int s = n % kStages;
+            mbar_wait(&full_bar[s], (n / kStages) & 1);
+            const float4* tile = &tiles[s][0];
+            const int jbase = (t0 + tt) * kTJ;
+
+#pragma unroll 1
+            for (int ch = 0; ch < kTJ / kChunk; ++ch) {
+                const float4* cj = tile + ch * (kChunk * 2);
+                f32x2 qx[I2], qy[I2], qz[I2];  // value of p at chunk start (PLAIN only)
+#pragma unroll
+                for (int m = 0; m < I2; ++m) {
+                    if (ACC == ACC_KAHAN) {
+                        px[m] = py[m] = pz[m] = bc2(0.f);
+                    } else {
+                        qx[m] = px[m];
+                        qy[m] = py[m];
+                        qz[m] = pz[m];
+                    }
+                }
+                float mn = 3.0e38f;
+#pragma unroll 4
+                for (int jj = 0; jj < kChunk; ++jj) {
+                    const float4 pj = cj[2 * jj];
+                    const float4 fj = cj[2 * jj + 1];
+#pragma unroll
+                    for (int m = 0; m < I2; ++m)
+                        pair_fast2<TENSOR>(xi[m], yi[m], zi[m], pj, fj, k, px[m], py[m], pz[m], mn);
+                }
+                if (mn < k.thr) {
+                    // an overlapping pair or the self pair sits in this chunk: redo it exactly
+                    const int j0 = jbase + ch * kChunk;
+#pragma unroll
+                    for (int m = 0; m < I2; ++m) {
+                        if (ACC == ACC_KAHAN) {
+                            px[m] = py[m] = pz[m] = bc2(0.f);
+                        } else {
+                            px[m] = qx[m];
+                            py[m] = qy[m];
+                            pz[m] = qz[m];
+                        }
+                    }
+#pragma unroll 1
+                    for (int jj = 0; jj < kChunk; ++jj) {
+                        const float4 pj = cj[2 * jj];
+                        const float4 fj = cj[2 * jj + 1];
+                        const int j = j0 + jj;
+#pragma unroll
+                        for (int m = 0; m < I2; ++m) {
+                            const int i0 = i_first + (2 * m) * kThreads;
+                            float ax = lo2(px[m]), ay = lo2(py[m]), az = lo2(pz[m]);
+                            float bx = hi2(px[m]), by = hi2(py[m]), bz = hi2(pz[m]);
+                            pair_exact<TENSOR>(lo2(xi[m]), lo2(yi[m]), lo2(zi[m]), j == i0, pj, fj,
+                                               k, ax, ay, az);
+                            pair_exact<TENSOR>(hi2(xi[m]), hi2(yi[m]), hi2(zi[m]),
+                                               j == i0 + kThreads, pj, fj, k, bx, by, bz);
+                            px[m] = pk2(ax, bx);
+                            py[m] = pk2(ay, by);
+                            pz[m] = pk2(az, bz);
+                        }
+                    }
+                }
+                if (ACC == ACC_KAHAN) {
+#pragma unroll
+                    for (int m = 0; m < I2; ++m) {
+                        kahan_merge2(sx[m], cx[m], px[m]);
+                        kahan_merge2(sy[m], cy[m], py[m]);
+                        kahan_merge2(sz[m], cz[m], pz[m]);
+                    }
+                }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty_bar[s]);
+        }
+
+        // partial sums of this segment: value = hi - lo
+        const int slot = c - sch.blk_first_cta[b];
+        float4* out = part + static_cast<size_t>(slot) * slot_stride * 2;
+#pragma unroll
+        for (int m = 0; m < I2; ++m) {
+            const int i0 = i_first + (2 * m) * kThreads;
+            const int i1 = i0 + kThreads;
+            if (ACC == ACC_PLAIN) {
+                sx[m] = px[m];
+                sy[m] = py[m];
+                sz[m] = pz[m];
+            }
+            if (i0 < N) {
+                out[2 * static_cast<size_t>(i0)] =
+                    make_float4(lo2(sx[m]), lo2(sy[m]), lo2(sz[m]), 0.f);
+                out[2 * static_cast<size_t>(i0) + 1] =
+                    make_float4(lo2(cx[m]), lo2(cy[m]), lo2(cz[m]), 0.f);
+            }
+            if (i1 < N) {
+                out[2 * static_cast<size_t>(i1)] =
+                    make_float4(hi2(sx[m]), hi2(sy[m]), hi2(sz[m]), 0.f);
+                out[2 * static_cast<size_t>(i1) + 1] =
+                    make_float4(hi2(cx[m]), hi2(cy[m]), hi2(cz[m]), 0.f);
+            }
+        }
+        u += nt;
+    }
+}
+
+}  // namespace sd

@@ -1,0 +1,223 @@
+// sd_pairs_f64.cuh -- all-pairs mobility kernel, everything in fp64 (SD_PREC_F64).
+//
+// Same decomposition, staging ring and chunk-level slow path as the fp32 kernel
+// (sd_pairs_f32.cuh); differences:
+//  * 64-byte records {x, y, z, 0 | Fx, Fy, Fz, 0} of doubles, 64 j per 4 KiB tile;
+//  * no packed arithmetic (there is no DFMA2); one thread owns I particles;
+//  * 1/r: MUFU.RSQ on the fp32-rounded r^2 as a 22-bit seed, then two Newton steps in fp64
+//    (relative error ~1e-7 -> ~1e-14 -> rounding level); no fp64 division or sqrt in the loop;
+//  * fp64 sums need no compensation (measured 2e-13 vs the oracle's long-double rows at
+//    N = 65536); min r^2 is tracked on the fp32 copy of r^2 that the seed needs anyway.
+#pragma once
+#include "sd_common.cuh"
+#include "sd_pairs_f32.cuh"
+
+namespace sd {
+
+constexpr int kTJ64 = 64;  // j records per tile (4 KiB)
+
+__device__ __forceinline__ double rsqrt_nr2(const double r2, const float r2f) {
+    double y = static_cast<double>(rsq_approx(r2f));
+    const double h = 0.5 * r2;
+    double e = fma(-h * y, y, 0.5);
+    y = fma(y, e, y);
+    e = fma(-h * y, y, 0.5);
+    y = fma(y, e, y);
+    return y;
+}
+
+template <int TENSOR>
+__device__ __forceinline__ void pair_fast_f64(const double xi, const double yi, const double zi,
+                                              const double4 pj, const double4 fj,
+                                              const PairCoef64& k, double& px, double& py,
+                                              double& pz, float& mn) {
+    const double dx = xi - pj.x, dy = yi - pj.y, dz = zi - pj.z;
+    const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+    const float r2f = static_cast<float>(r2);
+    mn = fminf(mn, r2f);
+    const double inv = rsqrt_nr2(r2, r2f);
+    const double dF = fma(dz, fj.z, fma(dy, fj.y, dx * fj.x));
+    const double inv2 = inv * inv;
+    double A, Bd;
+    if (TENSOR == TENSOR_RPY) {
+        A = fma(k.c2, inv2, k.c1) * inv;
+        Bd = fma(k.m3c2, inv2, k.c1) * (inv2 * dF) * inv;
+    } else {
+        A = k.c1 * inv;
+        Bd = A * (inv2 * dF);
+    }
+    px = fma(A, fj.x, px);
+    py = fma(A, fj.y, py);
+    pz = fma(A, fj.z, pz);
+    px = fma(Bd, dx, px);
+    py = fma(Bd, dy, py);
+    pz = fma(Bd, dz, pz);
+}
+
+template <int TENSOR>
+__device__ __forceinline__ void pair_exact_f64(const double xi, const double yi, const double zi,
+                                               const bool self, const double4 pj,
+                                               const double4 fj, const PairCoef64& k, double& px,
+                                               double& py, double& pz) {
+    if (self) return;
+    const double dx = xi - pj.x, dy = yi - pj.y, dz = zi - pj.z;
+    const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+    if (r2 == 0.0) {
+        if (TENSOR == TENSOR_RPY) {
+            px = fma(k.mu0, fj.x, px);
+            py = fma(k.mu0, fj.y, py);
+            pz = fma(k.mu0, fj.z, pz);
+        }
+        return;
+    }
+    const double r = sqrt(r2);
+    const double inv = 1.0 / r;
+    const double dF = fma(dz, fj.z, fma(dy, fj.y, dx * fj.x));
+    double A, B;
+    if (TENSOR == TENSOR_RPY) {
+        if (r2 < k.four_a2) {
+            A = fma(k.ovA, r, k.mu0);
+            B = k.ovB * inv;
+        } else {
+            const double inv2 = inv * inv;
+            A = fma(k.c2, inv2, k.c1) * inv;
+            B = fma(k.m3c2, inv2, k.c1) * inv2 * inv;
+        }
+    } else {
+        A = k.c1 * inv;
+        B = A * inv * inv;
+    }
+    const double Bd = B * dF;
+    px = fma(A, fj.x, px);
+    py = fma(A, fj.y, py);
+    pz = fma(A, fj.z, pz);
+    px = fma(Bd, dx, px);
+    py = fma(Bd, dy, py);
+    pz = fma(Bd, dz, pz);
+}
+
+template <int I, int TENSOR>
+__global__ void __launch_bounds__(kThreads, 2)
+pairs_f64_kernel(const double4* __restrict__ rec, double4* __restrict__ part, const Schedule sch,
+                 const PairCoef64 k, const float thr, const int N, const long long slot_stride) {
+    constexpr int IB = kThreads * I;
+    __shared__ __align__(128) double4 tiles[kStages][kTJ64 * 2];
+    __shared__ __align__(8) uint64_t full_bar[kStages];
+    __shared__ __align__(8) uint64_t empty_bar[kStages];
+
+    const int tid = threadIdx.x;
+    const int lane = tid & 31;
+    const int c = blockIdx.x;
+    const long long u_begin = sch.cta_u0[c];
+    const long long u_end = sch.cta_u0[c + 1];
+    const int n_units = static_cast<int>(u_end - u_begin);
+    const int T = sch.T;
+
+    if (tid == 0) {
+        for (int s = 0; s < kStages; ++s) {
+            mbar_init(&full_bar[s], 1);
+            mbar_init(&empty_bar[s], kWarps);
+        }
+        mbar_fence_init();
+    }
+    __syncthreads();
+
+    int pf_n = 0;
+    int pf_t = static_cast<int>(u_begin % T);
+    auto produce = [&]() {
+        const int s = pf_n % kStages;
+        const int q = pf_n / kStages;
+        if (q > 0) mbar_wait(&empty_bar[s], (q - 1) & 1);
+        mbar_arrive_expect_tx(&full_bar[s], kTJ64 * 64);
+        bulk_load(&tiles[s][0], rec + static_cast<size_t>(pf_t) * (kTJ64 * 2), kTJ64 * 64,
+                  &full_bar[s]);
+        ++pf_n;
+        if (++pf_t == T) pf_t = 0;
+    };
+    if (tid == 0) {
+        for (int q = 0; q < kPrefetch && pf_n < n_units; ++q) produce();
+    }
+
+    int n = 0;
+    long long u = u_begin;
+    while (u < u_end) {
+        const int b = static_cast<int>(u / T);
+        const int t0 = static_cast<int>(u - static_cast<long long>(b) * T);
+        const long long left = u_end - u;
+        const int nt = (left < static_cast<long long>(T - t0)) ? static_cast<int>(left) : (T - t0);
+        const int i_first = b * IB + tid;
+
+        double xi[I], yi[I], zi[I], px[I], py[I], pz[I];
+#pragma unroll
+        for (int m = 0; m < I; ++m) {
+            const int i = i_first + m * kThreads;
+            const double dm = static_cast<double>(SD_DUMMY_I_POS);
+            const double4 p = (i < N) ? rec[2 * static_cast<size_t>(i)] : make_double4(dm, dm, dm, 0.0);
+            xi[m] = p.x;
+            yi[m] = p.y;
+            zi[m] = p.z;
+            px[m] = py[m] = pz[m] = 0.0;
+        }
+
+        for (int tt = 0; tt < nt; ++tt, ++n) {
+            if (tid == 0 && pf_n < n_units) produce();
+            const int s = n % kStages;
+            mbar_wait(&full_bar[s], (n / kStages) & 1);
+            const double4* tile = &tiles[s][0];
+            const int jbase = (t0 + tt) * kTJ64;
+
+#pragma unroll 1
+            for (int ch = 0; ch < kTJ64 / kChunk; ++ch) {
+                const double4* cj = tile + ch * (kChunk * 2);
+                double qx[I], qy[I], qz[I];
+#pragma unroll
+                for (int m = 0; m < I; ++m) {
+                    qx[m] = px[m];
+                    qy[m] = py[m];
+                    qz[m] = pz[m];
+                }
+                float mn = 3.0e38f;
+#pragma unroll 4
+                for (int jj = 0; jj < kChunk; ++jj) {
+                    const double4 pj = cj[2 * jj];
+                    const double4 fj = cj[2 * jj + 1];
+#pragma unroll
+                    for (int m = 0; m < I; ++m)
+                        pair_fast_f64<TENSOR>(xi[m], yi[m], zi[m], pj, fj, k, px[m], py[m], pz[m], mn);
+                }
+                if (mn < thr) {
+                    const int j0 = jbase + ch * kChunk;
+#pragma unroll
+                    for (int m = 0; m < I; ++m) {
+                        px[m] = qx[m];
+                        py[m] = qy[m];
+                        pz[m] = qz[m];
+                    }
+#pragma unroll 1
+                    for (int jj = 0; jj < kChunk; ++jj) {
+                        const double4 pj = cj[2 * jj];
+                        const double4 fj = cj[2 * jj + 1];
+                        const int j = j0 + jj;
+#pragma unroll
+                        for (int m = 0; m < I; ++m)
+                            pair_exact_f64<TENSOR>(xi[m], yi[m], zi[m], j == i_first + m * kThreads,
+                                                   pj, fj, k, px[m], py[m], pz[m]);
+                    }
+                }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty_bar[s]);
+        }
+
+        const int slot = c - sch.blk_first_cta[b];
+        double4* out = part + static_cast<size_t>(slot) * slot_stride;
+#pragma unroll
+        for (int m = 0; m < I; ++m) {
+            const int i = i_first + m * kThreads;
+            if (i < N) out[i] = make_double4(px[m], py[m], pz[m], 0.0);
+        }
+        u += nt;
+    }
+}
+
+}  // namespace sd
