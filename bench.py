@@ -1,0 +1,250 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the mobility product v = M(r) F on B200 (BASELINE.json metric).
+
+A "step" is one pass of the whole hot path (pack -> all-pairs kernel -> reduce + self term) over
+one batch of synthetic particles: sd_mobility_apply at N = 1,048,576 (uniform cube, volume
+fraction 0.01, N(0,1) forces, Rotne-Prager-Yamakawa, fp32 terms + Kahan accumulation), the
+configuration the north_star target is quoted on.  Prints ONE JSON line.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+
+N > 1 (torchrun): independent replicas, one per GPU ("replicas only"); the value is
+the summed pair rate over the max-over-ranks time.  --impl reference times the CPU oracle on
+the host cores on a bounded row sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+FLOPS_PER_PAIR = {"rpy": 34, "oseen": 29}       # algorithmic flops
+FP32_LANES_PER_SM, FP64_LANES_PER_SM = 128, 64  # CUDA-core FMA lanes per SM (measured: ubench)
+# DRAM bytes per pair-kernel launch from the ncu --set full capture named in profiles/README.md
+NCU_TRAFFIC_BYTES = {}
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--n", type=int, default=1048576)
+    ap.add_argument("--precision", choices=["f32", "f64"], default="f32")
+    ap.add_argument("--tensor", choices=["rpy", "oseen"], default="rpy")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def workload(n):
+    from paper_1205_6333_b200 import workloads as wl
+    pos, force = wl.sweep(n)
+    return pos, force, wl
+
+
+def workload_name(args):
+    return (f"sd_mobility_apply N={args.n} uniform cube phi=0.01, N(0,1) forces, "
+            f"{args.tensor.upper()}, {'fp32-Kahan' if args.precision == 'f32' else 'fp64'}")
+
+
+def time_oracle(pos64, force64, wl, tensor, target_seconds, n_threads=None):
+    """Oracle pair rate on a bounded seeded row sample sized for about target_seconds."""
+    from oracle import sd_oracle as orc
+    otensor = orc.TENSOR_RPY if tensor == "rpy" else orc.TENSOR_OSEEN
+    n = pos64.shape[0]
+    cores = orc.num_threads()
+    probe_rows = wl.row_subset(n, min(n, 8 * cores), wl.SEED_BASE + 9)
+    t0 = time.perf_counter()
+    orc.apply_rows(pos64, force64, probe_rows, wl.A, wl.ETA, otensor)
+    t_probe = max(time.perf_counter() - t0, 1e-6)
+    rows = int(min(n, max(len(probe_rows), len(probe_rows) * target_seconds / t_probe)))
+    sample = wl.row_subset(n, rows, wl.SEED_BASE + 10)
+    t0 = time.perf_counter()
+    orc.apply_rows(pos64, force64, sample, wl.A, wl.ETA, otensor)
+    t = time.perf_counter() - t0
+    return len(sample) * n / t, cores, len(sample), t
+
+
+def run_reference(args, rank):
+    """--impl reference: the oracle as it stands, on the host cores."""
+    if rank != 0:
+        return
+    pos, force, wl = workload(args.n)
+    p64 = wl.to_xyzw(pos, np.float32)[:, :3].astype(np.float64)
+    f64 = wl.to_xyzw(force, np.float32)[:, :3].astype(np.float64)
+    from oracle import sd_oracle as orc
+    otensor = orc.TENSOR_RPY if args.tensor == "rpy" else orc.TENSOR_OSEEN
+    cores = orc.num_threads()
+    # size one step for ~2 s so that W + K steps stay within a few minutes
+    rate0, _, _, _ = time_oracle(p64, f64, wl, args.tensor, 1.0)
+    rows = int(max(8 * cores, min(args.n, 2.0 * rate0 / args.n)))
+    sample = wl.row_subset(args.n, rows, wl.SEED_BASE + 11)
+    for _ in range(args.warmup):
+        orc.apply_rows(p64, f64, sample, wl.A, wl.ETA, otensor)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        orc.apply_rows(p64, f64, sample, wl.A, wl.ETA, otensor)
+    t = time.perf_counter() - t0
+    value = args.steps * len(sample) * args.n / t
+    sample_desc = f"{len(sample)} seeded rows x all {args.n} columns per step"
+    line = {
+        "impl": "reference", "metric": "pair interactions/s (mobility matvec)", "value": value,
+        "unit": "pairs/s", "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": 1e3 * t / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_name(args), "reference": "CPU oracle (oracle/sd_oracle.c), "
+                   "fp64 + long-double rows, OpenMP", "step": sample_desc},
+        "cpu_baseline": {"value": value, "unit": "pairs/s", "cores": cores, "kind": "oracle",
+                         "sample": sample_desc},
+        "e2e": {"value": value, "unit": "pairs/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    args = parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+
+    import torch
+    import torch.distributed as dist
+    from paper_1205_6333_b200 import benchutil, sd
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    sd.load_library()
+
+    n = args.n
+    pos, force, wl = workload(n)
+    f64mode = args.precision == "f64"
+    npdt = np.float64 if f64mode else np.float32
+    prec = sd.PREC_F64 if f64mode else sd.PREC_F32_KAHAN
+    tensor = sd.TENSOR_RPY if args.tensor == "rpy" else sd.TENSOR_OSEEN
+    h_pos = torch.from_numpy(wl.to_xyzw(pos, npdt)).pin_memory()
+    h_force = torch.from_numpy(wl.to_xyzw(force, npdt)).pin_memory()
+    h_vel = torch.empty_like(h_pos).pin_memory()
+    d_pos, d_force = h_pos.to(dev), h_force.to(dev)
+    d_vel = torch.empty_like(d_pos)
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)  # > 126 MB L2
+
+    ctx = sd.Context(n, wl.A, wl.ETA)
+    ctx.set_precision(prec)
+    ctx.set_tensor(tensor)
+    peak_probe = ctx.fma_peak_probe(prec)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident timing ------------------------------------------------------------
+    for _ in range(args.warmup):
+        ctx.mobility_apply(d_pos, d_force, d_vel)
+    barrier()
+    ctx.profile_enable(True)
+    ctx.profile_read()
+    launches0 = ctx.launch_count
+    sampler = benchutil.ClockSampler(local_rank)
+    sampler.start()
+    evs = []
+    barrier()
+    for _ in range(args.steps):
+        flush.zero_()  # L2 flush between timed iterations (outside the event pair)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        ctx.mobility_apply(d_pos, d_force, d_vel)
+        e1.record()
+        evs.append((e0, e1))
+    barrier()
+    clocks = sampler.stop()
+    local_s = sum(a.elapsed_time(b) for a, b in evs) * 1e-3
+    gpu_launches = ctx.launch_count - launches0
+    pair_ms, pair_launches = ctx.profile_read()
+    ctx.profile_enable(False)
+    units, t_max = benchutil.aggregate_over_ranks(local_s, float(args.steps) * n * n)
+    value = units / t_max
+
+    # ---- end to end through the host-buffer entry point ------------------------------------
+    ctx.mobility_apply_host(h_pos, h_force, h_vel)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        ctx.mobility_apply_host(h_pos, h_force, h_vel)  # returns after vel landed on the host
+    torch.cuda.synchronize()
+    e2e_local = time.perf_counter() - t0
+    barrier()
+    e2e_units, e2e_t = benchutil.aggregate_over_ranks(e2e_local, float(args.steps) * n * n)
+    rec_bytes = n * 4 * (8 if f64mode else 4)
+
+    # ---- roofline of the dominant kernel (compute bound on the CUDA-core FMA pipes) --------
+    sm_count = torch.cuda.get_device_properties(dev).multi_processor_count
+    peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    sm_max_mhz = 1965.0
+    if os.path.exists(peaks_path):
+        with open(peaks_path) as f:
+            sm_max_mhz = float(json.load(f).get("sm_max_mhz", sm_max_mhz))
+    lanes = FP64_LANES_PER_SM if f64mode else FP32_LANES_PER_SM
+    peak_tflops = sm_count * lanes * 2 * sm_max_mhz * 1e6 / 1e12
+    flops = FLOPS_PER_PAIR[args.tensor]
+    achieved = flops * float(n) * n * pair_launches / (pair_ms * 1e-3) / 1e12 if pair_ms > 0 else None
+    roofline = {
+        "bound": "alu", "kernel": ctx.kernel_name, "achieved": achieved, "peak": peak_tflops,
+        "unit": "TFLOP/s", "frac": (achieved / peak_tflops) if achieved else None,
+        "traffic": NCU_TRAFFIC_BYTES.get((n, args.precision, args.tensor)),
+        "peak_source": f"derived: {sm_count} SMs x {lanes} FMA lanes x 2 flop x {sm_max_mhz:.0f} MHz "
+                       "(sm_max_mhz of MEASURED_PEAKS.json; DESIGN.md)",
+        "fma_probe_tflops": peak_probe,
+        "flops_per_pair": flops, "kernel_ms": pair_ms / max(pair_launches, 1),
+        "kernel_share_of_step": pair_ms * 1e-3 / local_s if local_s > 0 else None,
+        "frac_at_measured_clock": (achieved / (peak_tflops * clocks["sm_mhz"] / sm_max_mhz))
+        if achieved and clocks.get("sm_mhz") else None,
+    }
+
+    line = {
+        "metric": "pair interactions/s (mobility matvec)", "value": value, "unit": "pairs/s",
+        "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": 1e3 * t_max / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64" if f64mode else "f32", "data": "synthetic",
+        "config": {"workload": workload_name(args), "kernel": ctx.kernel_name,
+                   "parallelism": "replicas only (no sharding, no collective)" if world > 1 else "1 GPU",
+                   "l2": "inputs (33.5 MB) fit in L2; L2 flushed with a 256 MiB write between timed iterations"},
+        "clocks": clocks, "gpu_launches": gpu_launches,
+        "e2e": {"value": e2e_units / e2e_t, "unit": "pairs/s", "h2d_bytes_per_step": 2 * rec_bytes,
+                "d2h_bytes_per_step": rec_bytes},
+        "roofline": roofline,
+    }
+
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        p64 = h_pos.numpy()[:, :3].astype(np.float64)
+        f64 = h_force.numpy()[:, :3].astype(np.float64)
+        rate, cores, rows, secs = time_oracle(p64, f64, wl, args.tensor, 15.0)
+        line["cpu_baseline"] = {"value": rate, "unit": "pairs/s", "cores": cores, "kind": "oracle",
+                                "sample": f"{rows} seeded rows x all {n} columns of the same "
+                                          f"workload, {secs:.1f} s"}
+    ctx.close()
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -113,6 +113,13 @@ double sd_self_mobility(const sd_ctx* ctx); /* mu0 = 1/(6 pi eta a) */
 /* Number of kernel launches enqueued by this context since creation (bench bookkeeping). */
 long long sd_launch_count(const sd_ctx* ctx);
 
+/* Per-kernel timing for the roofline report: while enabled, every launch of the pair kernel is
+ * bracketed by CUDA events on the launching stream.  sd_profile_read waits for the recorded
+ * launches, returns their summed duration [ms] and count, and clears the record.  At most 4096
+ * launches are kept between reads (later ones are not recorded). */
+sd_status sd_profile_enable(sd_ctx* ctx, int on);
+sd_status sd_profile_read(sd_ctx* ctx, double* pair_kernel_ms, long long* pair_kernel_launches);
+
 /* Name of the pair kernel the dispatcher picks for the current settings, e.g.
  * "pairs_f32x2_i8_rpy"; static storage. */
 const char* sd_kernel_name(const sd_ctx* ctx);

@@ -11,6 +11,7 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <utility>
 #include <vector>
 
 #include "../../include/sd_b200.h"
@@ -61,6 +62,9 @@ struct sd_ctx {
     int* d_blk_nslots = nullptr;
     bool lo_valid = false;
     long long launches = 0;
+    bool profiling = false;
+    std::vector<std::pair<cudaEvent_t, cudaEvent_t>> prof_events;  // recorded, not yet read
+    std::vector<std::pair<cudaEvent_t, cudaEvent_t>> prof_pool;    // reusable
     std::string err;
 };
 
@@ -114,20 +118,29 @@ sd_status configure(sd_ctx* c) {
     const bool rpy = c->tensor == SD_TENSOR_RPY;
     if (!f64) {
         const bool plain = c->precision == SD_PREC_F32_PLAIN;
-        const int i2 = (c->N > 8192) ? 2 : 1;  // small N: smaller i-blocks, more CTAs
+        // particles per thread: 8 once there is enough work to balance 2048-particle i-blocks
+        // over the SMs (more operand reuse per j record); smaller i-blocks below that
+        const int i2 = (c->N >= 131072) ? 4 : (c->N > 8192) ? 2 : 1;
         cfg.ipt = 2 * i2;
         cfg.TJ = sd::kTJ;
-        if (i2 == 2) {
+        static const char* names[3][2][2] = {
+            {{"pairs_f32x2_i2_rpy_kahan", "pairs_f32x2_i2_rpy_plain"},
+             {"pairs_f32x2_i2_oseen_kahan", "pairs_f32x2_i2_oseen_plain"}},
+            {{"pairs_f32x2_i4_rpy_kahan", "pairs_f32x2_i4_rpy_plain"},
+             {"pairs_f32x2_i4_oseen_kahan", "pairs_f32x2_i4_oseen_plain"}},
+            {{"pairs_f32x2_i8_rpy_kahan", "pairs_f32x2_i8_rpy_plain"},
+             {"pairs_f32x2_i8_oseen_kahan", "pairs_f32x2_i8_oseen_plain"}}};
+        const int v = (i2 == 1) ? 0 : (i2 == 2) ? 1 : 2;
+        cfg.name = names[v][rpy ? 0 : 1][plain ? 1 : 0];
+        if (i2 == 4)
+            cfg.kernel = rpy ? (plain ? f32_kernel<4, 0, 1>() : f32_kernel<4, 0, 0>())
+                             : (plain ? f32_kernel<4, 1, 1>() : f32_kernel<4, 1, 0>());
+        else if (i2 == 2)
             cfg.kernel = rpy ? (plain ? f32_kernel<2, 0, 1>() : f32_kernel<2, 0, 0>())
                              : (plain ? f32_kernel<2, 1, 1>() : f32_kernel<2, 1, 0>());
-            cfg.name = rpy ? (plain ? "pairs_f32x2_i4_rpy_plain" : "pairs_f32x2_i4_rpy_kahan")
-                           : (plain ? "pairs_f32x2_i4_oseen_plain" : "pairs_f32x2_i4_oseen_kahan");
-        } else {
+        else
             cfg.kernel = rpy ? (plain ? f32_kernel<1, 0, 1>() : f32_kernel<1, 0, 0>())
                              : (plain ? f32_kernel<1, 1, 1>() : f32_kernel<1, 1, 0>());
-            cfg.name = rpy ? (plain ? "pairs_f32x2_i2_rpy_plain" : "pairs_f32x2_i2_rpy_kahan")
-                           : (plain ? "pairs_f32x2_i2_oseen_plain" : "pairs_f32x2_i2_oseen_kahan");
-        }
     } else {
         cfg.ipt = 2;
         cfg.TJ = sd::kTJ64;
@@ -214,7 +227,26 @@ sd_status launch_pack(sd_ctx* c, const void* pos, const void* force, int what, c
     return check_launch(c, "pack_kernel");
 }
 
+sd_status launch_pairs_impl(sd_ctx* c, cudaStream_t st);
+
 sd_status launch_pairs(sd_ctx* c, cudaStream_t st) {
+    if (!c->profiling || c->prof_events.size() >= 4096) return launch_pairs_impl(c, st);
+    std::pair<cudaEvent_t, cudaEvent_t> ev;
+    if (!c->prof_pool.empty()) {
+        ev = c->prof_pool.back();
+        c->prof_pool.pop_back();
+    } else {
+        SD_CUDA(c, cudaEventCreate(&ev.first));
+        SD_CUDA(c, cudaEventCreate(&ev.second));
+    }
+    SD_CUDA(c, cudaEventRecord(ev.first, st));
+    sd_status s = launch_pairs_impl(c, st);
+    SD_CUDA(c, cudaEventRecord(ev.second, st));
+    c->prof_events.push_back(ev);
+    return s;
+}
+
+sd_status launch_pairs_impl(sd_ctx* c, cudaStream_t st) {
     sd::Schedule sch = schedule_of(c);
     int n = static_cast<int>(c->N);
     long long stride = c->Nrec;
@@ -245,6 +277,7 @@ sd_status launch_pairs(sd_ctx* c, cudaStream_t st) {
         k.ovA = static_cast<float>(-9.0 * mu0 / (32.0 * a));
         k.ovB = static_cast<float>(3.0 * mu0 / (32.0 * a));
         k.thr = (c->tensor == SD_TENSOR_RPY) ? static_cast<float>(4.0 * a * a) : 1e-30f;
+        k.det_thr = 0.f;  // only read by the experimental summed detectors (SD_DETECT 3/4)
         const float4* rec = static_cast<const float4*>(c->rec);
         float4* part = static_cast<float4*>(c->part);
         void* args[] = {&rec, &part, &sch, &k, &n, &stride};
@@ -438,6 +471,30 @@ double sd_self_mobility(const sd_ctx* ctx) { return ctx ? ctx->mu0 : 0.0; }
 long long sd_launch_count(const sd_ctx* ctx) { return ctx ? ctx->launches : 0; }
 const char* sd_kernel_name(const sd_ctx* ctx) { return ctx ? ctx->cfg.name : ""; }
 
+sd_status sd_profile_enable(sd_ctx* ctx, int on) {
+    if (!ctx) return fail(nullptr, SD_ERR_INVALID_ARG, "sd_profile_enable: ctx is NULL");
+    ctx->profiling = on != 0;
+    return SD_OK;
+}
+
+sd_status sd_profile_read(sd_ctx* ctx, double* pair_kernel_ms, long long* pair_kernel_launches) {
+    if (!ctx) return fail(nullptr, SD_ERR_INVALID_ARG, "sd_profile_read: ctx is NULL");
+    if (!pair_kernel_ms || !pair_kernel_launches)
+        return fail(ctx, SD_ERR_INVALID_ARG, "sd_profile_read: NULL output");
+    double total = 0.0;
+    for (auto& ev : ctx->prof_events) {
+        SD_CUDA(ctx, cudaEventSynchronize(ev.second));
+        float ms = 0.f;
+        SD_CUDA(ctx, cudaEventElapsedTime(&ms, ev.first, ev.second));
+        total += ms;
+        ctx->prof_pool.push_back(ev);
+    }
+    *pair_kernel_ms = total;
+    *pair_kernel_launches = static_cast<long long>(ctx->prof_events.size());
+    ctx->prof_events.clear();
+    return SD_OK;
+}
+
 sd_status sd_fma_peak_probe(sd_ctx* ctx, sd_precision precision, double* tflops_out, void* stream) {
     if (!ctx) return fail(nullptr, SD_ERR_INVALID_ARG, "sd_fma_peak_probe: ctx is NULL");
     if (!tflops_out) return fail(ctx, SD_ERR_INVALID_ARG, "sd_fma_peak_probe: tflops_out is NULL");
@@ -474,6 +531,11 @@ const char* sd_last_error(const sd_ctx* ctx) { return ctx ? ctx->err.c_str() : g
 void sd_destroy(sd_ctx* ctx) {
     if (!ctx) return;
     cudaDeviceSynchronize();
+    for (auto* v : {&ctx->prof_events, &ctx->prof_pool})
+        for (auto& ev : *v) {
+            cudaEventDestroy(ev.first);
+            cudaEventDestroy(ev.second);
+        }
     free_buffers(ctx);
     delete ctx;
 }

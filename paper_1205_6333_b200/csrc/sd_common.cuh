@@ -83,6 +83,7 @@ struct PairCoef {
     float ovA;    // -9 mu0 / (32 a)     overlap branch: A = mu0 + ovA * r
     float ovB;    // 3 mu0 / (32 a)      overlap branch: B = ovB / r
     float thr;    // slow-path threshold on r^2: 4a^2 for RPY, tiny for Oseen (only r == 0)
+    float det_thr;  // same threshold for the summed detector (SD_DETECT 3: 1/thr^2, 4: 1/thr)
 };
 
 struct PairCoef64 {

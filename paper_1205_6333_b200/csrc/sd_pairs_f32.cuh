@@ -11,7 +11,8 @@
 //  * j data (32-byte records) are staged in shared memory by 1-D bulk async copies
 //    (cp.async.bulk + mbarrier transaction counts) in a kStages-deep ring; every lane reads the
 //    same record (LDS.128 broadcast), so there are no bank conflicts by construction;
-//  * 1/r comes from one MUFU.RSQ per pair; coefficients need FMUL/FFMA only;
+//  * 1/r and 1/r^2 come from MUFU.RSQ and MUFU.RCP (the XU pipe is otherwise idle); the
+//    coefficients need FMUL/FFMA only: 21 packed FP32 instructions per two pairs (RPY);
 //  * accumulation (terms of very different magnitude): plain fp32 adds inside a
 //    chunk of kChunk consecutive j, Kahan merge of the chunk sum into (s, c) per particle;
 //  * the r < 2a branch and the j == i exclusion are NOT evaluated per pair: the fast body
@@ -22,14 +23,38 @@
 #pragma once
 #include "sd_common.cuh"
 
+// Tuning knobs (defaults are the shipped configuration; the experiment harness overrides them)
+#ifndef SD_THREADS
+#define SD_THREADS 256
+#endif
+#ifndef SD_UNROLL_J
+#define SD_UNROLL_J 4
+#endif
+#ifndef SD_ACC_ORDER
+#define SD_ACC_ORDER 0
+#endif
+#ifndef SD_RCP
+#define SD_RCP 1      // 1: 1/r^2 from MUFU.RCP instead of inv*inv (one packed multiply less)
+#endif
+#ifndef SD_DETECT
+#define SD_DETECT 0   // how the chunk-level overlap/self detector is fed (see pair_fast2)
+#endif
+#ifndef SD_STAGED
+#define SD_STAGED 1
+#endif
+#ifndef SD_MIN_BLOCKS
+#define SD_MIN_BLOCKS(I2) (((I2) <= 2) ? 2 : 1)
+#endif
+
 namespace sd {
 
-constexpr int kThreads = 256;
+constexpr int kThreads = SD_THREADS;
 constexpr int kWarps = kThreads / 32;
 constexpr int kTJ = 128;     // j records per tile (4 KiB)
 constexpr int kStages = 4;   // ring depth
 constexpr int kPrefetch = 2; // tiles in flight ahead of the one being consumed
 constexpr int kChunk = 32;   // j per compensation chunk
+constexpr int kUnrollJ = SD_UNROLL_J;
 
 enum { TENSOR_RPY = 0, TENSOR_OSEEN = 1 };
 enum { ACC_KAHAN = 0, ACC_PLAIN = 1 };
@@ -37,6 +62,11 @@ enum { ACC_KAHAN = 0, ACC_PLAIN = 1 };
 __device__ __forceinline__ float rsq_approx(float x) {
     float y;
     asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ float rcp_approx(float x) {
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
 }
 // Packed f32x2 values live in one 64-bit register (an aligned register pair) and are only
@@ -81,12 +111,13 @@ __device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b) {
     return d;
 }
 
-// Far-field body for two particles i (packed) against one j.  22 packed FP32 instructions + 2
-// MUFU for Rotne-Prager, 19 + 2 for Oseen.
+// Far-field body for two particles i (packed) against one j.  21 packed FP32 instructions + 4
+// MUFU for Rotne-Prager, 18 + 4 for Oseen (one more packed multiply and 2 MUFU with SD_RCP 0).
 template <int TENSOR>
 __device__ __forceinline__ void pair_fast2(const f32x2 xi, const f32x2 yi, const f32x2 zi,
                                            const float4 pj, const float4 fj, const PairCoef& k,
-                                           f32x2& px, f32x2& py, f32x2& pz, float& mn) {
+                                           f32x2& px, f32x2& py, f32x2& pz, float& mn,
+                                           f32x2& det) {
     const f32x2 dx = sub2(xi, bc2(pj.x));
     const f32x2 dy = sub2(yi, bc2(pj.y));
     const f32x2 dz = sub2(zi, bc2(pj.z));
@@ -94,13 +125,36 @@ __device__ __forceinline__ void pair_fast2(const f32x2 xi, const f32x2 yi, const
     r2 = fma2(dy, dy, r2);
     r2 = fma2(dz, dz, r2);
     const float r2a = lo2(r2), r2b = hi2(r2);
+#ifndef SD_EXP_NOMIN
+#if SD_DETECT == 0
     mn = fminf(mn, fminf(r2a, r2b));
+#elif SD_DETECT == 1
+    mn = fminf(mn, r2a);
+    mn = fminf(mn, r2b);
+#elif SD_DETECT == 2
+    if (r2a < k.thr) mn = 0.f;
+    if (r2b < k.thr) mn = 0.f;
+#endif
+#endif
+#ifndef SD_EXP_NOMUFU
     const f32x2 inv = pk2(rsq_approx(r2a), rsq_approx(r2b));
+#else
+    const f32x2 inv = mul2(r2, bc2(1e-3f));
+#endif
     const f32x2 fx = bc2(fj.x), fy = bc2(fj.y), fz = bc2(fj.z);
     f32x2 dF = mul2(dx, fx);
     dF = fma2(dy, fy, dF);
     dF = fma2(dz, fz, dF);
+#if SD_RCP
+    const f32x2 inv2 = pk2(rcp_approx(r2a), rcp_approx(r2b));
+#else
     const f32x2 inv2 = mul2(inv, inv);
+#endif
+#if SD_DETECT == 3
+    det = fma2(inv2, inv2, det);   // sum of 1/r^4 >= max of 1/r^4: never misses an overlap
+#elif SD_DETECT == 4
+    det = add2(det, inv2);
+#endif
     f32x2 A, Bd;
     if (TENSOR == TENSOR_RPY) {
         const f32x2 P = fma2(inv2, bc2(k.c2), bc2(k.c1));    // c1 + c2/r^2
@@ -114,12 +168,100 @@ __device__ __forceinline__ void pair_fast2(const f32x2 xi, const f32x2 yi, const
         const f32x2 t = mul2(inv2, dF);
         Bd = mul2(A, t);                                     // c1 (d.F)/r^3
     }
+#if SD_ACC_ORDER == 0
     px = fma2(A, fx, px);
     py = fma2(A, fy, py);
     pz = fma2(A, fz, pz);
     px = fma2(Bd, dx, px);
     py = fma2(Bd, dy, py);
     pz = fma2(Bd, dz, pz);
+#elif SD_ACC_ORDER == 1
+    px = fma2(A, fx, px);
+    px = fma2(Bd, dx, px);
+    py = fma2(A, fy, py);
+    py = fma2(Bd, dy, py);
+    pz = fma2(A, fz, pz);
+    pz = fma2(Bd, dz, pz);
+#else
+    // fold A F + Bd d into a temporary first: one accumulator read per component
+    const f32x2 tx = fma2(Bd, dx, mul2(A, fx));
+    const f32x2 ty = fma2(Bd, dy, mul2(A, fy));
+    const f32x2 tz = fma2(Bd, dz, mul2(A, fz));
+    px = add2(px, tx);
+    py = add2(py, ty);
+    pz = add2(pz, tz);
+#endif
+}
+
+// The same body for all I2 packed groups of a thread against one j, written stage by stage so
+// that consecutive instructions share the broadcast j operand (operand-reuse cache) -- the
+// register file, not the FMA pipe, is the binding resource of this kernel.
+template <int I2, int TENSOR>
+__device__ __forceinline__ void pair_fast_staged(const f32x2 (&xi)[I2], const f32x2 (&yi)[I2],
+                                                 const f32x2 (&zi)[I2], const float4 pj,
+                                                 const float4 fj, const PairCoef& k,
+                                                 f32x2 (&px)[I2], f32x2 (&py)[I2], f32x2 (&pz)[I2],
+                                                 float& mn) {
+    f32x2 dx[I2], dy[I2], dz[I2], r2[I2], inv[I2], inv2[I2], dF[I2], A[I2], Bd[I2];
+    const f32x2 xj = bc2(pj.x), yj = bc2(pj.y), zj = bc2(pj.z);
+    const f32x2 fx = bc2(fj.x), fy = bc2(fj.y), fz = bc2(fj.z);
+#pragma unroll
+    for (int m = 0; m < I2; ++m) dx[m] = sub2(xi[m], xj);
+#pragma unroll
+    for (int m = 0; m < I2; ++m) dy[m] = sub2(yi[m], yj);
+#pragma unroll
+    for (int m = 0; m < I2; ++m) dz[m] = sub2(zi[m], zj);
+#pragma unroll
+    for (int m = 0; m < I2; ++m) {
+        r2[m] = mul2(dx[m], dx[m]);
+        r2[m] = fma2(dy[m], dy[m], r2[m]);
+        r2[m] = fma2(dz[m], dz[m], r2[m]);
+    }
+#pragma unroll
+    for (int m = 0; m < I2; ++m) {
+        const float a = lo2(r2[m]), b = hi2(r2[m]);
+        mn = fminf(mn, fminf(a, b));
+        inv[m] = pk2(rsq_approx(a), rsq_approx(b));
+#if SD_RCP
+        inv2[m] = pk2(rcp_approx(a), rcp_approx(b));
+#endif
+    }
+#pragma unroll
+    for (int m = 0; m < I2; ++m) dF[m] = mul2(dx[m], fx);
+#pragma unroll
+    for (int m = 0; m < I2; ++m) dF[m] = fma2(dy[m], fy, dF[m]);
+#pragma unroll
+    for (int m = 0; m < I2; ++m) dF[m] = fma2(dz[m], fz, dF[m]);
+#pragma unroll
+    for (int m = 0; m < I2; ++m) {
+#if !SD_RCP
+        inv2[m] = mul2(inv[m], inv[m]);
+#endif
+        if (TENSOR == TENSOR_RPY) {
+            const f32x2 P = fma2(inv2[m], bc2(k.c2), bc2(k.c1));
+            const f32x2 Q = fma2(inv2[m], bc2(k.m3c2), bc2(k.c1));
+            A[m] = mul2(P, inv[m]);
+            const f32x2 t = mul2(inv2[m], dF[m]);
+            const f32x2 u = mul2(Q, t);
+            Bd[m] = mul2(u, inv[m]);
+        } else {
+            A[m] = mul2(inv[m], bc2(k.c1));
+            const f32x2 t = mul2(inv2[m], dF[m]);
+            Bd[m] = mul2(A[m], t);
+        }
+    }
+#pragma unroll
+    for (int m = 0; m < I2; ++m) px[m] = fma2(A[m], fx, px[m]);
+#pragma unroll
+    for (int m = 0; m < I2; ++m) py[m] = fma2(A[m], fy, py[m]);
+#pragma unroll
+    for (int m = 0; m < I2; ++m) pz[m] = fma2(A[m], fz, pz[m]);
+#pragma unroll
+    for (int m = 0; m < I2; ++m) {
+        px[m] = fma2(Bd[m], dx[m], px[m]);
+        py[m] = fma2(Bd[m], dy[m], py[m]);
+        pz[m] = fma2(Bd[m], dz[m], pz[m]);
+    }
 }
 
 // Exact body for one (i, j): self exclusion, coincident centres, overlap branch.
@@ -172,7 +314,7 @@ __device__ __forceinline__ void kahan_merge2(f32x2& s, f32x2& c, const f32x2 p) 
 }
 
 template <int I2, int TENSOR, int ACC>
-__global__ void __launch_bounds__(kThreads, (I2 <= 2) ? 2 : 1)
+__global__ void __launch_bounds__(kThreads, SD_MIN_BLOCKS(I2))
 pairs_f32_kernel(const float4* __restrict__ rec, float4* __restrict__ part, const Schedule sch,
                  const PairCoef k, const int N, const long long slot_stride) {
     constexpr int I = 2 * I2;
@@ -269,14 +411,30 @@ pairs_f32_kernel(const float4* __restrict__ rec, float4* __restrict__ part, cons
                     }
                 }
                 float mn = 3.0e38f;
-#pragma unroll 4
+                f32x2 det = bc2(0.f);
+#pragma unroll kUnrollJ
                 for (int jj = 0; jj < kChunk; ++jj) {
                     const float4 pj = cj[2 * jj];
                     const float4 fj = cj[2 * jj + 1];
+#if SD_STAGED
+                    pair_fast_staged<I2, TENSOR>(xi, yi, zi, pj, fj, k, px, py, pz, mn);
+#else
 #pragma unroll
                     for (int m = 0; m < I2; ++m)
-                        pair_fast2<TENSOR>(xi[m], yi[m], zi[m], pj, fj, k, px[m], py[m], pz[m], mn);
+                        pair_fast2<TENSOR>(xi[m], yi[m], zi[m], pj, fj, k, px[m], py[m], pz[m], mn, det);
+#endif
                 }
+#if SD_DETECT == 3
+                {   // NaN (self pair: inf - inf never occurs, inf does) and sums >= 1/thr^2
+                    const float dmax = fmaxf(lo2(det), hi2(det));
+                    if (!(dmax < k.det_thr)) mn = 0.f;
+                }
+#elif SD_DETECT == 4
+                {
+                    const float dmax = fmaxf(lo2(det), hi2(det));
+                    if (!(dmax < k.det_thr)) mn = 0.f;
+                }
+#endif
                 if (mn < k.thr) {
                     // an overlapping pair or the self pair sits in this chunk: redo it exactly
                     const int j0 = jbase + ch * kChunk;

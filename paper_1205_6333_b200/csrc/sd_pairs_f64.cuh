@@ -4,8 +4,9 @@
 // (sd_pairs_f32.cuh); differences:
 //  * 64-byte records {x, y, z, 0 | Fx, Fy, Fz, 0} of doubles, 64 j per 4 KiB tile;
 //  * no packed arithmetic (there is no DFMA2); one thread owns I particles;
-//  * 1/r: MUFU.RSQ on the fp32-rounded r^2 as a 22-bit seed, then two Newton steps in fp64
-//    (relative error ~1e-7 -> ~1e-14 -> rounding level); no fp64 division or sqrt in the loop;
+//  * 1/r: MUFU.RSQ on the fp32-rounded r^2 as a 22-bit seed, then one third-order (Halley) step
+//    in fp64 (relative error ~2e-7 -> ~1e-21, i.e. rounding level); no fp64 division or sqrt
+//    in the loop;
 //  * fp64 sums need no compensation (measured 2e-13 vs the oracle's long-double rows at
 //    N = 65536); min r^2 is tracked on the fp32 copy of r^2 that the seed needs anyway.
 #pragma once
@@ -16,14 +17,14 @@ namespace sd {
 
 constexpr int kTJ64 = 64;  // j records per tile (4 KiB)
 
+// y0 = MUFU.RSQ(float(r2)) has relative error e0 <~ 2^-22; one Halley step
+//   e = 1 - r2 y0^2 ,  y = y0 (1 + e/2 + 3 e^2/8)
+// leaves ~0.3 e0^3 ~ 1e-21, i.e. rounding level, in 5 fp64 instructions.
 __device__ __forceinline__ double rsqrt_nr2(const double r2, const float r2f) {
-    double y = static_cast<double>(rsq_approx(r2f));
-    const double h = 0.5 * r2;
-    double e = fma(-h * y, y, 0.5);
-    y = fma(y, e, y);
-    e = fma(-h * y, y, 0.5);
-    y = fma(y, e, y);
-    return y;
+    const double y = static_cast<double>(rsq_approx(r2f));
+    const double e = fma(-r2, y * y, 1.0);
+    const double p = fma(0.375, e, 0.5);
+    return fma(y * e, p, y);
 }
 
 template <int TENSOR>

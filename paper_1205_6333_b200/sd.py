@@ -42,6 +42,8 @@ SYMBOLS = {
     "sd_self_mobility": (_D, [_P]),
     "sd_launch_count": (_LL, [_P]),
     "sd_kernel_name": (ctypes.c_char_p, [_P]),
+    "sd_profile_enable": (_I, [_P, _I]),
+    "sd_profile_read": (_I, [_P, ctypes.POINTER(_D), ctypes.POINTER(_LL)]),
     "sd_fma_peak_probe": (_I, [_P, _I, ctypes.POINTER(_D), _P]),
     "sd_last_error": (ctypes.c_char_p, [_P]),
     "sd_destroy": (None, [_P]),
@@ -157,6 +159,15 @@ class Context:
         self._check(self._lib.sd_fma_peak_probe(self._h, int(precision), ctypes.byref(out),
                                                 _stream_ptr(stream)))
         return out.value
+
+    def profile_enable(self, on: bool = True):
+        self._check(self._lib.sd_profile_enable(self._h, 1 if on else 0))
+
+    def profile_read(self):
+        """(summed pair-kernel ms, launches) since the last read; waits for those launches."""
+        ms, cnt = ctypes.c_double(0.0), ctypes.c_longlong(0)
+        self._check(self._lib.sd_profile_read(self._h, ctypes.byref(ms), ctypes.byref(cnt)))
+        return ms.value, cnt.value
 
     @property
     def self_mobility(self) -> float:
