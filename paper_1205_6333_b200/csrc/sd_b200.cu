@@ -18,6 +18,7 @@
 #include "sd_common.cuh"
 #include "sd_pairs_f32.cuh"
 #include "sd_pairs_f64.cuh"
+#include "sd_small.cuh"
 #include "sd_stream.cuh"
 
 namespace {
@@ -52,6 +53,7 @@ struct sd_ctx {
     void* vel = nullptr;        // velocities of the last product
     void* pos_lo = nullptr;     // low words of the positions (fp32 modes)
     void* pos_half = nullptr;   // midpoint positions (for force callbacks)
+    void* pos_alt = nullptr;    // ping-pong partner of pos (small-N Euler)
     void* force_buf = nullptr;  // forces written by a callback
     void* stage_pos = nullptr;  // device staging of the _host entry point
     void* stage_force = nullptr;
@@ -96,7 +98,7 @@ const void* f64_kernel() {
 }
 
 void free_buffers(sd_ctx* c) {
-    void** bufs[] = {&c->rec,       &c->part,        &c->vel,       &c->pos_lo, &c->pos_half,
+    void** bufs[] = {&c->rec,       &c->part,        &c->vel,       &c->pos_lo, &c->pos_half, &c->pos_alt,
                      &c->force_buf, &c->stage_pos,   &c->stage_force, &c->stage_vel, &c->probe};
     for (void** b : bufs) {
         if (*b) cudaFree(*b);
@@ -119,28 +121,23 @@ sd_status configure(sd_ctx* c) {
     if (!f64) {
         const bool plain = c->precision == SD_PREC_F32_PLAIN;
         // particles per thread: 8 once there is enough work to balance 2048-particle i-blocks
-        // over the SMs (more operand reuse per j record); smaller i-blocks below that
-        const int i2 = (c->N >= 131072) ? 4 : (c->N > 8192) ? 2 : 1;
+        // over the SMs (more operand reuse per j record), 4 below that.  (N <= kSmallApplyMax
+        // never reaches this kernel: sd_small.cuh.)
+        const int i2 = (c->N >= 131072) ? 4 : 2;
         cfg.ipt = 2 * i2;
         cfg.TJ = sd::kTJ;
-        static const char* names[3][2][2] = {
-            {{"pairs_f32x2_i2_rpy_kahan", "pairs_f32x2_i2_rpy_plain"},
-             {"pairs_f32x2_i2_oseen_kahan", "pairs_f32x2_i2_oseen_plain"}},
+        static const char* names[2][2][2] = {
             {{"pairs_f32x2_i4_rpy_kahan", "pairs_f32x2_i4_rpy_plain"},
              {"pairs_f32x2_i4_oseen_kahan", "pairs_f32x2_i4_oseen_plain"}},
             {{"pairs_f32x2_i8_rpy_kahan", "pairs_f32x2_i8_rpy_plain"},
              {"pairs_f32x2_i8_oseen_kahan", "pairs_f32x2_i8_oseen_plain"}}};
-        const int v = (i2 == 1) ? 0 : (i2 == 2) ? 1 : 2;
-        cfg.name = names[v][rpy ? 0 : 1][plain ? 1 : 0];
+        cfg.name = names[i2 == 4 ? 1 : 0][rpy ? 0 : 1][plain ? 1 : 0];
         if (i2 == 4)
             cfg.kernel = rpy ? (plain ? f32_kernel<4, 0, 1>() : f32_kernel<4, 0, 0>())
                              : (plain ? f32_kernel<4, 1, 1>() : f32_kernel<4, 1, 0>());
-        else if (i2 == 2)
+        else
             cfg.kernel = rpy ? (plain ? f32_kernel<2, 0, 1>() : f32_kernel<2, 0, 0>())
                              : (plain ? f32_kernel<2, 1, 1>() : f32_kernel<2, 1, 0>());
-        else
-            cfg.kernel = rpy ? (plain ? f32_kernel<1, 0, 1>() : f32_kernel<1, 0, 0>())
-                             : (plain ? f32_kernel<1, 1, 1>() : f32_kernel<1, 1, 0>());
     } else {
         cfg.ipt = 2;
         cfg.TJ = sd::kTJ64;
@@ -180,6 +177,7 @@ sd_status configure(sd_ctx* c) {
     SD_CUDA(c, cudaMalloc(&c->vel, nrec * v4));
     SD_CUDA(c, cudaMalloc(&c->pos_lo, nrec * v4));
     SD_CUDA(c, cudaMalloc(&c->pos_half, nrec * v4));
+    SD_CUDA(c, cudaMalloc(&c->pos_alt, nrec * v4));
     SD_CUDA(c, cudaMalloc(&c->force_buf, nrec * v4));
     SD_CUDA(c, cudaMemset(c->pos_lo, 0, nrec * v4));
     SD_CUDA(c, cudaMemset(c->vel, 0, nrec * v4));
@@ -304,6 +302,96 @@ sd_status launch_finalize(sd_ctx* c, void* vel, void* pos, double dt, cudaStream
     return check_launch(c, "finalize_kernel");
 }
 
+// ---- small-N path (sd_small.cuh) -------------------------------------------------------------
+template <typename S>
+sd::CoefT<S> coef_of(const sd_ctx* c) {
+    const double a = c->a, mu0 = c->mu0;
+    sd::CoefT<S> k;
+    k.c1 = static_cast<S>(mu0 * 0.75 * a);
+    k.c2 = static_cast<S>(mu0 * 0.5 * a * a * a);
+    k.m3c2 = static_cast<S>(-1.5 * mu0 * a * a * a);
+    k.mu0 = static_cast<S>(mu0);
+    k.ovA = static_cast<S>(-9.0 * mu0 / (32.0 * a));
+    k.ovB = static_cast<S>(3.0 * mu0 / (32.0 * a));
+    k.four_a2 = static_cast<S>(4.0 * a * a);
+    return k;
+}
+
+template <typename T4, bool KAHAN>
+sd_status launch_small_apply_t(sd_ctx* c, const void* posx, const void* force, const double g[3],
+                               void* vel, const void* pos_base, void* pos_out, double dt, int mode,
+                               cudaStream_t st) {
+    typedef typename sd::Vec4<T4>::S S;
+    const int n = static_cast<int>(c->N);
+    const int ipw = (n > 2368) ? 2 : 1;  // one particle per warp while that leaves SMs idle
+    const int per_cta = (sd::kSmallThreads / 32) * ipw;
+    const int blocks = (n + per_cta - 1) / per_cta;
+    const sd::CoefT<S> k = coef_of<S>(c);
+    const double gx = g ? g[0] : 0.0, gy = g ? g[1] : 0.0, gz = g ? g[2] : 0.0;
+    const bool rpy = c->tensor == SD_TENSOR_RPY;
+#define SD_SMALL_LAUNCH(TEN, IPW)                                                                  \
+    sd::small_apply_kernel<T4, TEN, KAHAN, IPW><<<blocks, sd::kSmallThreads, 0, st>>>(             \
+        static_cast<const T4*>(posx), static_cast<const T4*>(force), gx, gy, gz,                   \
+        static_cast<T4*>(vel), static_cast<const T4*>(pos_base), static_cast<T4*>(c->pos_lo),      \
+        static_cast<T4*>(pos_out), dt, mode, k, n)
+    if (rpy) {
+        if (ipw == 2) SD_SMALL_LAUNCH(0, 2); else SD_SMALL_LAUNCH(0, 1);
+    } else {
+        if (ipw == 2) SD_SMALL_LAUNCH(1, 2); else SD_SMALL_LAUNCH(1, 1);
+    }
+#undef SD_SMALL_LAUNCH
+    return check_launch(c, "small_apply_kernel");
+}
+
+sd_status launch_small_apply(sd_ctx* c, const void* posx, const void* force, const double g[3],
+                             void* vel, const void* pos_base, void* pos_out, double dt, int mode,
+                             cudaStream_t st) {
+    if (c->precision == SD_PREC_F64)
+        return launch_small_apply_t<double4, false>(c, posx, force, g, vel, pos_base, pos_out, dt, mode, st);
+    if (c->precision == SD_PREC_F32_PLAIN)
+        return launch_small_apply_t<float4, false>(c, posx, force, g, vel, pos_base, pos_out, dt, mode, st);
+    return launch_small_apply_t<float4, true>(c, posx, force, g, vel, pos_base, pos_out, dt, mode, st);
+}
+
+template <typename T4, bool KAHAN>
+sd_status launch_stepper_t(sd_ctx* c, void* pos, const void* force, const double g[3], double dt,
+                           long long n_steps, int integrator, cudaStream_t st) {
+    typedef typename sd::Vec4<T4>::S S;
+    const int n = static_cast<int>(c->N);
+    const int sub = (n <= 32) ? 32 : 16;  // lanes per particle; n <= kStepperMax = 64
+    const int threads = (n * sub + 31) / 32 * 32;
+    const sd::CoefT<S> k = coef_of<S>(c);
+    const double gx = g ? g[0] : 0.0, gy = g ? g[1] : 0.0, gz = g ? g[2] : 0.0;
+    const bool rpy = c->tensor == SD_TENSOR_RPY;
+    // bounded launches: a kernel that runs for minutes is a hazard on shared boxes
+    const long long chunk = 1LL << 20;
+    for (long long done = 0; done < n_steps; done += chunk) {
+        const long long ns = std::min(chunk, n_steps - done);
+#define SD_STEP_LAUNCH(TEN, SUB)                                                                   \
+    sd::small_stepper_kernel<T4, TEN, KAHAN, SUB><<<1, threads, 0, st>>>(                          \
+        static_cast<T4*>(pos), static_cast<T4*>(c->pos_lo), static_cast<const T4*>(force), gx, gy, \
+        gz, static_cast<T4*>(c->vel), dt, ns, integrator, k, n)
+        if (rpy) {
+            if (sub == 32) SD_STEP_LAUNCH(0, 32); else SD_STEP_LAUNCH(0, 16);
+        } else {
+            if (sub == 32) SD_STEP_LAUNCH(1, 32); else SD_STEP_LAUNCH(1, 16);
+        }
+#undef SD_STEP_LAUNCH
+        sd_status s = check_launch(c, "small_stepper_kernel");
+        if (s != SD_OK) return s;
+    }
+    return SD_OK;
+}
+
+sd_status launch_stepper(sd_ctx* c, void* pos, const void* force, const double g[3], double dt,
+                         long long n_steps, int integrator, cudaStream_t st) {
+    if (c->precision == SD_PREC_F64)
+        return launch_stepper_t<double4, false>(c, pos, force, g, dt, n_steps, integrator, st);
+    if (c->precision == SD_PREC_F32_PLAIN)
+        return launch_stepper_t<float4, false>(c, pos, force, g, dt, n_steps, integrator, st);
+    return launch_stepper_t<float4, true>(c, pos, force, g, dt, n_steps, integrator, st);
+}
+
 bool misaligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) & (a - 1)) != 0; }
 
 }  // namespace
@@ -376,6 +464,8 @@ sd_status sd_mobility_apply(sd_ctx* ctx, const void* pos, const void* force, voi
         return fail(ctx, SD_ERR_INVALID_ARG, "sd_mobility_apply: records must be 16-byte (float) / 32-byte (double) aligned");
     if (vel == pos || vel == force) return fail(ctx, SD_ERR_INVALID_ARG, "sd_mobility_apply: vel aliases an input");
     cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (ctx->N <= sd::kSmallApplyMax)  // small-N path: one launch, no pack / partials / finalize
+        return launch_small_apply(ctx, pos, force, nullptr, vel, nullptr, nullptr, 0.0, sd::FIN_VEL, st);
     sd_status s = launch_pack(ctx, pos, force, sd::PACK_POS | sd::PACK_FORCE, nullptr, st);
     if (s != SD_OK) return s;
     s = launch_pairs(ctx, st);
@@ -424,6 +514,36 @@ sd_status sd_step(sd_ctx* ctx, void* pos, sd_force_fn fn, void* user, const void
         SD_CUDA(ctx, cudaMemsetAsync(ctx->pos_lo, 0, static_cast<size_t>(ctx->Nrec) * al, st));
         ctx->lo_valid = true;
     }
+    if (!fn && ctx->N <= sd::kStepperMax)  // all steps in one launch
+        return launch_stepper(ctx, pos, force, gravity, dt, n_steps, integrator, st);
+    if (ctx->N <= sd::kSmallApplyMax) {    // one launch per product
+        const void* fptr = fn ? ctx->force_buf : force;
+        const double* g = (fn || force) ? nullptr : gravity;
+        void* cur = pos;
+        void* other = ctx->pos_alt;
+        for (long long step = 0; step < n_steps; ++step) {
+            if (integrator == SD_INT_EULER) {
+                if (fn && fn(cur, ctx->force_buf, ctx->N, user, stream) != 0)
+                    return fail(ctx, SD_ERR_INVALID_ARG, "sd_step: force callback failed");
+                s = launch_small_apply(ctx, cur, fptr, g, ctx->vel, cur, other, dt, sd::FIN_EULER, st);
+                if (s != SD_OK) return s;
+                std::swap(cur, other);
+            } else {
+                if (fn && fn(pos, ctx->force_buf, ctx->N, user, stream) != 0)
+                    return fail(ctx, SD_ERR_INVALID_ARG, "sd_step: force callback failed");
+                s = launch_small_apply(ctx, pos, fptr, g, ctx->vel, pos, ctx->pos_half, dt, sd::FIN_HALF, st);
+                if (s != SD_OK) return s;
+                if (fn && fn(ctx->pos_half, ctx->force_buf, ctx->N, user, stream) != 0)
+                    return fail(ctx, SD_ERR_INVALID_ARG, "sd_step: force callback failed");
+                s = launch_small_apply(ctx, ctx->pos_half, fptr, g, ctx->vel, pos, pos, dt, sd::FIN_FULL, st);
+                if (s != SD_OK) return s;
+            }
+        }
+        if (cur != pos)
+            SD_CUDA(ctx, cudaMemcpyAsync(pos, cur, static_cast<size_t>(ctx->N) * al,
+                                         cudaMemcpyDeviceToDevice, st));
+        return SD_OK;
+    }
     // constant forces are packed once; callback forces before every product
     const int force_what = fn ? 0 : (force ? sd::PACK_FORCE : sd::PACK_GRAVITY);
     s = launch_pack(ctx, pos, force, sd::PACK_POS | force_what, gravity, st);
@@ -469,7 +589,12 @@ sd_status sd_reset_compensation(sd_ctx* ctx, void* stream) {
 long long sd_num_particles(const sd_ctx* ctx) { return ctx ? ctx->N : 0; }
 double sd_self_mobility(const sd_ctx* ctx) { return ctx ? ctx->mu0 : 0.0; }
 long long sd_launch_count(const sd_ctx* ctx) { return ctx ? ctx->launches : 0; }
-const char* sd_kernel_name(const sd_ctx* ctx) { return ctx ? ctx->cfg.name : ""; }
+const char* sd_kernel_name(const sd_ctx* ctx) {
+    if (!ctx) return "";
+    if (ctx->N <= sd::kSmallApplyMax)
+        return ctx->precision == SD_PREC_F64 ? "small_apply_f64" : "small_apply_f32";
+    return ctx->cfg.name;
+}
 
 sd_status sd_profile_enable(sd_ctx* ctx, int on) {
     if (!ctx) return fail(nullptr, SD_ERR_INVALID_ARG, "sd_profile_enable: ctx is NULL");

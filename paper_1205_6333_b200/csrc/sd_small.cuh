@@ -1,0 +1,285 @@
+// sd_small.cuh -- the small-N path (below a few thousand
+// particles the device is under-filled and the run time is linear in N).
+//
+// For small N the all-pairs arithmetic is microseconds; what counts is the number of launches and
+// how many SMs get work.  Two kernels, both evaluating every pair with the exact branching body
+// (self exclusion, coincident centres, r < 2a branch) -- no fast/slow split is worth it here:
+//
+//  small_apply_kernel   N <= kSmallApplyMax.  ONE launch per product, straight from the caller's
+//      pos/force arrays (no pack, no partial buffer, no finalize).  A warp owns IPW particles i
+//      and its 32 lanes split j (lane l takes j = l, l+32, ...); j tiles of 256 records are staged
+//      in shared memory by the whole CTA; per-lane Kahan sums are combined by warp shuffles of the
+//      3-vector in fp64; lane 0 adds mu0 F_i, writes vel and applies the fused integrator update
+//      (Euler needs ping-pong position buffers, the midpoint stages do not).
+//      Grid = N / (8 IPW) CTAs, IPW chosen so that every SM gets a CTA as early as possible.
+//
+//  small_stepper_kernel N <= kStepperMax, constant forces.  ONE launch for n_steps steps: a
+//      single CTA keeps the positions in shared memory (fp64 = hi + lo of the fp32 modes), S lanes
+//      per particle split j, shuffle reduction, two block barriers per product.  Removes the
+//      launch latency (~10 us per 4-launch step) that dominates N = 4 (config 1) and makes the
+//      5e7-step stability runs of PAPER.md:253 a matter of seconds.
+#pragma once
+#include "sd_common.cuh"
+#include "sd_pairs_f32.cuh"
+#include "sd_stream.cuh"
+
+namespace sd {
+
+constexpr int kSmallApplyMax = 4096;  // above this the tiled packed kernel wins (measured)
+constexpr int kStepperMax = 64;   // above this one launch per product is faster (measured)
+constexpr int kSmallThreads = 256;
+constexpr int kSmallTile = 256;
+
+template <typename S>
+struct CoefT {
+    S c1, c2, m3c2, mu0, ovA, ovB, four_a2;
+};
+
+__device__ __forceinline__ float inv_sqrt_exact(float r2) {
+    float y = rsq_approx(r2);
+    // one Newton step: the small path is not throughput-bound, take the extra bits
+    const float e = fmaf(-r2 * y, y, 1.0f);
+    return fmaf(0.5f * y, e, y);
+}
+__device__ __forceinline__ double inv_sqrt_exact(double r2) { return 1.0 / sqrt(r2); }
+
+// One exact pair term added to (px, py, pz); `self` pairs are skipped.
+template <typename S, int TENSOR>
+__device__ __forceinline__ void pair_term(const S xi, const S yi, const S zi, const bool self,
+                                          const S xj, const S yj, const S zj, const S fx,
+                                          const S fy, const S fz, const CoefT<S>& k, S& px, S& py,
+                                          S& pz) {
+    if (self) return;
+    const S dx = xi - xj, dy = yi - yj, dz = zi - zj;
+    const S r2 = dx * dx + dy * dy + dz * dz;
+    if (r2 == S(0)) {
+        if (TENSOR == TENSOR_RPY) {
+            px += k.mu0 * fx;
+            py += k.mu0 * fy;
+            pz += k.mu0 * fz;
+        }
+        return;
+    }
+    const S inv = inv_sqrt_exact(r2);
+    const S dF = dx * fx + dy * fy + dz * fz;
+    S A, B;
+    if (TENSOR == TENSOR_RPY) {
+        if (r2 < k.four_a2) {
+            const S r = r2 * inv;
+            A = k.mu0 + k.ovA * r;
+            B = k.ovB * inv;
+        } else {
+            const S inv2 = inv * inv;
+            A = (k.c1 + k.c2 * inv2) * inv;
+            B = (k.c1 + k.m3c2 * inv2) * inv2 * inv;
+        }
+    } else {
+        A = k.c1 * inv;
+        B = A * inv * inv;
+    }
+    const S Bd = B * dF;
+    px += A * fx + Bd * dx;
+    py += A * fy + Bd * dy;
+    pz += A * fz + Bd * dz;
+}
+
+// Kahan (KAHAN = true) or plain running sum of 3-vectors.
+template <typename S, bool KAHAN>
+struct Acc3 {
+    S sx = S(0), sy = S(0), sz = S(0), cx = S(0), cy = S(0), cz = S(0);
+    __device__ __forceinline__ void add(const S tx, const S ty, const S tz) {
+        if (KAHAN) {
+            S y = tx - cx, t = sx + y;
+            cx = (t - sx) - y;
+            sx = t;
+            y = ty - cy, t = sy + y;
+            cy = (t - sy) - y;
+            sy = t;
+            y = tz - cz, t = sz + y;
+            cz = (t - sz) - y;
+            sz = t;
+        } else {
+            sx += tx;
+            sy += ty;
+            sz += tz;
+        }
+    }
+    __device__ __forceinline__ void value(double& x, double& y, double& z) const {
+        x = static_cast<double>(sx) - static_cast<double>(cx);
+        y = static_cast<double>(sy) - static_cast<double>(cy);
+        z = static_cast<double>(sz) - static_cast<double>(cz);
+    }
+};
+
+template <int WIDTH>
+__device__ __forceinline__ double lanes_sum(double v) {
+#pragma unroll
+    for (int o = WIDTH / 2; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o, WIDTH);
+    return v;
+}
+
+// ---- one product per launch -----------------------------------------------------------------
+// posx: positions the distances are taken from; force: per-particle forces or NULL (uniform g).
+// MODE (sd_stream.cuh, run-time): FIN_VEL writes vel only; otherwise pos_base (+ pos_lo) + h v
+// -> pos_out.
+template <typename T4, int TENSOR, bool KAHAN, int IPW>
+__global__ void __launch_bounds__(kSmallThreads)
+small_apply_kernel(const T4* __restrict__ posx, const T4* __restrict__ force, const double gx,
+                   const double gy, const double gz, T4* __restrict__ vel,
+                   const T4* __restrict__ pos_base, T4* __restrict__ pos_lo,
+                   T4* __restrict__ pos_out, const double dt, const int MODE,
+                   const CoefT<typename Vec4<T4>::S> k, const int N) {
+    typedef typename Vec4<T4>::S S;
+    __shared__ T4 sp[kSmallTile];
+    __shared__ T4 sf[kSmallTile];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int i0 = (blockIdx.x * (kSmallThreads / 32) + warp) * IPW;
+    S xi[IPW], yi[IPW], zi[IPW];
+    Acc3<S, KAHAN> acc[IPW];
+#pragma unroll
+    for (int m = 0; m < IPW; ++m) {
+        const int i = min(i0 + m, N - 1);
+        const T4 p = posx[i];
+        xi[m] = p.x;
+        yi[m] = p.y;
+        zi[m] = p.z;
+    }
+    for (int j0 = 0; j0 < N; j0 += kSmallTile) {
+        const int j = j0 + tid;
+        if (j < N) {
+            sp[tid] = posx[j];
+            sf[tid] = force ? force[j] : Vec4<T4>::make(S(gx), S(gy), S(gz), S(0));
+        }
+        __syncthreads();
+        const int nj = min(kSmallTile, N - j0);
+        for (int jj = lane; jj < nj; jj += 32) {
+            const T4 pj = sp[jj];
+            const T4 fj = sf[jj];
+#pragma unroll
+            for (int m = 0; m < IPW; ++m) {
+                S tx = S(0), ty = S(0), tz = S(0);
+                pair_term<S, TENSOR>(xi[m], yi[m], zi[m], (j0 + jj) == (i0 + m), pj.x, pj.y, pj.z,
+                                     fj.x, fj.y, fj.z, k, tx, ty, tz);
+                acc[m].add(tx, ty, tz);
+            }
+        }
+        __syncthreads();
+    }
+#pragma unroll
+    for (int m = 0; m < IPW; ++m) {
+        double vx, vy, vz;
+        acc[m].value(vx, vy, vz);
+        vx = lanes_sum<32>(vx);
+        vy = lanes_sum<32>(vy);
+        vz = lanes_sum<32>(vz);
+        const int i = i0 + m;
+        if (lane == 0 && i < N) {
+            double fx = gx, fy = gy, fz = gz;
+            if (force) {
+                const T4 f = force[i];
+                fx = f.x, fy = f.y, fz = f.z;
+            }
+            const double mu0 = static_cast<double>(k.mu0);
+            vx += mu0 * static_cast<double>(S(fx));
+            vy += mu0 * static_cast<double>(S(fy));
+            vz += mu0 * static_cast<double>(S(fz));
+            vel[i] = Vec4<T4>::make(S(vx), S(vy), S(vz), S(0));
+            if (MODE != FIN_VEL) {
+                const T4 ph = pos_base[i];
+                double X = ph.x, Y = ph.y, Z = ph.z;
+                if (sizeof(S) == 4) {
+                    const T4 pl = pos_lo[i];
+                    X += pl.x, Y += pl.y, Z += pl.z;
+                }
+                const double h = (MODE == FIN_HALF) ? 0.5 * dt : dt;
+                X += h * vx, Y += h * vy, Z += h * vz;
+                const S xh = S(X), yh = S(Y), zh = S(Z);
+                pos_out[i] = Vec4<T4>::make(xh, yh, zh, S(0));
+                if (MODE != FIN_HALF && sizeof(S) == 4)
+                    pos_lo[i] = Vec4<T4>::make(S(X - static_cast<double>(xh)),
+                                               S(Y - static_cast<double>(yh)),
+                                               S(Z - static_cast<double>(zh)), S(0));
+            }
+        }
+    }
+}
+
+// ---- all steps in one launch ------------------------------------------------------------------
+// One CTA of N * SUB threads (SUB lanes per particle, SUB | 32).  Positions live in shared memory
+// as doubles (= hi + lo of the fp32 modes); the pair arithmetic runs in S on S-rounded positions,
+// exactly like the large-N path.  integrator: 0 Euler, 1 midpoint.
+template <typename T4, int TENSOR, bool KAHAN, int SUB>
+__global__ void __launch_bounds__(1024)
+small_stepper_kernel(T4* __restrict__ pos, T4* __restrict__ pos_lo, const T4* __restrict__ force,
+                     const double gx, const double gy, const double gz, T4* __restrict__ vel,
+                     const double dt, const long long n_steps, const int integrator,
+                     const CoefT<typename Vec4<T4>::S> k, const int N) {
+    typedef typename Vec4<T4>::S S;
+    __shared__ double P[kStepperMax][3];   // current positions r_n
+    __shared__ S X[kStepperMax][3];        // positions the distances are taken from (S-rounded)
+    __shared__ S F[kStepperMax][3];
+    const int tid = threadIdx.x;
+    const int i = tid / SUB, sub = tid % SUB;
+    const bool owner = (sub == 0) && (i < N);
+    if (owner) {
+        const T4 p = pos[i];
+        double x = p.x, y = p.y, z = p.z;
+        if (sizeof(S) == 4) {
+            const T4 l = pos_lo[i];
+            x += l.x, y += l.y, z += l.z;
+        }
+        P[i][0] = x, P[i][1] = y, P[i][2] = z;
+        X[i][0] = S(x), X[i][1] = S(y), X[i][2] = S(z);
+        if (force) {
+            const T4 f = force[i];
+            F[i][0] = f.x, F[i][1] = f.y, F[i][2] = f.z;
+        } else {
+            F[i][0] = S(gx), F[i][1] = S(gy), F[i][2] = S(gz);
+        }
+    }
+    __syncthreads();
+    const double mu0 = static_cast<double>(k.mu0);
+    double vx = 0.0, vy = 0.0, vz = 0.0;
+    const int n_products = (integrator == 1) ? 2 : 1;
+    for (long long step = 0; step < n_steps; ++step) {
+        for (int stage = 0; stage < n_products; ++stage) {
+            Acc3<S, KAHAN> acc;
+            if (i < N) {
+                const S xi = X[i][0], yi = X[i][1], zi = X[i][2];
+                for (int j = sub; j < N; j += SUB) {
+                    S tx = S(0), ty = S(0), tz = S(0);
+                    pair_term<S, TENSOR>(xi, yi, zi, j == i, X[j][0], X[j][1], X[j][2], F[j][0],
+                                         F[j][1], F[j][2], k, tx, ty, tz);
+                    acc.add(tx, ty, tz);
+                }
+            }
+            acc.value(vx, vy, vz);
+            vx = lanes_sum<SUB>(vx);
+            vy = lanes_sum<SUB>(vy);
+            vz = lanes_sum<SUB>(vz);
+            __syncthreads();  // every lane has read X
+            if (owner) {
+                vx += mu0 * static_cast<double>(F[i][0]);
+                vy += mu0 * static_cast<double>(F[i][1]);
+                vz += mu0 * static_cast<double>(F[i][2]);
+                const bool half = (n_products == 2) && (stage == 0);
+                const double h = half ? 0.5 * dt : dt;
+                const double x = P[i][0] + h * vx, y = P[i][1] + h * vy, z = P[i][2] + h * vz;
+                X[i][0] = S(x), X[i][1] = S(y), X[i][2] = S(z);
+                if (!half) P[i][0] = x, P[i][1] = y, P[i][2] = z;
+            }
+            __syncthreads();
+        }
+    }
+    if (owner) {
+        const S xh = S(P[i][0]), yh = S(P[i][1]), zh = S(P[i][2]);
+        pos[i] = Vec4<T4>::make(xh, yh, zh, S(0));
+        if (sizeof(S) == 4)
+            pos_lo[i] = Vec4<T4>::make(S(P[i][0] - static_cast<double>(xh)),
+                                       S(P[i][1] - static_cast<double>(yh)),
+                                       S(P[i][2] - static_cast<double>(zh)), S(0));
+        vel[i] = Vec4<T4>::make(S(vx), S(vy), S(vz), S(0));
+    }
+}
+
+}  // namespace sd
