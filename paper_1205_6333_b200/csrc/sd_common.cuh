@@ -2,7 +2,8 @@
 // the static work schedule and the packed-particle record layout.
 //
 // Data layout in HBM (all context-owned):
-//   rec32 : [Nrec][2] float4  = { x, y, z, 0 | Fx, Fy, Fz, 0 }   one 32-byte record per particle,
+//   rec32 : [Nrec][2] float4  = { x, y, z, 0 | c1 Fx, c1 Fy, c1 Fz, 0 }  one 32-byte record per
+//           particle (c1 = mu0 3a/4 folded into the force, see PairCoefT below),
 //   rec64 : [Nrec][2] double4 = same in fp64 (64 bytes),
 //           the paper's "32 bytes per particle (2 x float4)" record.  Nrec is N
 //           rounded up to SD_REC_ALIGN; pad records sit at SD_PAD_POS with zero force, so they
@@ -75,19 +76,21 @@ struct Schedule {
     int G;                     // CTAs
 };
 
-struct PairCoef {
-    float c1;     // mu0 * 3a/4          (Oseen / RP 1/r coefficient)
-    float c2;     // mu0 * a^3/2         (RP 1/r^3 coefficient)
-    float m3c2;   // -3 * c2
-    float mu0;    // 1/(6 pi eta a)
-    float ovA;    // -9 mu0 / (32 a)     overlap branch: A = mu0 + ovA * r
-    float ovB;    // 3 mu0 / (32 a)      overlap branch: B = ovB / r
-    float thr;    // slow-path threshold on r^2: 4a^2 for RPY, tiny for Oseen (only r == 0)
-    float det_thr;  // same threshold for the summed detector (SD_DETECT 3: 1/thr^2, 4: 1/thr)
+// Coefficients of the pair kernels in "folded" units: the force lane of a record holds
+// F' = c1 F with c1 = mu0 3a/4 (the 1/r coefficient of Eq. 4 / 7b), so that
+//   far field  T.F = (1/r + k2/r^3) F' + (1 - 3 k2/r^2)/r^3 (d.F') d ,   k2 = (a^3/2)/(3a/4) = 2a^2/3
+//   overlap    T.F = (mu0r + ovA r) F' + (ovB/r) (d.F') d                (A4)
+// and every coefficient depends on a only.
+template <typename S>
+struct PairCoefT {
+    S k2;     // 2 a^2 / 3
+    S m3k2;   // -2 a^2
+    S mu0r;   // mu0 / c1 = 4 / (3a)      (coincident centres; self term in the finalize kernel)
+    S ovA;    // -3 / (8 a^2)             overlap branch: A = mu0r + ovA * r
+    S ovB;    // 1 / (8 a^2)              overlap branch: B = ovB / r
+    S thr;    // slow-path threshold on r^2: 4a^2 for RPY, tiny for Oseen (only r == 0)
 };
-
-struct PairCoef64 {
-    double c1, c2, m3c2, mu0, ovA, ovB, four_a2;
-};
+typedef PairCoefT<float> PairCoef;
+typedef PairCoefT<double> PairCoef64;
 
 }  // namespace sd

@@ -11,8 +11,13 @@
 //  * j data (32-byte records) are staged in shared memory by 1-D bulk async copies
 //    (cp.async.bulk + mbarrier transaction counts) in a kStages-deep ring; every lane reads the
 //    same record (LDS.128 broadcast), so there are no bank conflicts by construction;
-//  * 1/r and 1/r^2 come from MUFU.RSQ and MUFU.RCP (the XU pipe is otherwise idle); the
-//    coefficients need FMUL/FFMA only: 21 packed FP32 instructions per two pairs (RPY);
+//  * the 1/r coefficient c1 = mu0 3a/4 is folded into the force lane of the records
+//    (F' = c1 F, written by the pack / finalize kernels), so the far-field tensor becomes
+//        T(d).F = A' F' + B' (d.F') d ,  A' = 1/r + k2/r^3 ,  B' = (1 - 3 k2/r^2)/r^3 ,
+//    k2 = c2/c1 = 2a^2/3: the coefficients depend on a only and cost 5 packed instructions;
+//  * 1/r and 1/r^2 come from MUFU.RSQ and MUFU.RCP (two MUFU issue as cheaply as the packed
+//    multiply they replace); everything else is FMUL2/FFMA2/FADD2: 20 packed FP32 instructions
+//    per two pairs (Rotne-Prager), 17 (Oseen);
 //  * accumulation (terms of very different magnitude): plain fp32 adds inside a
 //    chunk of kChunk consecutive j, Kahan merge of the chunk sum into (s, c) per particle;
 //  * the r < 2a branch and the j == i exclusion are NOT evaluated per pair: the fast body
@@ -23,38 +28,15 @@
 #pragma once
 #include "sd_common.cuh"
 
-// Tuning knobs (defaults are the shipped configuration; the experiment harness overrides them)
-#ifndef SD_THREADS
-#define SD_THREADS 256
-#endif
-#ifndef SD_UNROLL_J
-#define SD_UNROLL_J 4
-#endif
-#ifndef SD_ACC_ORDER
-#define SD_ACC_ORDER 0
-#endif
-#ifndef SD_RCP
-#define SD_RCP 1      // 1: 1/r^2 from MUFU.RCP instead of inv*inv (one packed multiply less)
-#endif
-#ifndef SD_DETECT
-#define SD_DETECT 0   // how the chunk-level overlap/self detector is fed (see pair_fast2)
-#endif
-#ifndef SD_STAGED
-#define SD_STAGED 1
-#endif
-#ifndef SD_MIN_BLOCKS
-#define SD_MIN_BLOCKS(I2) (((I2) <= 2) ? 2 : 1)
-#endif
-
 namespace sd {
 
-constexpr int kThreads = SD_THREADS;
+constexpr int kThreads = 256;
 constexpr int kWarps = kThreads / 32;
 constexpr int kTJ = 128;     // j records per tile (4 KiB)
 constexpr int kStages = 4;   // ring depth
 constexpr int kPrefetch = 2; // tiles in flight ahead of the one being consumed
 constexpr int kChunk = 32;   // j per compensation chunk
-constexpr int kUnrollJ = SD_UNROLL_J;
+constexpr int kUnrollJ = 4;  // j per unrolled loop body
 
 enum { TENSOR_RPY = 0, TENSOR_OSEEN = 1 };
 enum { ACC_KAHAN = 0, ACC_PLAIN = 1 };
@@ -111,91 +93,12 @@ __device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b) {
     return d;
 }
 
-// Far-field body for two particles i (packed) against one j.  21 packed FP32 instructions + 4
-// MUFU for Rotne-Prager, 18 + 4 for Oseen (one more packed multiply and 2 MUFU with SD_RCP 0).
-template <int TENSOR>
-__device__ __forceinline__ void pair_fast2(const f32x2 xi, const f32x2 yi, const f32x2 zi,
-                                           const float4 pj, const float4 fj, const PairCoef& k,
-                                           f32x2& px, f32x2& py, f32x2& pz, float& mn,
-                                           f32x2& det) {
-    const f32x2 dx = sub2(xi, bc2(pj.x));
-    const f32x2 dy = sub2(yi, bc2(pj.y));
-    const f32x2 dz = sub2(zi, bc2(pj.z));
-    f32x2 r2 = mul2(dx, dx);
-    r2 = fma2(dy, dy, r2);
-    r2 = fma2(dz, dz, r2);
-    const float r2a = lo2(r2), r2b = hi2(r2);
-#ifndef SD_EXP_NOMIN
-#if SD_DETECT == 0
-    mn = fminf(mn, fminf(r2a, r2b));
-#elif SD_DETECT == 1
-    mn = fminf(mn, r2a);
-    mn = fminf(mn, r2b);
-#elif SD_DETECT == 2
-    if (r2a < k.thr) mn = 0.f;
-    if (r2b < k.thr) mn = 0.f;
-#endif
-#endif
-#ifndef SD_EXP_NOMUFU
-    const f32x2 inv = pk2(rsq_approx(r2a), rsq_approx(r2b));
-#else
-    const f32x2 inv = mul2(r2, bc2(1e-3f));
-#endif
-    const f32x2 fx = bc2(fj.x), fy = bc2(fj.y), fz = bc2(fj.z);
-    f32x2 dF = mul2(dx, fx);
-    dF = fma2(dy, fy, dF);
-    dF = fma2(dz, fz, dF);
-#if SD_RCP
-    const f32x2 inv2 = pk2(rcp_approx(r2a), rcp_approx(r2b));
-#else
-    const f32x2 inv2 = mul2(inv, inv);
-#endif
-#if SD_DETECT == 3
-    det = fma2(inv2, inv2, det);   // sum of 1/r^4 >= max of 1/r^4: never misses an overlap
-#elif SD_DETECT == 4
-    det = add2(det, inv2);
-#endif
-    f32x2 A, Bd;
-    if (TENSOR == TENSOR_RPY) {
-        const f32x2 P = fma2(inv2, bc2(k.c2), bc2(k.c1));    // c1 + c2/r^2
-        const f32x2 Q = fma2(inv2, bc2(k.m3c2), bc2(k.c1));  // c1 - 3 c2/r^2
-        A = mul2(P, inv);                                    // c1/r + c2/r^3
-        const f32x2 t = mul2(inv2, dF);                      // (d.F)/r^2
-        const f32x2 u = mul2(Q, t);
-        Bd = mul2(u, inv);                                   // B (d.F)
-    } else {
-        A = mul2(inv, bc2(k.c1));                            // c1/r
-        const f32x2 t = mul2(inv2, dF);
-        Bd = mul2(A, t);                                     // c1 (d.F)/r^3
-    }
-#if SD_ACC_ORDER == 0
-    px = fma2(A, fx, px);
-    py = fma2(A, fy, py);
-    pz = fma2(A, fz, pz);
-    px = fma2(Bd, dx, px);
-    py = fma2(Bd, dy, py);
-    pz = fma2(Bd, dz, pz);
-#elif SD_ACC_ORDER == 1
-    px = fma2(A, fx, px);
-    px = fma2(Bd, dx, px);
-    py = fma2(A, fy, py);
-    py = fma2(Bd, dy, py);
-    pz = fma2(A, fz, pz);
-    pz = fma2(Bd, dz, pz);
-#else
-    // fold A F + Bd d into a temporary first: one accumulator read per component
-    const f32x2 tx = fma2(Bd, dx, mul2(A, fx));
-    const f32x2 ty = fma2(Bd, dy, mul2(A, fy));
-    const f32x2 tz = fma2(Bd, dz, mul2(A, fz));
-    px = add2(px, tx);
-    py = add2(py, ty);
-    pz = add2(pz, tz);
-#endif
-}
-
-// The same body for all I2 packed groups of a thread against one j, written stage by stage so
-// that consecutive instructions share the broadcast j operand (operand-reuse cache) -- the
-// register file, not the FMA pipe, is the binding resource of this kernel.
+// Far-field body for the I2 packed groups of a thread (2*I2 particles i) against one j, written
+// stage by stage so that consecutive instructions share the broadcast j operand (operand-reuse
+// cache): the register-file read ports, not the FMA pipe, are the binding resource (an FFMA2
+// with three distinct register operands in one bank takes 3 cycles instead of 2).
+// 20 packed FP32 instructions + 4 MUFU per two pairs for Rotne-Prager, 17 + 4 for Oseen.
+// fj holds F' = c1 F (see the file header); k.k2 = 2a^2/3, k.m3k2 = -2a^2.
 template <int I2, int TENSOR>
 __device__ __forceinline__ void pair_fast_staged(const f32x2 (&xi)[I2], const f32x2 (&yi)[I2],
                                                  const f32x2 (&zi)[I2], const float4 pj,
@@ -222,9 +125,7 @@ __device__ __forceinline__ void pair_fast_staged(const f32x2 (&xi)[I2], const f3
         const float a = lo2(r2[m]), b = hi2(r2[m]);
         mn = fminf(mn, fminf(a, b));
         inv[m] = pk2(rsq_approx(a), rsq_approx(b));
-#if SD_RCP
         inv2[m] = pk2(rcp_approx(a), rcp_approx(b));
-#endif
     }
 #pragma unroll
     for (int m = 0; m < I2; ++m) dF[m] = mul2(dx[m], fx);
@@ -234,20 +135,15 @@ __device__ __forceinline__ void pair_fast_staged(const f32x2 (&xi)[I2], const f3
     for (int m = 0; m < I2; ++m) dF[m] = fma2(dz[m], fz, dF[m]);
 #pragma unroll
     for (int m = 0; m < I2; ++m) {
-#if !SD_RCP
-        inv2[m] = mul2(inv[m], inv[m]);
-#endif
+        const f32x2 inv3 = mul2(inv[m], inv2[m]);
         if (TENSOR == TENSOR_RPY) {
-            const f32x2 P = fma2(inv2[m], bc2(k.c2), bc2(k.c1));
-            const f32x2 Q = fma2(inv2[m], bc2(k.m3c2), bc2(k.c1));
-            A[m] = mul2(P, inv[m]);
-            const f32x2 t = mul2(inv2[m], dF[m]);
-            const f32x2 u = mul2(Q, t);
-            Bd[m] = mul2(u, inv[m]);
+            A[m] = fma2(inv3, bc2(k.k2), inv[m]);                          // 1/r + k2/r^3
+            const f32x2 g = mul2(inv3, dF[m]);                             // (d.F')/r^3
+            const f32x2 Q = fma2(inv2[m], bc2(k.m3k2), bc2(1.0f));         // 1 - 3 k2/r^2
+            Bd[m] = mul2(g, Q);                                            // B' (d.F')
         } else {
-            A[m] = mul2(inv[m], bc2(k.c1));
-            const f32x2 t = mul2(inv2[m], dF[m]);
-            Bd[m] = mul2(A[m], t);
+            A[m] = inv[m];                                                 // 1/r
+            Bd[m] = mul2(inv3, dF[m]);                                     // (d.F')/r^3
         }
     }
 #pragma unroll
@@ -264,7 +160,8 @@ __device__ __forceinline__ void pair_fast_staged(const f32x2 (&xi)[I2], const f3
     }
 }
 
-// Exact body for one (i, j): self exclusion, coincident centres, overlap branch.
+// Exact body for one (i, j): self exclusion, coincident centres, overlap branch (A4,
+// A5), in the same folded units as the fast body (fj = c1 F_j, coefficients relative to c1).
 template <int TENSOR>
 __device__ __forceinline__ void pair_exact(const float xi, const float yi, const float zi,
                                            const bool self, const float4 pj, const float4 fj,
@@ -274,9 +171,9 @@ __device__ __forceinline__ void pair_exact(const float xi, const float yi, const
     const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
     if (r2 == 0.0f) {
         if (TENSOR == TENSOR_RPY) {  // limit of the overlap branch: mu0 F_j
-            px = fmaf(k.mu0, fj.x, px);
-            py = fmaf(k.mu0, fj.y, py);
-            pz = fmaf(k.mu0, fj.z, pz);
+            px = fmaf(k.mu0r, fj.x, px);
+            py = fmaf(k.mu0r, fj.y, py);
+            pz = fmaf(k.mu0r, fj.z, pz);
         }
         return;
     }
@@ -286,16 +183,17 @@ __device__ __forceinline__ void pair_exact(const float xi, const float yi, const
     if (TENSOR == TENSOR_RPY) {
         if (r2 < k.thr) {  // r < 2a
             const float r = r2 * inv;
-            A = fmaf(k.ovA, r, k.mu0);
+            A = fmaf(k.ovA, r, k.mu0r);
             B = k.ovB * inv;
         } else {
             const float inv2 = inv * inv;
-            A = fmaf(k.c2, inv2, k.c1) * inv;
-            B = fmaf(k.m3c2, inv2, k.c1) * inv2 * inv;
+            const float inv3 = inv2 * inv;
+            A = fmaf(k.k2, inv3, inv);
+            B = fmaf(k.m3k2, inv2, 1.0f) * inv3;
         }
     } else {
-        A = k.c1 * inv;
-        B = A * inv * inv;
+        A = inv;
+        B = inv * inv * inv;
     }
     const float Bd = B * dF;
     px = fmaf(A, fj.x, px);
@@ -314,7 +212,7 @@ __device__ __forceinline__ void kahan_merge2(f32x2& s, f32x2& c, const f32x2 p) 
 }
 
 template <int I2, int TENSOR, int ACC>
-__global__ void __launch_bounds__(kThreads, SD_MIN_BLOCKS(I2))
+__global__ void __launch_bounds__(kThreads, (I2 <= 2) ? 2 : 1)
 pairs_f32_kernel(const float4* __restrict__ rec, float4* __restrict__ part, const Schedule sch,
                  const PairCoef k, const int N, const long long slot_stride) {
     constexpr int I = 2 * I2;
@@ -411,30 +309,12 @@ pairs_f32_kernel(const float4* __restrict__ rec, float4* __restrict__ part, cons
                     }
                 }
                 float mn = 3.0e38f;
-                f32x2 det = bc2(0.f);
 #pragma unroll kUnrollJ
                 for (int jj = 0; jj < kChunk; ++jj) {
                     const float4 pj = cj[2 * jj];
                     const float4 fj = cj[2 * jj + 1];
-#if SD_STAGED
                     pair_fast_staged<I2, TENSOR>(xi, yi, zi, pj, fj, k, px, py, pz, mn);
-#else
-#pragma unroll
-                    for (int m = 0; m < I2; ++m)
-                        pair_fast2<TENSOR>(xi[m], yi[m], zi[m], pj, fj, k, px[m], py[m], pz[m], mn, det);
-#endif
                 }
-#if SD_DETECT == 3
-                {   // NaN (self pair: inf - inf never occurs, inf does) and sums >= 1/thr^2
-                    const float dmax = fmaxf(lo2(det), hi2(det));
-                    if (!(dmax < k.det_thr)) mn = 0.f;
-                }
-#elif SD_DETECT == 4
-                {
-                    const float dmax = fmaxf(lo2(det), hi2(det));
-                    if (!(dmax < k.det_thr)) mn = 0.f;
-                }
-#endif
                 if (mn < k.thr) {
                     // an overlapping pair or the self pair sits in this chunk: redo it exactly
                     const int j0 = jbase + ch * kChunk;

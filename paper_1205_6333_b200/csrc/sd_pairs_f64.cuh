@@ -3,7 +3,8 @@
 // Same decomposition, staging ring and chunk-level slow path as the fp32 kernel
 // (sd_pairs_f32.cuh); differences:
 //  * 64-byte records {x, y, z, 0 | Fx, Fy, Fz, 0} of doubles, 64 j per 4 KiB tile;
-//  * no packed arithmetic (there is no DFMA2); one thread owns I particles;
+//  * no packed arithmetic (there is no DFMA2); one thread owns I particles (4 at large N with
+//    one CTA per SM, 2 with two CTAs per SM below: halves the LDS.128 per pair);
 //  * 1/r: MUFU.RSQ on the fp32-rounded r^2 as a 22-bit seed, then one third-order (Halley) step
 //    in fp64 (relative error ~2e-7 -> ~1e-21, i.e. rounding level); no fp64 division or sqrt
 //    in the loop;
@@ -39,13 +40,14 @@ __device__ __forceinline__ void pair_fast_f64(const double xi, const double yi, 
     const double inv = rsqrt_nr2(r2, r2f);
     const double dF = fma(dz, fj.z, fma(dy, fj.y, dx * fj.x));
     const double inv2 = inv * inv;
+    const double inv3 = inv2 * inv;
     double A, Bd;
-    if (TENSOR == TENSOR_RPY) {
-        A = fma(k.c2, inv2, k.c1) * inv;
-        Bd = fma(k.m3c2, inv2, k.c1) * (inv2 * dF) * inv;
+    if (TENSOR == TENSOR_RPY) {   // folded units (PairCoefT): fj = c1 F_j
+        A = fma(k.k2, inv3, inv);
+        Bd = fma(k.m3k2, inv2, 1.0) * (inv3 * dF);
     } else {
-        A = k.c1 * inv;
-        Bd = A * (inv2 * dF);
+        A = inv;
+        Bd = inv3 * dF;
     }
     px = fma(A, fj.x, px);
     py = fma(A, fj.y, py);
@@ -65,9 +67,9 @@ __device__ __forceinline__ void pair_exact_f64(const double xi, const double yi,
     const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
     if (r2 == 0.0) {
         if (TENSOR == TENSOR_RPY) {
-            px = fma(k.mu0, fj.x, px);
-            py = fma(k.mu0, fj.y, py);
-            pz = fma(k.mu0, fj.z, pz);
+            px = fma(k.mu0r, fj.x, px);
+            py = fma(k.mu0r, fj.y, py);
+            pz = fma(k.mu0r, fj.z, pz);
         }
         return;
     }
@@ -76,17 +78,18 @@ __device__ __forceinline__ void pair_exact_f64(const double xi, const double yi,
     const double dF = fma(dz, fj.z, fma(dy, fj.y, dx * fj.x));
     double A, B;
     if (TENSOR == TENSOR_RPY) {
-        if (r2 < k.four_a2) {
-            A = fma(k.ovA, r, k.mu0);
+        if (r2 < k.thr) {
+            A = fma(k.ovA, r, k.mu0r);
             B = k.ovB * inv;
         } else {
             const double inv2 = inv * inv;
-            A = fma(k.c2, inv2, k.c1) * inv;
-            B = fma(k.m3c2, inv2, k.c1) * inv2 * inv;
+            const double inv3 = inv2 * inv;
+            A = fma(k.k2, inv3, inv);
+            B = fma(k.m3k2, inv2, 1.0) * inv3;
         }
     } else {
-        A = k.c1 * inv;
-        B = A * inv * inv;
+        A = inv;
+        B = inv * inv * inv;
     }
     const double Bd = B * dF;
     px = fma(A, fj.x, px);
@@ -98,7 +101,7 @@ __device__ __forceinline__ void pair_exact_f64(const double xi, const double yi,
 }
 
 template <int I, int TENSOR>
-__global__ void __launch_bounds__(kThreads, 2)
+__global__ void __launch_bounds__(kThreads, (I <= 2) ? 2 : 1)
 pairs_f64_kernel(const double4* __restrict__ rec, double4* __restrict__ part, const Schedule sch,
                  const PairCoef64 k, const float thr, const int N, const long long slot_stride) {
     constexpr int IB = kThreads * I;

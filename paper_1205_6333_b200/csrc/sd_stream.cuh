@@ -1,5 +1,6 @@
 // sd_stream.cuh -- the O(N) streaming kernels around the pair kernel (HBM-bound):
-//   pack      : caller's pos/force [N][4]  ->  packed records (+ pad records)
+//   pack      : caller's pos/force [N][4]  ->  packed records {r | c1 F} (+ pad records); the
+//               1/r coefficient c1 = mu0 3a/4 is folded into the force lane (sd_common.cuh)
 //   finalize  : sum the segment partials of every row, add the self term mu0 F_i (Eq. 7a,
 //               PAPER.md:70-73), write vel, and -- fused -- apply the integrator update
 //               (Euler r <- r + dt v; midpoint half / full stage) including the
@@ -35,8 +36,8 @@ struct Vec4<double4> {
 template <typename T4>
 __global__ void __launch_bounds__(256)
 pack_kernel(const T4* __restrict__ pos, const T4* __restrict__ force, T4* __restrict__ rec,
-            const int what, const double gx, const double gy, const double gz, const int N,
-            const int Nrec) {
+            const int what, const double gx, const double gy, const double gz, const double c1,
+            const int N, const int Nrec) {
     typedef typename Vec4<T4>::S S;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= Nrec) return;
@@ -47,9 +48,10 @@ pack_kernel(const T4* __restrict__ pos, const T4* __restrict__ force, T4* __rest
         }
         if (what & PACK_FORCE) {
             const T4 f = force[i];
-            rec[2 * static_cast<size_t>(i) + 1] = Vec4<T4>::make(f.x, f.y, f.z, S(0));
+            const S k = S(c1);
+            rec[2 * static_cast<size_t>(i) + 1] = Vec4<T4>::make(k * f.x, k * f.y, k * f.z, S(0));
         } else if (what & PACK_GRAVITY) {
-            rec[2 * static_cast<size_t>(i) + 1] = Vec4<T4>::make(S(gx), S(gy), S(gz), S(0));
+            rec[2 * static_cast<size_t>(i) + 1] = Vec4<T4>::make(S(c1 * gx), S(c1 * gy), S(c1 * gz), S(0));
         }
     } else {
         const S pp = S(SD_PAD_POS);
@@ -64,14 +66,14 @@ __global__ void __launch_bounds__(256)
 finalize_f32_kernel(const float4* __restrict__ part, const int* __restrict__ blk_nslots,
                     float4* __restrict__ rec, float4* __restrict__ vel, float4* __restrict__ pos,
                     float4* __restrict__ pos_lo, float4* __restrict__ pos_half, const double dt,
-                    const double mu0, const int N, const int IB, const long long slot_stride) {
+                    const double mu0r, const int N, const int IB, const long long slot_stride) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N) return;
     const int nslots = blk_nslots[i / IB];
     const float4 f = rec[2 * static_cast<size_t>(i) + 1];
-    double vx = mu0 * static_cast<double>(f.x);
-    double vy = mu0 * static_cast<double>(f.y);
-    double vz = mu0 * static_cast<double>(f.z);
+    double vx = mu0r * static_cast<double>(f.x);   // self term mu0 F_i = (mu0 / c1) (c1 F_i)
+    double vy = mu0r * static_cast<double>(f.y);
+    double vz = mu0r * static_cast<double>(f.z);
     for (int s = 0; s < nslots; ++s) {
         const float4* p = part + (static_cast<size_t>(s) * slot_stride + i) * 2;
         const float4 hi = p[0];
@@ -106,12 +108,12 @@ __global__ void __launch_bounds__(256)
 finalize_f64_kernel(const double4* __restrict__ part, const int* __restrict__ blk_nslots,
                     double4* __restrict__ rec, double4* __restrict__ vel,
                     double4* __restrict__ pos, double4* __restrict__ pos_half, const double dt,
-                    const double mu0, const int N, const int IB, const long long slot_stride) {
+                    const double mu0r, const int N, const int IB, const long long slot_stride) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N) return;
     const int nslots = blk_nslots[i / IB];
     const double4 f = rec[2 * static_cast<size_t>(i) + 1];
-    double vx = mu0 * f.x, vy = mu0 * f.y, vz = mu0 * f.z;
+    double vx = mu0r * f.x, vy = mu0r * f.y, vz = mu0r * f.z;
     for (int s = 0; s < nslots; ++s) {
         const double4 p = part[static_cast<size_t>(s) * slot_stride + i];
         vx += p.x;
