@@ -31,12 +31,26 @@
  *   - Midpoint (north_star; PAPER.md:259 only hints at higher order):
  *         r_h = r + dt/2 M(r) F;   r <- r + dt M(r_h) F.
  *   - forces are inputs (constant during sdo_step).
+ *   - periodic box (the *_box entry points; PAPER.md:115 and its footnote 1: "a simulation
+ *     box with periodic boundaries and include only hydrodynamic interactions from the
+ *     nearest image of each particle"): cubic box of side L; every component of
+ *     d = r_i - r_j is replaced by d - L n, n = the integer nearest to d / L, so that
+ *     |d_alpha| <= L/2; positions need not lie inside the box; the self pair j == i stays
+ *     excluded.  SDO_IMAGE_DEFINITION takes n from C99 remainder() (exact, ties to even).
+ *     SDO_IMAGE_F32 / SDO_IMAGE_F64 take the DECISION n the way an fp32 / fp64 evaluation
+ *     does (reading B2): n = nearest integer (ties to even) of the exact product
+ *     d * inv with inv = 1/L rounded to that precision (and, for F32, d the fp32 difference
+ *     of the fp32 positions); the displacement d - L n itself is then formed in double.
+ *     The variants differ only for pairs within rounding of |d_alpha| = L/2.
  *
  * Pins (tests/test_oracle_pins.py, run with -m "not gpu"): single-sphere Stokes
  * velocity, closed-form two-sphere velocities, continuity and C1-continuity at r = 2a,
  * divergence-freeness, T = (1 + a^2/3 lap) G by finite differences, symmetry,
  * positive definiteness by Cholesky (+ negative controls), invariances, brute-force
  * matrix product, the 517 tau_s four-sphere cycle of PAPER.md:251-253.
+ *
+ * Positions are never wrapped into the box by sdo_step_box (the nearest-image rule does not
+ * need it).
  *
  * Arrays: pos, force, vel are contiguous [N][3] doubles (x, y, z), host memory,
  * caller-owned.  All functions return 0 on success, non-zero on invalid arguments.
@@ -82,6 +96,37 @@ static int sdo_pair_coef(int tensor, double r, double a, double mu0, double *A, 
     return 0;
 }
 
+#define SDO_IMAGE_DEFINITION 0 /* n from remainder(d, L): the plain definition          */
+#define SDO_IMAGE_F32 1        /* n decided as an fp32 evaluation decides it (reading B2) */
+#define SDO_IMAGE_F64 2        /* n decided as an fp64 evaluation decides it (reading B2) */
+
+/* nearest integer, ties to even, of the exact value hi + lo (|lo| <= ulp(hi)/2) */
+static double sdo_rint_exact(double hi, double lo) {
+    double n = nearbyint(hi); /* default rounding mode: to nearest, ties to even */
+    const double frac = hi - floor(hi);
+    if (frac == 0.5 && lo != 0.0) n = (lo > 0.0) ? floor(hi) + 1.0 : floor(hi);
+    return n;
+}
+
+/* Nearest-image displacement of one component (footnote 1).  L <= 0: free space. */
+static double sdo_min_image(double xi, double xj, double L, int image) {
+    if (!(L > 0.0)) return xi - xj;
+    if (image == SDO_IMAGE_F32) {
+        const float df = (float)xi - (float)xj;    /* fp32 difference of fp32 positions */
+        const float invf = 1.0f / (float)L;        /* 1/L rounded to fp32 */
+        const double prod = (double)df * (double)invf; /* 24 x 24 bits: exact in double */
+        return (double)df - nearbyint(prod) * (double)(float)L;
+    }
+    const double d = xi - xj;
+    if (image == SDO_IMAGE_F64) {
+        const double inv = 1.0 / L;
+        const double hi = d * inv;
+        const double lo = fma(d, inv, -hi);        /* hi + lo = d * inv exactly */
+        return d - sdo_rint_exact(hi, lo) * L;
+    }
+    return remainder(d, L);                        /* d - L * nearest integer to d/L */
+}
+
 static int sdo_args_ok(const double *pos, const double *force, long long N, double a, double eta,
                        int tensor) {
     if (!pos || !force || N < 1) return 0;
@@ -93,7 +138,7 @@ static int sdo_args_ok(const double *pos, const double *force, long long N, doub
 
 /* One row of Eq. (7a): velocity of particle i. */
 static void sdo_row(const double *pos, const double *force, long long N, double a, double mu0,
-                    int tensor, long long i, double *v) {
+                    int tensor, double L, int image, long long i, double *v) {
     long double sx, sy, sz;
     const double xi = pos[3 * i + 0], yi = pos[3 * i + 1], zi = pos[3 * i + 2];
     /* self contribution mu_ii = mu0 I */
@@ -102,9 +147,9 @@ static void sdo_row(const double *pos, const double *force, long long N, double 
     sz = (long double)(mu0 * force[3 * i + 2]);
     for (long long j = 0; j < N; ++j) {
         if (j == i) continue;
-        const double dx = xi - pos[3 * j + 0];
-        const double dy = yi - pos[3 * j + 1];
-        const double dz = zi - pos[3 * j + 2];
+        const double dx = sdo_min_image(xi, pos[3 * j + 0], L, image);
+        const double dy = sdo_min_image(yi, pos[3 * j + 1], L, image);
+        const double dz = sdo_min_image(zi, pos[3 * j + 2], L, image);
         const double fx = force[3 * j + 0], fy = force[3 * j + 1], fz = force[3 * j + 2];
         const double r = sqrt(dx * dx + dy * dy + dz * dz);
         double A, B;
@@ -126,32 +171,53 @@ static void sdo_row(const double *pos, const double *force, long long N, double 
     v[2] = (double)sz;
 }
 
-/* Velocities of the listed rows only: vel_out[k] = v_{rows[k]}, k < nrows. */
-int sdo_apply_rows(const double *pos, const double *force, long long N, double a, double eta,
-                   int tensor, const long long *rows, long long nrows, double *vel_out) {
+static int sdo_box_ok(double L, int image) {
+    if (!(L >= 0.0) || !isfinite(L)) return 0;
+    return image == SDO_IMAGE_DEFINITION || image == SDO_IMAGE_F32 || image == SDO_IMAGE_F64;
+}
+
+/* Velocities of the listed rows only: vel_out[k] = v_{rows[k]}, k < nrows.  L = 0: free space;
+ * L > 0: periodic cube of side L, nearest image only (see the header). */
+int sdo_apply_rows_box(const double *pos, const double *force, long long N, double a, double eta,
+                       int tensor, double L, int image, const long long *rows, long long nrows,
+                       double *vel_out) {
     if (!sdo_args_ok(pos, force, N, a, eta, tensor) || !rows || !vel_out || nrows < 0) return 1;
+    if (!sdo_box_ok(L, image)) return 1;
     for (long long k = 0; k < nrows; ++k)
         if (rows[k] < 0 || rows[k] >= N) return 1;
     const double mu0 = sdo_mu0(a, eta);
 #pragma omp parallel for schedule(dynamic, 8)
     for (long long k = 0; k < nrows; ++k)
-        sdo_row(pos, force, N, a, mu0, tensor, rows[k], vel_out + 3 * k);
+        sdo_row(pos, force, N, a, mu0, tensor, L, image, rows[k], vel_out + 3 * k);
     return 0;
+}
+
+int sdo_apply_rows(const double *pos, const double *force, long long N, double a, double eta,
+                   int tensor, const long long *rows, long long nrows, double *vel_out) {
+    return sdo_apply_rows_box(pos, force, N, a, eta, tensor, 0.0, SDO_IMAGE_DEFINITION, rows,
+                              nrows, vel_out);
 }
 
 /* All rows: vel[i] = v_i, i < N. */
-int sdo_apply(const double *pos, const double *force, long long N, double a, double eta,
-              int tensor, double *vel) {
-    if (!sdo_args_ok(pos, force, N, a, eta, tensor) || !vel) return 1;
+int sdo_apply_box(const double *pos, const double *force, long long N, double a, double eta,
+                  int tensor, double L, int image, double *vel) {
+    if (!sdo_args_ok(pos, force, N, a, eta, tensor) || !vel || !sdo_box_ok(L, image)) return 1;
     const double mu0 = sdo_mu0(a, eta);
 #pragma omp parallel for schedule(dynamic, 8) if (N >= 256)
-    for (long long i = 0; i < N; ++i) sdo_row(pos, force, N, a, mu0, tensor, i, vel + 3 * i);
+    for (long long i = 0; i < N; ++i)
+        sdo_row(pos, force, N, a, mu0, tensor, L, image, i, vel + 3 * i);
     return 0;
 }
 
+int sdo_apply(const double *pos, const double *force, long long N, double a, double eta,
+              int tensor, double *vel) {
+    return sdo_apply_box(pos, force, N, a, eta, tensor, 0.0, SDO_IMAGE_DEFINITION, vel);
+}
+
 /* Dense mobility matrix M[3N][3N], row-major, M[3i+al][3j+be] = (mu_ij)_{al be}. */
-int sdo_assemble(const double *pos, long long N, double a, double eta, int tensor, double *M) {
-    if (!sdo_args_ok(pos, pos, N, a, eta, tensor) || !M) return 1;
+int sdo_assemble_box(const double *pos, long long N, double a, double eta, int tensor, double L,
+                     int image, double *M) {
+    if (!sdo_args_ok(pos, pos, N, a, eta, tensor) || !M || !sdo_box_ok(L, image)) return 1;
     const double mu0 = sdo_mu0(a, eta);
     const long long n3 = 3 * N;
     for (long long i = 0; i < N; ++i) {
@@ -161,7 +227,8 @@ int sdo_assemble(const double *pos, long long N, double a, double eta, int tenso
                 blk[0][0] = blk[1][1] = blk[2][2] = mu0;
             } else {
                 double d[3];
-                for (int al = 0; al < 3; ++al) d[al] = pos[3 * i + al] - pos[3 * j + al];
+                for (int al = 0; al < 3; ++al)
+                    d[al] = sdo_min_image(pos[3 * i + al], pos[3 * j + al], L, image);
                 const double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
                 double A, B;
                 if (sdo_pair_coef(tensor, r, a, mu0, &A, &B)) {
@@ -179,14 +246,19 @@ int sdo_assemble(const double *pos, long long N, double a, double eta, int tenso
     return 0;
 }
 
+int sdo_assemble(const double *pos, long long N, double a, double eta, int tensor, double *M) {
+    return sdo_assemble_box(pos, N, a, eta, tensor, 0.0, SDO_IMAGE_DEFINITION, M);
+}
+
 /* Explicit integration with constant forces.  pos is updated in place.
  * If traj != NULL, the positions after steps rec_stride, 2 rec_stride, ... are appended to
  * traj ([n_steps / rec_stride][N][3]).  vel_last (optional) receives the velocities of the
  * last product evaluated (Euler: M(r_n)F of the last step; midpoint: M(r_h)F). */
-int sdo_step(double *pos, const double *force, long long N, double a, double eta, int tensor,
-             double dt, long long n_steps, int integrator, double *traj, long long rec_stride,
-             double *vel_last) {
+int sdo_step_box(double *pos, const double *force, long long N, double a, double eta, int tensor,
+                 double L, int image, double dt, long long n_steps, int integrator, double *traj,
+                 long long rec_stride, double *vel_last) {
     if (!sdo_args_ok(pos, force, N, a, eta, tensor) || !isfinite(dt) || n_steps < 0) return 1;
+    if (!sdo_box_ok(L, image)) return 1;
     if (integrator != SDO_INT_EULER && integrator != SDO_INT_MIDPOINT) return 1;
     if (traj && rec_stride < 1) return 1;
     double *v = (double *)malloc(sizeof(double) * 3 * (size_t)N);
@@ -198,12 +270,12 @@ int sdo_step(double *pos, const double *force, long long N, double a, double eta
     }
     long long nrec = 0;
     for (long long s = 0; s < n_steps; ++s) {
-        sdo_apply(pos, force, N, a, eta, tensor, v);
+        sdo_apply_box(pos, force, N, a, eta, tensor, L, image, v);
         if (integrator == SDO_INT_EULER) {
             for (long long k = 0; k < 3 * N; ++k) pos[k] = pos[k] + dt * v[k];
         } else {
             for (long long k = 0; k < 3 * N; ++k) ph[k] = pos[k] + 0.5 * dt * v[k];
-            sdo_apply(ph, force, N, a, eta, tensor, v);
+            sdo_apply_box(ph, force, N, a, eta, tensor, L, image, v);
             for (long long k = 0; k < 3 * N; ++k) pos[k] = pos[k] + dt * v[k];
         }
         if (traj && (s + 1) % rec_stride == 0) {
@@ -215,6 +287,13 @@ int sdo_step(double *pos, const double *force, long long N, double a, double eta
     free(v);
     free(ph);
     return 0;
+}
+
+int sdo_step(double *pos, const double *force, long long N, double a, double eta, int tensor,
+             double dt, long long n_steps, int integrator, double *traj, long long rec_stride,
+             double *vel_last) {
+    return sdo_step_box(pos, force, N, a, eta, tensor, 0.0, SDO_IMAGE_DEFINITION, dt, n_steps,
+                        integrator, traj, rec_stride, vel_last);
 }
 
 int sdo_num_threads(void) {

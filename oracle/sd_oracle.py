@@ -24,6 +24,9 @@ TENSOR_OSEEN = 1    # Eq. (4)
 TENSOR_RP_FAR = 2   # Eq. (7b) as printed for every r (negative control)
 INT_EULER = 0
 INT_MIDPOINT = 1
+IMAGE_DEFINITION = 0  # nearest image from C99 remainder(): the plain definition
+IMAGE_F32 = 1         # image index decided as an fp32 evaluation decides it (B2)
+IMAGE_F64 = 2         # image index decided as an fp64 evaluation decides it (B2)
 
 _lib = None
 
@@ -57,6 +60,14 @@ def _load():
     lib.sdo_assemble.argtypes = [dp, ll, dbl, dbl, ci, dp]
     lib.sdo_step.restype = ci
     lib.sdo_step.argtypes = [dp, dp, ll, dbl, dbl, ci, dbl, ll, ci, dp, ll, dp]
+    lib.sdo_apply_rows_box.restype = ci
+    lib.sdo_apply_rows_box.argtypes = [dp, dp, ll, dbl, dbl, ci, dbl, ci, lp, ll, dp]
+    lib.sdo_apply_box.restype = ci
+    lib.sdo_apply_box.argtypes = [dp, dp, ll, dbl, dbl, ci, dbl, ci, dp]
+    lib.sdo_assemble_box.restype = ci
+    lib.sdo_assemble_box.argtypes = [dp, ll, dbl, dbl, ci, dbl, ci, dp]
+    lib.sdo_step_box.restype = ci
+    lib.sdo_step_box.argtypes = [dp, dp, ll, dbl, dbl, ci, dbl, ci, dbl, ll, ci, dp, ll, dp]
     lib.sdo_num_threads.restype = ci
     lib.sdo_set_num_threads.argtypes = [ci]
     _lib = lib
@@ -83,42 +94,49 @@ def mu0(a: float, eta: float) -> float:
     return float(_load().sdo_mu0(a, eta))
 
 
-def apply(pos, force, a: float, eta: float, tensor: int = TENSOR_RPY) -> np.ndarray:
-    """All rows of Eq. (7a).  pos, force: [N, 3] -> vel [N, 3] (fp64)."""
+def apply(pos, force, a: float, eta: float, tensor: int = TENSOR_RPY, box: float = 0.0,
+          image: int = IMAGE_DEFINITION) -> np.ndarray:
+    """All rows of Eq. (7a).  pos, force: [N, 3] -> vel [N, 3] (fp64).  box > 0: periodic cube
+    of that side, nearest image only."""
     pos, force = _as3(pos, "pos"), _as3(force, "force")
     if pos.shape != force.shape:
         raise ValueError("pos and force must have the same shape")
     vel = np.empty_like(pos)
-    _check(_load().sdo_apply(_dp(pos), _dp(force), pos.shape[0], a, eta, tensor, _dp(vel)),
-           "sdo_apply")
+    _check(_load().sdo_apply_box(_dp(pos), _dp(force), pos.shape[0], a, eta, tensor, float(box),
+                                 int(image), _dp(vel)), "sdo_apply_box")
     return vel
 
 
-def apply_rows(pos, force, rows, a: float, eta: float, tensor: int = TENSOR_RPY) -> np.ndarray:
+def apply_rows(pos, force, rows, a: float, eta: float, tensor: int = TENSOR_RPY,
+               box: float = 0.0, image: int = IMAGE_DEFINITION) -> np.ndarray:
     """Rows `rows` of Eq. (7a): returns [len(rows), 3]."""
     pos, force = _as3(pos, "pos"), _as3(force, "force")
     if pos.shape != force.shape:
         raise ValueError("pos and force must have the same shape")
     rows = np.ascontiguousarray(np.asarray(rows, dtype=np.int64))
     out = np.empty((rows.shape[0], 3), dtype=np.float64)
-    rc = _load().sdo_apply_rows(_dp(pos), _dp(force), pos.shape[0], a, eta, tensor,
-                                rows.ctypes.data_as(ctypes.POINTER(ctypes.c_longlong)),
-                                rows.shape[0], _dp(out))
-    _check(rc, "sdo_apply_rows")
+    rc = _load().sdo_apply_rows_box(_dp(pos), _dp(force), pos.shape[0], a, eta, tensor,
+                                    float(box), int(image),
+                                    rows.ctypes.data_as(ctypes.POINTER(ctypes.c_longlong)),
+                                    rows.shape[0], _dp(out))
+    _check(rc, "sdo_apply_rows_box")
     return out
 
 
-def assemble(pos, a: float, eta: float, tensor: int = TENSOR_RPY) -> np.ndarray:
+def assemble(pos, a: float, eta: float, tensor: int = TENSOR_RPY, box: float = 0.0,
+             image: int = IMAGE_DEFINITION) -> np.ndarray:
     """Dense 3N x 3N mobility matrix (small N only)."""
     pos = _as3(pos, "pos")
     n = pos.shape[0]
     M = np.empty((3 * n, 3 * n), dtype=np.float64)
-    _check(_load().sdo_assemble(_dp(pos), n, a, eta, tensor, _dp(M)), "sdo_assemble")
+    _check(_load().sdo_assemble_box(_dp(pos), n, a, eta, tensor, float(box), int(image), _dp(M)),
+           "sdo_assemble_box")
     return M
 
 
 def step(pos, force, a: float, eta: float, dt: float, n_steps: int, integrator: int,
-         tensor: int = TENSOR_RPY, rec_stride: int = 0):
+         tensor: int = TENSOR_RPY, rec_stride: int = 0, box: float = 0.0,
+         image: int = IMAGE_DEFINITION):
     """Integrate n_steps with constant forces.  Returns (pos_final, vel_last, traj|None);
     traj[k] = positions after (k+1)*rec_stride steps when rec_stride > 0."""
     pos = _as3(pos, "pos").copy()
@@ -130,9 +148,9 @@ def step(pos, force, a: float, eta: float, dt: float, n_steps: int, integrator: 
         traj = np.empty((n_steps // rec_stride, n, 3), dtype=np.float64)
         tp = _dp(traj)
     vel = np.zeros_like(pos)
-    rc = _load().sdo_step(_dp(pos), _dp(force), n, a, eta, tensor, dt, n_steps, integrator,
-                          tp, max(rec_stride, 1), _dp(vel))
-    _check(rc, "sdo_step")
+    rc = _load().sdo_step_box(_dp(pos), _dp(force), n, a, eta, tensor, float(box), int(image),
+                              dt, n_steps, integrator, tp, max(rec_stride, 1), _dp(vel))
+    _check(rc, "sdo_step_box")
     return pos, vel, traj
 
 

@@ -100,14 +100,26 @@ def rsa_cube(n: int, phi: float, seed: int, a: float = A) -> np.ndarray:
     return pts - 0.5 * L
 
 
-def fcc_lattice(n_cells: int, number_density: float = 0.1, a: float = A) -> np.ndarray:
-    """fcc lattice of 4 n_cells^3 sites at the given number density, centred."""
+def fcc_lattice(n_cells: int, number_density: float = 0.1, a: float = A,
+                jitter_seed: int | None = None, jitter: float = 1e-2) -> np.ndarray:
+    """fcc lattice of 4 n_cells^3 sites at the given number density, centred.
+    With jitter_seed every site is moved by a seeded uniform offset in [-jitter, jitter]^3 (units
+    of a): the exact lattice has pairs at exactly half a box, where the nearest image of
+    PAPER.md:115 is ambiguous."""
     cell = (4.0 / number_density) ** (1.0 / 3.0) * a
     base = np.array([[0.0, 0.0, 0.0], [0.5, 0.5, 0.0], [0.5, 0.0, 0.5], [0.0, 0.5, 0.5]])
     g = np.arange(n_cells)
     ijk = np.stack(np.meshgrid(g, g, g, indexing="ij"), axis=-1).reshape(-1, 1, 3)
     pts = (ijk + base[None, :, :]).reshape(-1, 3) * cell
-    return pts - pts.mean(axis=0)
+    pts = pts - pts.mean(axis=0)
+    if jitter_seed is not None:
+        pts = pts + a * _rng(jitter_seed).uniform(-jitter, jitter, size=pts.shape)
+    return pts
+
+
+def fcc_box(n_cells: int, number_density: float = 0.1, a: float = A) -> float:
+    """Side L of the periodic cube commensurate with fcc_lattice(n_cells): N / L^3 = density."""
+    return n_cells * (4.0 / number_density) ** (1.0 / 3.0) * a
 
 
 def normal_forces(n: int, seed: int) -> np.ndarray:
