@@ -77,6 +77,17 @@ sd_status sd_create(sd_ctx** out, long long N, double a, double eta);
 sd_status sd_set_tensor(sd_ctx* ctx, sd_tensor tensor);
 sd_status sd_set_precision(sd_ctx* ctx, sd_precision precision);
 
+/* Boundary conditions (footnote 1: "a simulation box with periodic boundaries and
+ * include only hydrodynamic interactions from the nearest image of each particle").
+ * box_side = 0 (default): free space.  box_side = L > 0: periodic cube of side L; every
+ * component of d = r_i - r_j is replaced by d - L n, n the integer nearest to d / L, before the
+ * pair tensor is evaluated; the self pair stays excluded.  Positions need not lie inside the box
+ * and sd_step never wraps them.  n is taken in the arithmetic of the context's precision as
+ * rint(d * fl(1/fl(L))) with the product exact and ties to even (fl = rounding to float in the
+ * F32 modes, to double in F64), so a pair within rounding of |d| = L/2 may see the opposite,
+ * equally near image.  |d| / L must stay below 2^22 (F32) / 2^51 (F64). */
+sd_status sd_set_box(sd_ctx* ctx, double box_side);
+
 /* Step 3 of the paper's loop (Eq. 7a): vel = M(pos) force.
  * pos, force: in; vel: out (must not alias pos or force). */
 sd_status sd_mobility_apply(sd_ctx* ctx, const void* pos, const void* force, void* vel,
@@ -109,6 +120,7 @@ sd_status sd_reset_compensation(sd_ctx* ctx, void* stream);
 /* Accessors. */
 long long sd_num_particles(const sd_ctx* ctx);
 double sd_self_mobility(const sd_ctx* ctx); /* mu0 = 1/(6 pi eta a) */
+double sd_box(const sd_ctx* ctx);           /* side of the periodic cube, 0 in free space */
 
 /* Number of kernel launches enqueued by this context since creation (bench bookkeeping). */
 long long sd_launch_count(const sd_ctx* ctx);

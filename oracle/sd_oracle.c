@@ -100,12 +100,12 @@ static int sdo_pair_coef(int tensor, double r, double a, double mu0, double *A, 
 #define SDO_IMAGE_F32 1        /* n decided as an fp32 evaluation decides it (reading B2) */
 #define SDO_IMAGE_F64 2        /* n decided as an fp64 evaluation decides it (reading B2) */
 
-/* nearest integer, ties to even, of the exact value hi + lo (|lo| <= ulp(hi)/2) */
+/* nearest integer, ties to even, of the exact value hi + lo (|lo| <= ulp(hi)/2, |hi| < 2^51) */
 static double sdo_rint_exact(double hi, double lo) {
-    double n = nearbyint(hi); /* default rounding mode: to nearest, ties to even */
-    const double frac = hi - floor(hi);
-    if (frac == 0.5 && lo != 0.0) n = (lo > 0.0) ? floor(hi) + 1.0 : floor(hi);
-    return n;
+    const double t = 2.0 * hi;                                /* exact */
+    const int half_integer = (t == floor(t)) && (fmod(t, 2.0) != 0.0); /* hi = k + 1/2 */
+    if (half_integer && lo != 0.0) return (lo > 0.0) ? ceil(hi) : floor(hi);
+    return nearbyint(hi); /* default rounding mode: to nearest, ties to even */
 }
 
 /* Nearest-image displacement of one component (footnote 1).  L <= 0: free space. */

@@ -44,6 +44,7 @@ struct sd_ctx {
     double a = 0, eta = 0, mu0 = 0;
     int tensor = SD_TENSOR_RPY;
     int precision = SD_PREC_F32_KAHAN;
+    double box = 0.0;  // side of the periodic cube; 0 = free space
     int device = 0;
     int num_sms = 0;
     Config cfg;
@@ -88,13 +89,22 @@ sd_status fail(sd_ctx* ctx, sd_status code, const std::string& msg) {
                         std::string(#call) + ": " + cudaGetErrorString(e_));               \
     } while (0)
 
-template <int I2, int TENSOR, int ACC>
+template <int I2, int TENSOR, int ACC, bool PBC>
 const void* f32_kernel() {
-    return reinterpret_cast<const void*>(&sd::pairs_f32_kernel<I2, TENSOR, ACC>);
+    return reinterpret_cast<const void*>(&sd::pairs_f32_kernel<I2, TENSOR, ACC, PBC>);
 }
-template <int I, int TENSOR>
+template <int I, int TENSOR, bool PBC>
 const void* f64_kernel() {
-    return reinterpret_cast<const void*>(&sd::pairs_f64_kernel<I, TENSOR>);
+    return reinterpret_cast<const void*>(&sd::pairs_f64_kernel<I, TENSOR, PBC>);
+}
+template <int I2, bool PBC>
+const void* f32_pick(bool rpy, bool plain) {
+    return rpy ? (plain ? f32_kernel<I2, 0, 1, PBC>() : f32_kernel<I2, 0, 0, PBC>())
+               : (plain ? f32_kernel<I2, 1, 1, PBC>() : f32_kernel<I2, 1, 0, PBC>());
+}
+template <int I, bool PBC>
+const void* f64_pick(bool rpy) {
+    return rpy ? f64_kernel<I, 0, PBC>() : f64_kernel<I, 1, PBC>();
 }
 
 void free_buffers(sd_ctx* c) {
@@ -118,6 +128,7 @@ sd_status configure(sd_ctx* c) {
     Config cfg;
     const bool f64 = c->precision == SD_PREC_F64;
     const bool rpy = c->tensor == SD_TENSOR_RPY;
+    const bool pbc = c->box > 0.0;
     if (!f64) {
         const bool plain = c->precision == SD_PREC_F32_PLAIN;
         // particles per thread: 8 once there is enough work to balance 2048-particle i-blocks
@@ -126,30 +137,33 @@ sd_status configure(sd_ctx* c) {
         const int i2 = (c->N >= 131072) ? 4 : 2;
         cfg.ipt = 2 * i2;
         cfg.TJ = sd::kTJ;
-        static const char* names[2][2][2] = {
-            {{"pairs_f32x2_i4_rpy_kahan", "pairs_f32x2_i4_rpy_plain"},
-             {"pairs_f32x2_i4_oseen_kahan", "pairs_f32x2_i4_oseen_plain"}},
-            {{"pairs_f32x2_i8_rpy_kahan", "pairs_f32x2_i8_rpy_plain"},
-             {"pairs_f32x2_i8_oseen_kahan", "pairs_f32x2_i8_oseen_plain"}}};
-        cfg.name = names[i2 == 4 ? 1 : 0][rpy ? 0 : 1][plain ? 1 : 0];
+        static const char* names[2][2][2][2] = {
+            {{{"pairs_f32x2_i4_rpy_kahan", "pairs_f32x2_i4_rpy_kahan_pbc"},
+              {"pairs_f32x2_i4_rpy_plain", "pairs_f32x2_i4_rpy_plain_pbc"}},
+             {{"pairs_f32x2_i4_oseen_kahan", "pairs_f32x2_i4_oseen_kahan_pbc"},
+              {"pairs_f32x2_i4_oseen_plain", "pairs_f32x2_i4_oseen_plain_pbc"}}},
+            {{{"pairs_f32x2_i8_rpy_kahan", "pairs_f32x2_i8_rpy_kahan_pbc"},
+              {"pairs_f32x2_i8_rpy_plain", "pairs_f32x2_i8_rpy_plain_pbc"}},
+             {{"pairs_f32x2_i8_oseen_kahan", "pairs_f32x2_i8_oseen_kahan_pbc"},
+              {"pairs_f32x2_i8_oseen_plain", "pairs_f32x2_i8_oseen_plain_pbc"}}}};
+        cfg.name = names[i2 == 4 ? 1 : 0][rpy ? 0 : 1][plain ? 1 : 0][pbc ? 1 : 0];
         if (i2 == 4)
-            cfg.kernel = rpy ? (plain ? f32_kernel<4, 0, 1>() : f32_kernel<4, 0, 0>())
-                             : (plain ? f32_kernel<4, 1, 1>() : f32_kernel<4, 1, 0>());
+            cfg.kernel = pbc ? f32_pick<4, true>(rpy, plain) : f32_pick<4, false>(rpy, plain);
         else
-            cfg.kernel = rpy ? (plain ? f32_kernel<2, 0, 1>() : f32_kernel<2, 0, 0>())
-                             : (plain ? f32_kernel<2, 1, 1>() : f32_kernel<2, 1, 0>());
+            cfg.kernel = pbc ? f32_pick<2, true>(rpy, plain) : f32_pick<2, false>(rpy, plain);
     } else {
         // 4 particles per thread (one CTA per SM) once 1024-particle i-blocks balance over the
         // SMs: one LDS.128 per pair instead of two (measured +3 % at N = 524288)
         cfg.ipt = (c->N >= 131072) ? 4 : 2;
         cfg.TJ = sd::kTJ64;
-        if (cfg.ipt == 4) {
-            cfg.kernel = rpy ? f64_kernel<4, 0>() : f64_kernel<4, 1>();
-            cfg.name = rpy ? "pairs_f64_i4_rpy" : "pairs_f64_i4_oseen";
-        } else {
-            cfg.kernel = rpy ? f64_kernel<2, 0>() : f64_kernel<2, 1>();
-            cfg.name = rpy ? "pairs_f64_i2_rpy" : "pairs_f64_i2_oseen";
-        }
+        static const char* names64[2][2][2] = {
+            {{"pairs_f64_i2_rpy", "pairs_f64_i2_rpy_pbc"}, {"pairs_f64_i2_oseen", "pairs_f64_i2_oseen_pbc"}},
+            {{"pairs_f64_i4_rpy", "pairs_f64_i4_rpy_pbc"}, {"pairs_f64_i4_oseen", "pairs_f64_i4_oseen_pbc"}}};
+        cfg.name = names64[cfg.ipt == 4 ? 1 : 0][rpy ? 0 : 1][pbc ? 1 : 0];
+        if (cfg.ipt == 4)
+            cfg.kernel = pbc ? f64_pick<4, true>(rpy) : f64_pick<4, false>(rpy);
+        else
+            cfg.kernel = pbc ? f64_pick<2, true>(rpy) : f64_pick<2, false>(rpy);
     }
     cfg.IB = sd::kThreads * cfg.ipt;
     cfg.B = static_cast<int>((c->N + cfg.IB - 1) / cfg.IB);
@@ -235,6 +249,19 @@ sd_status launch_pack(sd_ctx* c, const void* pos, const void* force, int what, c
 
 sd_status launch_pairs_impl(sd_ctx* c, cudaStream_t st);
 
+// nearest-image constants (PAPER.md:115 footnote 1): L is rounded to S first, 1/L is the
+// correctly rounded quotient in S (reading B2); free space: all zero
+template <typename S>
+void box_coef(const sd_ctx* c, S& invL, S& mL, S& magic) {
+    invL = mL = magic = S(0);
+    if (c->box > 0.0) {
+        const S L = static_cast<S>(c->box);
+        invL = S(1) / L;
+        mL = -L;
+        magic = (sizeof(S) == 4) ? static_cast<S>(12582912.0) : static_cast<S>(6755399441055744.0);
+    }
+}
+
 // coefficients in the folded units of sd_common.cuh (PairCoefT): they depend on a only
 template <typename S>
 sd::PairCoefT<S> folded_coef(const sd_ctx* c) {
@@ -246,6 +273,7 @@ sd::PairCoefT<S> folded_coef(const sd_ctx* c) {
     k.ovA = static_cast<S>(-3.0 / (8.0 * a * a));
     k.ovB = static_cast<S>(1.0 / (8.0 * a * a));
     k.thr = (c->tensor == SD_TENSOR_RPY) ? static_cast<S>(4.0 * a * a) : static_cast<S>(1e-30);
+    box_coef<S>(c, k.invL, k.mL, k.magic);
     return k;
 }
 
@@ -320,6 +348,7 @@ sd::CoefT<S> coef_of(const sd_ctx* c) {
     k.ovA = static_cast<S>(-9.0 * mu0 / (32.0 * a));
     k.ovB = static_cast<S>(3.0 * mu0 / (32.0 * a));
     k.four_a2 = static_cast<S>(4.0 * a * a);
+    box_coef<S>(c, k.invL, k.mL, k.magic);
     return k;
 }
 
@@ -462,6 +491,19 @@ sd_status sd_set_precision(sd_ctx* ctx, sd_precision precision) {
     return configure(ctx);
 }
 
+sd_status sd_set_box(sd_ctx* ctx, double box_side) {
+    if (!ctx) return fail(nullptr, SD_ERR_INVALID_ARG, "sd_set_box: ctx is NULL");
+    if (!(box_side >= 0.0) || !std::isfinite(box_side))
+        return fail(ctx, SD_ERR_INVALID_ARG, "sd_set_box: box side must be finite and >= 0 (0 = free space)");
+    if (box_side > 0.0 && !(static_cast<float>(box_side) > 0.0f) )
+        return fail(ctx, SD_ERR_INVALID_ARG, "sd_set_box: box side underflows in fp32");
+    const bool was = ctx->box > 0.0, is = box_side > 0.0;
+    ctx->box = box_side;
+    if (was == is) return SD_OK;  // same kernels, only the constants change
+    cudaDeviceSynchronize();
+    return configure(ctx);
+}
+
 sd_status sd_mobility_apply(sd_ctx* ctx, const void* pos, const void* force, void* vel, void* stream) {
     if (!ctx) return fail(nullptr, SD_ERR_INVALID_ARG, "sd_mobility_apply: ctx is NULL");
     if (!pos || !force || !vel) return fail(ctx, SD_ERR_INVALID_ARG, "sd_mobility_apply: NULL pointer");
@@ -594,6 +636,7 @@ sd_status sd_reset_compensation(sd_ctx* ctx, void* stream) {
 
 long long sd_num_particles(const sd_ctx* ctx) { return ctx ? ctx->N : 0; }
 double sd_self_mobility(const sd_ctx* ctx) { return ctx ? ctx->mu0 : 0.0; }
+double sd_box(const sd_ctx* ctx) { return ctx ? ctx->box : 0.0; }
 long long sd_launch_count(const sd_ctx* ctx) { return ctx ? ctx->launches : 0; }
 const char* sd_kernel_name(const sd_ctx* ctx) {
     if (!ctx) return "";

@@ -7,7 +7,9 @@
 //   rec64 : [Nrec][2] double4 = same in fp64 (64 bytes),
 //           the paper's "32 bytes per particle (2 x float4)" record.  Nrec is N
 //           rounded up to SD_REC_ALIGN; pad records sit at SD_PAD_POS with zero force, so they
-//           add exactly 0 to every sum and a j-tile is always one full bulk copy.
+//           add exactly 0 to every sum and a j-tile is always one full bulk copy.  (With a
+//           periodic box the wrapped image of a pad can land anywhere: it still adds 0 on the
+//           fast path, and the exact body skips j >= N.)
 //   part  : [slot][Nrec][2]   = compensated partial sums (hi, lo) of one (i-block, j-range)
 //           segment; combined by the finalize kernel.
 #pragma once
@@ -89,6 +91,10 @@ struct PairCoefT {
     S ovA;    // -3 / (8 a^2)             overlap branch: A = mu0r + ovA * r
     S ovB;    // 1 / (8 a^2)              overlap branch: B = ovB / r
     S thr;    // slow-path threshold on r^2: 4a^2 for RPY, tiny for Oseen (only r == 0)
+    // periodic cube of side L, nearest image only (PAPER.md:115 footnote 1); unused in free space
+    S invL;   // 1 / L rounded to S
+    S mL;     // -L
+    S magic;  // 1.5 * 2^23 (float) / 1.5 * 2^52 (double): fma(d, invL, magic) - magic = rint(d invL)
 };
 typedef PairCoefT<float> PairCoef;
 typedef PairCoefT<double> PairCoef64;

@@ -99,7 +99,11 @@ __device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b) {
 // with three distinct register operands in one bank takes 3 cycles instead of 2).
 // 20 packed FP32 instructions + 4 MUFU per two pairs for Rotne-Prager, 17 + 4 for Oseen.
 // fj holds F' = c1 F (see the file header); k.k2 = 2a^2/3, k.m3k2 = -2a^2.
-template <int I2, int TENSOR>
+// PBC (periodic cube, nearest image only; PAPER.md:115 footnote 1): every component of d is
+// replaced by d - L n with n = rint(d / L) taken as (fma(d, 1/L, M) - M), M = 1.5 * 2^23: the
+// fma rounds the exact product d * fl(1/L) to an integer, ties to even (reading B2).
+// 3 more packed instructions per component: 29 per two pairs (Rotne-Prager), 26 (Oseen).
+template <int I2, int TENSOR, bool PBC>
 __device__ __forceinline__ void pair_fast_staged(const f32x2 (&xi)[I2], const f32x2 (&yi)[I2],
                                                  const f32x2 (&zi)[I2], const float4 pj,
                                                  const float4 fj, const PairCoef& k,
@@ -114,6 +118,18 @@ __device__ __forceinline__ void pair_fast_staged(const f32x2 (&xi)[I2], const f3
     for (int m = 0; m < I2; ++m) dy[m] = sub2(yi[m], yj);
 #pragma unroll
     for (int m = 0; m < I2; ++m) dz[m] = sub2(zi[m], zj);
+    if (PBC) {
+        const f32x2 il = bc2(k.invL), mg = bc2(k.magic), nl = bc2(k.mL);
+#pragma unroll
+        for (int m = 0; m < I2; ++m) {
+            const f32x2 qx = sub2(fma2(dx[m], il, mg), mg);
+            const f32x2 qy = sub2(fma2(dy[m], il, mg), mg);
+            const f32x2 qz = sub2(fma2(dz[m], il, mg), mg);
+            dx[m] = fma2(qx, nl, dx[m]);
+            dy[m] = fma2(qy, nl, dy[m]);
+            dz[m] = fma2(qz, nl, dz[m]);
+        }
+    }
 #pragma unroll
     for (int m = 0; m < I2; ++m) {
         r2[m] = mul2(dx[m], dx[m]);
@@ -162,12 +178,17 @@ __device__ __forceinline__ void pair_fast_staged(const f32x2 (&xi)[I2], const f3
 
 // Exact body for one (i, j): self exclusion, coincident centres, overlap branch (A4,
 // A5), in the same folded units as the fast body (fj = c1 F_j, coefficients relative to c1).
-template <int TENSOR>
+template <int TENSOR, bool PBC>
 __device__ __forceinline__ void pair_exact(const float xi, const float yi, const float zi,
                                            const bool self, const float4 pj, const float4 fj,
                                            const PairCoef& k, float& px, float& py, float& pz) {
     if (self) return;
-    const float dx = xi - pj.x, dy = yi - pj.y, dz = zi - pj.z;
+    float dx = xi - pj.x, dy = yi - pj.y, dz = zi - pj.z;
+    if (PBC) {  // same nearest-image rule as the fast body
+        dx = __fmaf_rn(__fsub_rn(__fmaf_rn(dx, k.invL, k.magic), k.magic), k.mL, dx);
+        dy = __fmaf_rn(__fsub_rn(__fmaf_rn(dy, k.invL, k.magic), k.magic), k.mL, dy);
+        dz = __fmaf_rn(__fsub_rn(__fmaf_rn(dz, k.invL, k.magic), k.magic), k.mL, dz);
+    }
     const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
     if (r2 == 0.0f) {
         if (TENSOR == TENSOR_RPY) {  // limit of the overlap branch: mu0 F_j
@@ -211,7 +232,7 @@ __device__ __forceinline__ void kahan_merge2(f32x2& s, f32x2& c, const f32x2 p) 
     s = t;
 }
 
-template <int I2, int TENSOR, int ACC>
+template <int I2, int TENSOR, int ACC, bool PBC>
 __global__ void __launch_bounds__(kThreads, (I2 <= 2) ? 2 : 1)
 pairs_f32_kernel(const float4* __restrict__ rec, float4* __restrict__ part, const Schedule sch,
                  const PairCoef k, const int N, const long long slot_stride) {
@@ -313,7 +334,7 @@ pairs_f32_kernel(const float4* __restrict__ rec, float4* __restrict__ part, cons
                 for (int jj = 0; jj < kChunk; ++jj) {
                     const float4 pj = cj[2 * jj];
                     const float4 fj = cj[2 * jj + 1];
-                    pair_fast_staged<I2, TENSOR>(xi, yi, zi, pj, fj, k, px, py, pz, mn);
+                    pair_fast_staged<I2, TENSOR, PBC>(xi, yi, zi, pj, fj, k, px, py, pz, mn);
                 }
                 if (mn < k.thr) {
                     // an overlapping pair or the self pair sits in this chunk: redo it exactly
@@ -338,10 +359,13 @@ pairs_f32_kernel(const float4* __restrict__ rec, float4* __restrict__ part, cons
                             const int i0 = i_first + (2 * m) * kThreads;
                             float ax = lo2(px[m]), ay = lo2(py[m]), az = lo2(pz[m]);
                             float bx = hi2(px[m]), by = hi2(py[m]), bz = hi2(pz[m]);
-                            pair_exact<TENSOR>(lo2(xi[m]), lo2(yi[m]), lo2(zi[m]), j == i0, pj, fj,
-                                               k, ax, ay, az);
-                            pair_exact<TENSOR>(hi2(xi[m]), hi2(yi[m]), hi2(zi[m]),
-                                               j == i0 + kThreads, pj, fj, k, bx, by, bz);
+                            // pad records (j >= N) are skipped here: under PBC their wrapped
+                            // image can land anywhere in the box
+                            pair_exact<TENSOR, PBC>(lo2(xi[m]), lo2(yi[m]), lo2(zi[m]),
+                                                    j == i0 || j >= N, pj, fj, k, ax, ay, az);
+                            pair_exact<TENSOR, PBC>(hi2(xi[m]), hi2(yi[m]), hi2(zi[m]),
+                                                    j == i0 + kThreads || j >= N, pj, fj, k, bx,
+                                                    by, bz);
                             px[m] = pk2(ax, bx);
                             py[m] = pk2(ay, by);
                             pz[m] = pk2(az, bz);

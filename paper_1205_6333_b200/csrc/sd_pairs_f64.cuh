@@ -28,12 +28,21 @@ __device__ __forceinline__ double rsqrt_nr2(const double r2, const float r2f) {
     return fma(y * e, p, y);
 }
 
-template <int TENSOR>
+// PBC: nearest image as in the fp32 kernel, d <- d - L rint(d / L) with rint taken as
+// fma(d, 1/L, M) - M, M = 1.5 * 2^52 (PAPER.md:115 footnote 1; reading B2).
+template <bool PBC>
+__device__ __forceinline__ double min_image_f64(const double d, const PairCoef64& k) {
+    if (!PBC) return d;
+    return fma(__dsub_rn(fma(d, k.invL, k.magic), k.magic), k.mL, d);
+}
+
+template <int TENSOR, bool PBC>
 __device__ __forceinline__ void pair_fast_f64(const double xi, const double yi, const double zi,
                                               const double4 pj, const double4 fj,
                                               const PairCoef64& k, double& px, double& py,
                                               double& pz, float& mn) {
-    const double dx = xi - pj.x, dy = yi - pj.y, dz = zi - pj.z;
+    const double dx = min_image_f64<PBC>(xi - pj.x, k), dy = min_image_f64<PBC>(yi - pj.y, k),
+                 dz = min_image_f64<PBC>(zi - pj.z, k);
     const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
     const float r2f = static_cast<float>(r2);
     mn = fminf(mn, r2f);
@@ -57,13 +66,14 @@ __device__ __forceinline__ void pair_fast_f64(const double xi, const double yi, 
     pz = fma(Bd, dz, pz);
 }
 
-template <int TENSOR>
+template <int TENSOR, bool PBC>
 __device__ __forceinline__ void pair_exact_f64(const double xi, const double yi, const double zi,
                                                const bool self, const double4 pj,
                                                const double4 fj, const PairCoef64& k, double& px,
                                                double& py, double& pz) {
     if (self) return;
-    const double dx = xi - pj.x, dy = yi - pj.y, dz = zi - pj.z;
+    const double dx = min_image_f64<PBC>(xi - pj.x, k), dy = min_image_f64<PBC>(yi - pj.y, k),
+                 dz = min_image_f64<PBC>(zi - pj.z, k);
     const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
     if (r2 == 0.0) {
         if (TENSOR == TENSOR_RPY) {
@@ -100,7 +110,7 @@ __device__ __forceinline__ void pair_exact_f64(const double xi, const double yi,
     pz = fma(Bd, dz, pz);
 }
 
-template <int I, int TENSOR>
+template <int I, int TENSOR, bool PBC>
 __global__ void __launch_bounds__(kThreads, (I <= 2) ? 2 : 1)
 pairs_f64_kernel(const double4* __restrict__ rec, double4* __restrict__ part, const Schedule sch,
                  const PairCoef64 k, const float thr, const int N, const long long slot_stride) {
@@ -187,7 +197,8 @@ pairs_f64_kernel(const double4* __restrict__ rec, double4* __restrict__ part, co
                     const double4 fj = cj[2 * jj + 1];
 #pragma unroll
                     for (int m = 0; m < I; ++m)
-                        pair_fast_f64<TENSOR>(xi[m], yi[m], zi[m], pj, fj, k, px[m], py[m], pz[m], mn);
+                        pair_fast_f64<TENSOR, PBC>(xi[m], yi[m], zi[m], pj, fj, k, px[m], py[m], pz[m],
+                                                   mn);
                 }
                 if (mn < thr) {
                     const int j0 = jbase + ch * kChunk;
@@ -204,8 +215,9 @@ pairs_f64_kernel(const double4* __restrict__ rec, double4* __restrict__ part, co
                         const int j = j0 + jj;
 #pragma unroll
                         for (int m = 0; m < I; ++m)
-                            pair_exact_f64<TENSOR>(xi[m], yi[m], zi[m], j == i_first + m * kThreads,
-                                                   pj, fj, k, px[m], py[m], pz[m]);
+                            pair_exact_f64<TENSOR, PBC>(xi[m], yi[m], zi[m],
+                                                        j == i_first + m * kThreads || j >= N, pj,
+                                                        fj, k, px[m], py[m], pz[m]);
                     }
                 }
             }

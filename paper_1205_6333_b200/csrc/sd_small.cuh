@@ -33,7 +33,20 @@ constexpr int kSmallTile = 256;
 template <typename S>
 struct CoefT {
     S c1, c2, m3c2, mu0, ovA, ovB, four_a2;
+    // periodic cube (PAPER.md:115 footnote 1): invL = 0 means free space; see PairCoefT
+    S invL, mL, magic;
 };
+
+// nearest image of one displacement component, same rule as the tiled kernels (the branch is
+// uniform over the grid)
+__device__ __forceinline__ float min_image(const float d, const CoefT<float>& k) {
+    if (k.invL == 0.0f) return d;
+    return __fmaf_rn(__fsub_rn(__fmaf_rn(d, k.invL, k.magic), k.magic), k.mL, d);
+}
+__device__ __forceinline__ double min_image(const double d, const CoefT<double>& k) {
+    if (k.invL == 0.0) return d;
+    return fma(__dsub_rn(fma(d, k.invL, k.magic), k.magic), k.mL, d);
+}
 
 __device__ __forceinline__ float inv_sqrt_exact(float r2) {
     float y = rsq_approx(r2);
@@ -50,7 +63,7 @@ __device__ __forceinline__ void pair_term(const S xi, const S yi, const S zi, co
                                           const S fy, const S fz, const CoefT<S>& k, S& px, S& py,
                                           S& pz) {
     if (self) return;
-    const S dx = xi - xj, dy = yi - yj, dz = zi - zj;
+    const S dx = min_image(xi - xj, k), dy = min_image(yi - yj, k), dz = min_image(zi - zj, k);
     const S r2 = dx * dx + dy * dy + dz * dz;
     if (r2 == S(0)) {
         if (TENSOR == TENSOR_RPY) {

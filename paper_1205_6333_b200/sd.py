@@ -33,6 +33,8 @@ SYMBOLS = {
     "sd_create": (_I, [ctypes.POINTER(_P), _LL, _D, _D]),
     "sd_set_tensor": (_I, [_P, _I]),
     "sd_set_precision": (_I, [_P, _I]),
+    "sd_set_box": (_I, [_P, _D]),
+    "sd_box": (_D, [_P]),
     "sd_mobility_apply": (_I, [_P, _P, _P, _P, _P]),
     "sd_mobility_apply_host": (_I, [_P, _P, _P, _P, _P]),
     "sd_step": (_I, [_P, _P, FORCE_FN, _P, _P, ctypes.POINTER(_D), _D, _LL, _I, _P]),
@@ -120,6 +122,14 @@ class Context:
     def set_precision(self, precision: int):
         self._check(self._lib.sd_set_precision(self._h, int(precision)))
         self.precision = int(precision)
+
+    def set_box(self, box_side: float):
+        """Periodic cube of that side, nearest image only; 0 = free space."""
+        self._check(self._lib.sd_set_box(self._h, float(box_side)))
+
+    @property
+    def box(self) -> float:
+        return float(self._lib.sd_box(self._h))
 
     def mobility_apply(self, pos, force, vel, stream=None):
         self._check(self._lib.sd_mobility_apply(self._h, self._ptr(pos, "pos"),

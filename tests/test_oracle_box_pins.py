@@ -170,6 +170,50 @@ def test_image_decision_variants_agree_away_from_half_box(image):
     np.testing.assert_allclose(got, want, rtol=0, atol=1e-5 if image == orc.IMAGE_F32 else 1e-13)
 
 
+@pytest.mark.parametrize("image", [orc.IMAGE_F32, orc.IMAGE_F64])
+def test_image_decision_rule_against_exact_rational_arithmetic(image):
+    """Reading B2 spelled out with fractions.Fraction: n = nearest integer, ties to even, of the
+    EXACT product d * fl(1/fl(L)).  The exact fcc lattice supplies hundreds of coordinate pairs
+    whose product is within an ulp of +-1/2, on either side of it."""
+    from fractions import Fraction
+
+    def rint_even(fr):
+        fl = math.floor(fr)
+        r = fr - fl
+        if r != Fraction(1, 2):
+            return fl if r < Fraction(1, 2) else fl + 1
+        return fl if fl % 2 == 0 else fl + 1
+
+    F = np.array([[1.0, 2.0, 3.0], [0.5, -1.0, 2.0]])
+    checked, below, above = 0, 0, 0
+    for cells in (3, 5, 6, 7):
+        pos = wl.fcc_lattice(cells, 0.1)
+        L = wl.fcc_box(cells, 0.1)
+        if image == orc.IMAGE_F32:
+            pos = pos.astype(np.float32).astype(np.float64)
+            L = float(np.float32(L))
+            inv = float(np.float32(1.0) / np.float32(L))
+        else:
+            inv = 1.0 / L
+        xs = sorted(set(pos[:, 0]))
+        for xa in xs:
+            for xb in xs:
+                d = float(np.float32(xa) - np.float32(xb)) if image == orc.IMAGE_F32 else xa - xb
+                prod = Fraction(d) * Fraction(inv)
+                if abs(abs(float(prod)) - 0.5) > 1e-6:
+                    continue
+                n = rint_even(prod)
+                below += abs(prod) < Fraction(1, 2)
+                above += abs(prod) > Fraction(1, 2)
+                got = orc.apply(np.array([[xa, 0.25, 0.125], [xb, 0.0, 0.0]]), F, 1.0, ETA1,
+                                box=L, image=image)
+                want = orc.apply(np.array([[d - n * L, 0.25, 0.125], [0.0, 0.0, 0.0]]), F, 1.0,
+                                 ETA1)
+                np.testing.assert_allclose(got, want, rtol=0, atol=1e-14)
+                checked += 1
+    assert checked >= 40 and below > 0 and above > 0
+
+
 def test_image_decision_at_exactly_half_a_box():
     """d = L/2 exactly: both images are nearest.  remainder() takes the even multiple (n = 0);
     the fp32 rule rounds d * fl32(1/L), and fl32(1/3) > 1/3 tips it to n = 1.  Same distance,
