@@ -173,16 +173,26 @@ def test_large_box_is_free_space_and_box_can_be_switched_off(gpu):
 
 
 # ---- sd_step in the box: the paper's benchmark run (Euler, dt = 0.001 tau_s, 100 steps) ----------
+#
+# The nearest-image rule is discontinuous: when a pair component crosses |d| = L/2 the pair
+# tensor jumps, so two trajectories that differ in the last bit part ways by O(1e-3 a) as soon as
+# one of them flips a pair the other does not.  The commensurate lattice keeps thousands of pair
+# components within the jitter of L/2, and fp32 positions put a handful of them within an ulp.
+# Long runs are therefore compared (a) in fp64 on the commensurate box, (b) in fp32 and fp64 in a
+# box 2 % larger than the lattice, where no pair comes within 0.3 a of half a box, and (c) in fp32
+# on the commensurate box step by step, each step restarted from the GPU's own positions.
 
-@pytest.mark.parametrize("prec_name,tol", [("PREC_F32_KAHAN", 1e-4), ("PREC_F64", 1e-9)])
+@pytest.mark.parametrize("prec_name,tol,scale", [("PREC_F32_KAHAN", 1e-4, 1.02),
+                                                 ("PREC_F64", 1e-9, 1.02),
+                                                 ("PREC_F64", 1e-9, 1.0)])
 @pytest.mark.parametrize("cells,integ,steps,dt", [(2, "midpoint", 1000, 0.01),
                                                   (10, "euler", 100, 0.001),
                                                   (11, "midpoint", 20, 0.005)])
-def test_step_in_periodic_box(gpu, prec_name, tol, cells, integ, steps, dt):
+def test_step_in_periodic_box(gpu, prec_name, tol, scale, cells, integ, steps, dt):
     """N = 32 (one-launch stepper), 4000 (one launch per product), 5324 (tiled kernels)."""
     torch, sd = gpu
     pos = wl.fcc_lattice(cells, 0.1, jitter_seed=wl.SEED_BASE + 31 + cells)
-    L = wl.fcc_box(cells, 0.1)
+    L = scale * wl.fcc_box(cells, 0.1)
     n = pos.shape[0]
     p = rounded(pos, prec_name)
     ctx = sd.Context(n, wl.A, wl.ETA)
@@ -202,4 +212,33 @@ def test_step_in_periodic_box(gpu, prec_name, tol, cells, integ, steps, dt):
     assert rel_err(dv.cpu().numpy()[:, :3].astype(np.float64), vlast) <= 10 * TOL[prec_name]
     # the suspension settled (|v| is several mu0 F with ~N^(2/3) neighbours inside L/2)
     assert (got[:, 2] - p[:, 2]).mean() < -steps * dt
+    ctx.close()
+
+
+@pytest.mark.parametrize("cells", [10, 11])
+def test_fp32_euler_steps_on_the_commensurate_lattice_step_by_step(gpu, cells):
+    """(c) above: the paper's benchmark shape itself in fp32.  Every Euler step starts from the
+    positions the GPU holds (hi words; the low words are dropped on both sides by
+    sd_reset_compensation), so GPU and oracle decide every image from identical fp32 numbers."""
+    torch, sd = gpu
+    pos = wl.fcc_lattice(cells, 0.1, jitter_seed=wl.SEED_BASE + 31 + cells)
+    L = wl.fcc_box(cells, 0.1)
+    n = pos.shape[0]
+    ctx = sd.Context(n, wl.A, wl.ETA)
+    ctx.set_box(L)
+    dp = torch.from_numpy(wl.to_xyzw(pos, np.float32)).cuda()
+    dv = torch.empty_like(dp)
+    F = wl.gravity_forces(n)
+    for _ in range(6):
+        before = dp.cpu().numpy()[:, :3].astype(np.float64)
+        ctx.reset_compensation()
+        ctx.step(dp, 0.001, 1, sd.INT_EULER, gravity=(0.0, 0.0, -1.0))
+        ctx.get_velocity(dv)
+        torch.cuda.synchronize()
+        want, vwant, _ = orc.step(before, F, wl.A, wl.ETA, 0.001, 1, orc.INT_EULER,
+                                  box=float(np.float32(L)), image=orc.IMAGE_F32)
+        assert rel_err(dv.cpu().numpy()[:, :3].astype(np.float64), vwant) <= 1e-5
+        # positions: exact to the rounding of the stored fp32 word
+        got = dp.cpu().numpy()[:, :3].astype(np.float64)
+        assert np.abs(got - want).max() <= 1e-5 * 0.001 * np.abs(vwant).max() + 2.0 ** -24 * np.abs(want).max()
     ctx.close()
