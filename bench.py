@@ -27,6 +27,7 @@ if ROOT not in sys.path:
 import numpy as np  # noqa: E402
 
 FLOPS_PER_PAIR = {"rpy": 34, "oseen": 29}       # algorithmic flops
+FLOPS_NEAREST_IMAGE = 15                        # + 3 x (fma, add, fma) per pair in a periodic box
 FP32_LANES_PER_SM, FP64_LANES_PER_SM = 128, 64  # CUDA-core FMA lanes per SM (measured: ubench)
 # DRAM bytes per pair-kernel launch from the ncu --set full capture named in profiles/README.md
 NCU_TRAFFIC_BYTES = {(1048576, "f32", "rpy"): 43.9e6}  # profiles/r01_pairs_f32_ncu_full.md
@@ -41,6 +42,12 @@ def parse_args():
     ap.add_argument("--n", type=int, default=1048576)
     ap.add_argument("--precision", choices=["f32", "f64"], default="f32")
     ap.add_argument("--tensor", choices=["rpy", "oseen"], default="rpy")
+    ap.add_argument("--box", action="store_true",
+                    help="periodic cube of the cloud's own side, nearest image only (PAPER.md:115)")
+    ap.add_argument("--fcc-cells", type=int, default=0,
+                    help="instead of the product: the paper's benchmark run (PAPER.md:231), fcc "
+                         "lattice of 4 cells^3 spheres at n = 0.1 a^-3 in its periodic box, 100 "
+                         "Euler steps of 0.001 tau_s per timed step; reports simulation steps/s")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
 
@@ -53,10 +60,15 @@ def workload(n):
 
 def workload_name(args):
     return (f"sd_mobility_apply N={args.n} uniform cube phi=0.01, N(0,1) forces, "
-            f"{args.tensor.upper()}, {'fp32-Kahan' if args.precision == 'f32' else 'fp64'}")
+            f"{args.tensor.upper()}, {'fp32-Kahan' if args.precision == 'f32' else 'fp64'}"
+            + (", periodic box (nearest image)" if args.box else ""))
 
 
-def time_oracle(pos64, force64, wl, tensor, target_seconds, n_threads=None):
+def box_side(args, wl):
+    return wl.cube_side(args.n, 0.01) if args.box else 0.0
+
+
+def time_oracle(pos64, force64, wl, tensor, target_seconds, box=0.0, image=0):
     """Oracle pair rate on a bounded seeded row sample sized for about target_seconds."""
     from oracle import sd_oracle as orc
     otensor = orc.TENSOR_RPY if tensor == "rpy" else orc.TENSOR_OSEEN
@@ -64,12 +76,12 @@ def time_oracle(pos64, force64, wl, tensor, target_seconds, n_threads=None):
     cores = orc.num_threads()
     probe_rows = wl.row_subset(n, min(n, 8 * cores), wl.SEED_BASE + 9)
     t0 = time.perf_counter()
-    orc.apply_rows(pos64, force64, probe_rows, wl.A, wl.ETA, otensor)
+    orc.apply_rows(pos64, force64, probe_rows, wl.A, wl.ETA, otensor, box=box, image=image)
     t_probe = max(time.perf_counter() - t0, 1e-6)
     rows = int(min(n, max(len(probe_rows), len(probe_rows) * target_seconds / t_probe)))
     sample = wl.row_subset(n, rows, wl.SEED_BASE + 10)
     t0 = time.perf_counter()
-    orc.apply_rows(pos64, force64, sample, wl.A, wl.ETA, otensor)
+    orc.apply_rows(pos64, force64, sample, wl.A, wl.ETA, otensor, box=box, image=image)
     t = time.perf_counter() - t0
     return len(sample) * n / t, cores, len(sample), t
 
@@ -85,14 +97,15 @@ def run_reference(args, rank):
     otensor = orc.TENSOR_RPY if args.tensor == "rpy" else orc.TENSOR_OSEEN
     cores = orc.num_threads()
     # size one step for ~2 s so that W + K steps stay within a few minutes
-    rate0, _, _, _ = time_oracle(p64, f64, wl, args.tensor, 1.0)
+    box = float(np.float32(box_side(args, wl)))
+    rate0, _, _, _ = time_oracle(p64, f64, wl, args.tensor, 1.0, box=box)
     rows = int(max(8 * cores, min(args.n, 2.0 * rate0 / args.n)))
     sample = wl.row_subset(args.n, rows, wl.SEED_BASE + 11)
     for _ in range(args.warmup):
-        orc.apply_rows(p64, f64, sample, wl.A, wl.ETA, otensor)
+        orc.apply_rows(p64, f64, sample, wl.A, wl.ETA, otensor, box=box)
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        orc.apply_rows(p64, f64, sample, wl.A, wl.ETA, otensor)
+        orc.apply_rows(p64, f64, sample, wl.A, wl.ETA, otensor, box=box)
     t = time.perf_counter() - t0
     value = args.steps * len(sample) * args.n / t
     sample_desc = f"{len(sample)} seeded rows x all {args.n} columns per step"
@@ -111,11 +124,124 @@ def run_reference(args, rank):
     print(json.dumps(line), flush=True)
 
 
+def run_fcc_steps(args, rank):
+    """The paper's own benchmark run: fcc lattice at n = 0.1 a^-3 in its periodic
+    box, uniform gravity, Euler steps of 0.001 tau_s, 100 steps per timed "step" of this script.
+    Reports simulation steps/s and the pair rate; --impl reference runs the oracle instead (a
+    bounded number of simulation steps).  Single GPU (rank 0 only)."""
+    if rank != 0:
+        return
+    from paper_1205_6333_b200 import workloads as wl
+    cells = args.fcc_cells
+    pos = wl.fcc_lattice(cells, 0.1, jitter_seed=wl.SEED_BASE + 31 + cells)
+    L = wl.fcc_box(cells, 0.1)
+    n = pos.shape[0]
+    sim_steps, dt = 100, 0.001
+    f64mode = args.precision == "f64"
+    npdt = np.float64 if f64mode else np.float32
+    name = (f"sd_step N={n} fcc lattice n=0.1/a^3 (+1e-2 a seeded jitter) in its periodic box "
+            f"L={L:.3f} a, nearest image, gravity, Euler dt=0.001, {sim_steps} steps per timed step, "
+            f"{args.tensor.upper()}, {'fp64' if f64mode else 'fp32-Kahan'}")
+    base = {"metric": "simulation steps/s at N (Euler step = one mobility product + update)",
+            "unit": "steps/s", "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "data": "synthetic",
+            "paper_context": "5.7 ms per step at N = 4150 on a Tesla C2050 (PAPER.md:281), "
+                             "another machine and the whole HAL step: context only"}
+    if args.impl == "reference":
+        from oracle import sd_oracle as orc
+        otensor = orc.TENSOR_RPY if args.tensor == "rpy" else orc.TENSOR_OSEEN
+        p64 = wl.to_xyzw(pos, npdt)[:, :3].astype(np.float64)
+        F = wl.gravity_forces(n)
+        t0 = time.perf_counter()
+        orc.step(p64, F, wl.A, wl.ETA, dt, 1, orc.INT_EULER, otensor, box=L)
+        per = max(time.perf_counter() - t0, 1e-6)
+        k = int(max(1, min(sim_steps, 2.0 / per)))  # ~2 s per timed step
+        for _ in range(args.warmup):
+            orc.step(p64, F, wl.A, wl.ETA, dt, k, orc.INT_EULER, otensor, box=L)
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            orc.step(p64, F, wl.A, wl.ETA, dt, k, orc.INT_EULER, otensor, box=L)
+        t = time.perf_counter() - t0
+        value = args.steps * k / t
+        desc = f"{k} Euler steps of all {n} rows per timed step"
+        line = dict(base, impl="reference", value=value, ms_per_step=1e3 * t / args.steps,
+                    dtype="f64", config={"workload": name, "step": desc},
+                    cpu_baseline={"value": value, "unit": "steps/s", "cores": orc.num_threads(),
+                                  "kind": "oracle", "sample": desc},
+                    e2e={"value": value, "unit": "steps/s", "h2d_bytes_per_step": 0,
+                         "d2h_bytes_per_step": 0}, gpu_launches=0)
+        print(json.dumps(line), flush=True)
+        return
+
+    import torch
+    from paper_1205_6333_b200 import benchutil, sd
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product has no CPU fallback")
+    torch.cuda.set_device(0)
+    sd.load_library()
+    h_pos = torch.from_numpy(wl.to_xyzw(pos, npdt)).pin_memory()
+    h_out = torch.empty_like(h_pos).pin_memory()
+    d_pos0 = h_pos.cuda()
+    d_pos = d_pos0.clone()
+    ctx = sd.Context(n, wl.A, wl.ETA)
+    ctx.set_precision(sd.PREC_F64 if f64mode else sd.PREC_F32_KAHAN)
+    ctx.set_tensor(sd.TENSOR_RPY if args.tensor == "rpy" else sd.TENSOR_OSEEN)
+    ctx.set_box(L)
+    g = (0.0, 0.0, -1.0)
+
+    def one_run():
+        d_pos.copy_(d_pos0)
+        ctx.reset_compensation()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        ctx.step(d_pos, dt, sim_steps, sd.INT_EULER, gravity=g)
+        e1.record()
+        return e0, e1
+
+    for _ in range(args.warmup):
+        one_run()
+    torch.cuda.synchronize()
+    launches0 = ctx.launch_count
+    sampler = benchutil.ClockSampler(0)
+    sampler.start()
+    evs = [one_run() for _ in range(args.steps)]
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    secs = sum(a.elapsed_time(b) for a, b in evs) * 1e-3
+    gpu_launches = ctx.launch_count - launches0
+    # end to end: positions from pinned host memory, final positions back to the host
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        d_pos.copy_(h_pos, non_blocking=True)
+        ctx.reset_compensation()
+        ctx.step(d_pos, dt, sim_steps, sd.INT_EULER, gravity=g)
+        h_out.copy_(d_pos, non_blocking=True)
+        torch.cuda.synchronize()
+    e2e = time.perf_counter() - t0
+    rec_bytes = n * 4 * (8 if f64mode else 4)
+    value = args.steps * sim_steps / secs
+    line = dict(base, value=value, ms_per_step=1e3 * secs / args.steps,
+                dtype="f64" if f64mode else "f32",
+                config={"workload": name, "kernel": ctx.kernel_name, "parallelism": "1 GPU",
+                        "l2": "whole problem is L2-resident by nature (N x 32 B); no flush: the "
+                              "100 steps of one run reuse the same buffers as the paper's run does"},
+                clocks=clocks, gpu_launches=gpu_launches,
+                ms_per_simulation_step=1e3 * secs / (args.steps * sim_steps),
+                pairs_per_s=value * n * n,
+                e2e={"value": args.steps * sim_steps / e2e, "unit": "steps/s",
+                     "h2d_bytes_per_step": rec_bytes, "d2h_bytes_per_step": rec_bytes})
+    ctx.close()
+    print(json.dumps(line), flush=True)
+
+
 def main():
     args = parse_args()
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.fcc_cells > 0:
+        run_fcc_steps(args, rank)
+        return
     if args.impl == "reference":
         run_reference(args, rank)
         return
@@ -148,6 +274,7 @@ def main():
     ctx = sd.Context(n, wl.A, wl.ETA)
     ctx.set_precision(prec)
     ctx.set_tensor(tensor)
+    ctx.set_box(box_side(args, wl))
     peak_probe = ctx.fma_peak_probe(prec)
 
     def barrier():
@@ -203,12 +330,12 @@ def main():
             sm_max_mhz = float(json.load(f).get("sm_max_mhz", sm_max_mhz))
     lanes = FP64_LANES_PER_SM if f64mode else FP32_LANES_PER_SM
     peak_tflops = sm_count * lanes * 2 * sm_max_mhz * 1e6 / 1e12
-    flops = FLOPS_PER_PAIR[args.tensor]
+    flops = FLOPS_PER_PAIR[args.tensor] + (FLOPS_NEAREST_IMAGE if args.box else 0)
     achieved = flops * float(n) * n * pair_launches / (pair_ms * 1e-3) / 1e12 if pair_ms > 0 else None
     roofline = {
         "bound": "alu", "kernel": ctx.kernel_name, "achieved": achieved, "peak": peak_tflops,
         "unit": "TFLOP/s", "frac": (achieved / peak_tflops) if achieved else None,
-        "traffic": NCU_TRAFFIC_BYTES.get((n, args.precision, args.tensor)),
+        "traffic": None if args.box else NCU_TRAFFIC_BYTES.get((n, args.precision, args.tensor)),
         "peak_source": f"derived: {sm_count} SMs x {lanes} FMA lanes x 2 flop x {sm_max_mhz:.0f} MHz "
                        "(sm_max_mhz of MEASURED_PEAKS.json; DESIGN.md)",
         "fma_probe_tflops": peak_probe,
@@ -235,7 +362,8 @@ def main():
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         p64 = h_pos.numpy()[:, :3].astype(np.float64)
         f64 = h_force.numpy()[:, :3].astype(np.float64)
-        rate, cores, rows, secs = time_oracle(p64, f64, wl, args.tensor, 15.0)
+        rate, cores, rows, secs = time_oracle(p64, f64, wl, args.tensor, 15.0,
+                                              box=float(np.float32(box_side(args, wl))))
         line["cpu_baseline"] = {"value": rate, "unit": "pairs/s", "cores": cores, "kind": "oracle",
                                 "sample": f"{rows} seeded rows x all {n} columns of the same "
                                           f"workload, {secs:.1f} s"}

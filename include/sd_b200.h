@@ -77,6 +77,15 @@ sd_status sd_create(sd_ctx** out, long long N, double a, double eta);
 sd_status sd_set_tensor(sd_ctx* ctx, sd_tensor tensor);
 sd_status sd_set_precision(sd_ctx* ctx, sd_precision precision);
 
+/* Dispatch knobs of the small-N path (below a few thousand particles the device is
+ * under-filled), for ablations and tests; the defaults are the measured crossovers.
+ *   small_apply_max     : N up to which one product is ONE launch of the warp-per-particle kernel
+ *                         (no pack / partial sums / finalize); < 0 restores the default.
+ *   particles_per_thread: 2, 4 or 8 particles i per thread in the tiled kernels (fp64: half of
+ *                         it); 0 = automatic (by N).
+ * Reallocates the scratch buffers; synchronises the device. */
+sd_status sd_set_dispatch(sd_ctx* ctx, long long small_apply_max, int particles_per_thread);
+
 /* Boundary conditions (footnote 1: "a simulation box with periodic boundaries and
  * include only hydrodynamic interactions from the nearest image of each particle").
  * box_side = 0 (default): free space.  box_side = L > 0: periodic cube of side L; every

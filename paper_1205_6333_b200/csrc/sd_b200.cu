@@ -45,6 +45,8 @@ struct sd_ctx {
     int tensor = SD_TENSOR_RPY;
     int precision = SD_PREC_F32_KAHAN;
     double box = 0.0;  // side of the periodic cube; 0 = free space
+    long long small_apply_max = sd::kSmallApplyMax;  // N up to which the one-launch kernel runs
+    int ipt_override = 0;                            // particles per thread; 0 = automatic
     int device = 0;
     int num_sms = 0;
     Config cfg;
@@ -132,12 +134,17 @@ sd_status configure(sd_ctx* c) {
     if (!f64) {
         const bool plain = c->precision == SD_PREC_F32_PLAIN;
         // particles per thread: 8 once there is enough work to balance 2048-particle i-blocks
-        // over the SMs (more operand reuse per j record), 4 below that.  (N <= kSmallApplyMax
-        // never reaches this kernel: sd_small.cuh.)
-        const int i2 = (c->N >= 131072) ? 4 : 2;
+        // over the SMs (more operand reuse per j record), 4 and 2 below that (measured
+        // crossovers, profiles/r01c_sweep.md).  N <= small_apply_max never reaches this kernel.
+        int i2 = (c->N > sd::kIpt8Min) ? 4 : (c->N > sd::kIpt4Min ? 2 : 1);
+        if (c->ipt_override) i2 = c->ipt_override / 2;
         cfg.ipt = 2 * i2;
         cfg.TJ = sd::kTJ;
-        static const char* names[2][2][2][2] = {
+        static const char* names[3][2][2][2] = {
+            {{{"pairs_f32x2_i2_rpy_kahan", "pairs_f32x2_i2_rpy_kahan_pbc"},
+              {"pairs_f32x2_i2_rpy_plain", "pairs_f32x2_i2_rpy_plain_pbc"}},
+             {{"pairs_f32x2_i2_oseen_kahan", "pairs_f32x2_i2_oseen_kahan_pbc"},
+              {"pairs_f32x2_i2_oseen_plain", "pairs_f32x2_i2_oseen_plain_pbc"}}},
             {{{"pairs_f32x2_i4_rpy_kahan", "pairs_f32x2_i4_rpy_kahan_pbc"},
               {"pairs_f32x2_i4_rpy_plain", "pairs_f32x2_i4_rpy_plain_pbc"}},
              {{"pairs_f32x2_i4_oseen_kahan", "pairs_f32x2_i4_oseen_kahan_pbc"},
@@ -146,24 +153,30 @@ sd_status configure(sd_ctx* c) {
               {"pairs_f32x2_i8_rpy_plain", "pairs_f32x2_i8_rpy_plain_pbc"}},
              {{"pairs_f32x2_i8_oseen_kahan", "pairs_f32x2_i8_oseen_kahan_pbc"},
               {"pairs_f32x2_i8_oseen_plain", "pairs_f32x2_i8_oseen_plain_pbc"}}}};
-        cfg.name = names[i2 == 4 ? 1 : 0][rpy ? 0 : 1][plain ? 1 : 0][pbc ? 1 : 0];
+        cfg.name = names[i2 == 4 ? 2 : (i2 == 2 ? 1 : 0)][rpy ? 0 : 1][plain ? 1 : 0][pbc ? 1 : 0];
         if (i2 == 4)
             cfg.kernel = pbc ? f32_pick<4, true>(rpy, plain) : f32_pick<4, false>(rpy, plain);
-        else
+        else if (i2 == 2)
             cfg.kernel = pbc ? f32_pick<2, true>(rpy, plain) : f32_pick<2, false>(rpy, plain);
+        else
+            cfg.kernel = pbc ? f32_pick<1, true>(rpy, plain) : f32_pick<1, false>(rpy, plain);
     } else {
         // 4 particles per thread (one CTA per SM) once 1024-particle i-blocks balance over the
-        // SMs: one LDS.128 per pair instead of two (measured +3 % at N = 524288)
-        cfg.ipt = (c->N >= 131072) ? 4 : 2;
+        // SMs: one LDS.128 per pair instead of two; 2 and 1 below (measured crossovers)
+        cfg.ipt = (c->N > sd::kIpt4Min64) ? 4 : (c->N > sd::kIpt4Min ? 2 : 1);
+        if (c->ipt_override) cfg.ipt = std::max(1, c->ipt_override / 2);
         cfg.TJ = sd::kTJ64;
-        static const char* names64[2][2][2] = {
+        static const char* names64[3][2][2] = {
+            {{"pairs_f64_i1_rpy", "pairs_f64_i1_rpy_pbc"}, {"pairs_f64_i1_oseen", "pairs_f64_i1_oseen_pbc"}},
             {{"pairs_f64_i2_rpy", "pairs_f64_i2_rpy_pbc"}, {"pairs_f64_i2_oseen", "pairs_f64_i2_oseen_pbc"}},
             {{"pairs_f64_i4_rpy", "pairs_f64_i4_rpy_pbc"}, {"pairs_f64_i4_oseen", "pairs_f64_i4_oseen_pbc"}}};
-        cfg.name = names64[cfg.ipt == 4 ? 1 : 0][rpy ? 0 : 1][pbc ? 1 : 0];
+        cfg.name = names64[cfg.ipt == 4 ? 2 : (cfg.ipt == 2 ? 1 : 0)][rpy ? 0 : 1][pbc ? 1 : 0];
         if (cfg.ipt == 4)
             cfg.kernel = pbc ? f64_pick<4, true>(rpy) : f64_pick<4, false>(rpy);
-        else
+        else if (cfg.ipt == 2)
             cfg.kernel = pbc ? f64_pick<2, true>(rpy) : f64_pick<2, false>(rpy);
+        else
+            cfg.kernel = pbc ? f64_pick<1, true>(rpy) : f64_pick<1, false>(rpy);
     }
     cfg.IB = sd::kThreads * cfg.ipt;
     cfg.B = static_cast<int>((c->N + cfg.IB - 1) / cfg.IB);
@@ -273,6 +286,7 @@ sd::PairCoefT<S> folded_coef(const sd_ctx* c) {
     k.ovA = static_cast<S>(-3.0 / (8.0 * a * a));
     k.ovB = static_cast<S>(1.0 / (8.0 * a * a));
     k.thr = (c->tensor == SD_TENSOR_RPY) ? static_cast<S>(4.0 * a * a) : static_cast<S>(1e-30);
+    k.clampv = static_cast<S>(4.0 * a * a);
     box_coef<S>(c, k.invL, k.mL, k.magic);
     return k;
 }
@@ -322,14 +336,14 @@ sd_status launch_pairs_impl(sd_ctx* c, cudaStream_t st) {
 template <int MODE>
 sd_status launch_finalize(sd_ctx* c, void* vel, void* pos, double dt, cudaStream_t st) {
     const int n = static_cast<int>(c->N);
-    const int blocks = (n + 255) / 256;
+    const int blocks = (n + sd::kFinThreads - 1) / sd::kFinThreads;
     if (c->precision == SD_PREC_F64)
-        sd::finalize_f64_kernel<MODE><<<blocks, 256, 0, st>>>(
+        sd::finalize_f64_kernel<MODE><<<blocks, sd::kFinThreads, 0, st>>>(
             static_cast<const double4*>(c->part), c->d_blk_nslots, static_cast<double4*>(c->rec),
             static_cast<double4*>(vel), static_cast<double4*>(pos),
             static_cast<double4*>(c->pos_half), dt, 4.0 / (3.0 * c->a), n, c->cfg.IB, c->Nrec);
     else
-        sd::finalize_f32_kernel<MODE><<<blocks, 256, 0, st>>>(
+        sd::finalize_f32_kernel<MODE><<<blocks, sd::kFinThreads, 0, st>>>(
             static_cast<const float4*>(c->part), c->d_blk_nslots, static_cast<float4*>(c->rec),
             static_cast<float4*>(vel), static_cast<float4*>(pos), static_cast<float4*>(c->pos_lo),
             static_cast<float4*>(c->pos_half), dt, 4.0 / (3.0 * c->a), n, c->cfg.IB, c->Nrec);
@@ -491,6 +505,17 @@ sd_status sd_set_precision(sd_ctx* ctx, sd_precision precision) {
     return configure(ctx);
 }
 
+sd_status sd_set_dispatch(sd_ctx* ctx, long long small_apply_max, int particles_per_thread) {
+    if (!ctx) return fail(nullptr, SD_ERR_INVALID_ARG, "sd_set_dispatch: ctx is NULL");
+    if (particles_per_thread != 0 && particles_per_thread != 2 && particles_per_thread != 4 &&
+        particles_per_thread != 8)
+        return fail(ctx, SD_ERR_INVALID_ARG, "sd_set_dispatch: particles_per_thread must be 0, 2, 4 or 8");
+    cudaDeviceSynchronize();
+    ctx->small_apply_max = small_apply_max < 0 ? sd::kSmallApplyMax : small_apply_max;
+    ctx->ipt_override = particles_per_thread;
+    return configure(ctx);
+}
+
 sd_status sd_set_box(sd_ctx* ctx, double box_side) {
     if (!ctx) return fail(nullptr, SD_ERR_INVALID_ARG, "sd_set_box: ctx is NULL");
     if (!(box_side >= 0.0) || !std::isfinite(box_side))
@@ -512,7 +537,7 @@ sd_status sd_mobility_apply(sd_ctx* ctx, const void* pos, const void* force, voi
         return fail(ctx, SD_ERR_INVALID_ARG, "sd_mobility_apply: records must be 16-byte (float) / 32-byte (double) aligned");
     if (vel == pos || vel == force) return fail(ctx, SD_ERR_INVALID_ARG, "sd_mobility_apply: vel aliases an input");
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    if (ctx->N <= sd::kSmallApplyMax)  // small-N path: one launch, no pack / partials / finalize
+    if (ctx->N <= ctx->small_apply_max)  // small-N path: one launch, no pack / partials / finalize
         return launch_small_apply(ctx, pos, force, nullptr, vel, nullptr, nullptr, 0.0, sd::FIN_VEL, st);
     sd_status s = launch_pack(ctx, pos, force, sd::PACK_POS | sd::PACK_FORCE, nullptr, st);
     if (s != SD_OK) return s;
@@ -564,7 +589,7 @@ sd_status sd_step(sd_ctx* ctx, void* pos, sd_force_fn fn, void* user, const void
     }
     if (!fn && ctx->N <= sd::kStepperMax)  // all steps in one launch
         return launch_stepper(ctx, pos, force, gravity, dt, n_steps, integrator, st);
-    if (ctx->N <= sd::kSmallApplyMax) {    // one launch per product
+    if (ctx->N <= ctx->small_apply_max) {    // one launch per product
         const void* fptr = fn ? ctx->force_buf : force;
         const double* g = (fn || force) ? nullptr : gravity;
         void* cur = pos;
@@ -640,7 +665,7 @@ double sd_box(const sd_ctx* ctx) { return ctx ? ctx->box : 0.0; }
 long long sd_launch_count(const sd_ctx* ctx) { return ctx ? ctx->launches : 0; }
 const char* sd_kernel_name(const sd_ctx* ctx) {
     if (!ctx) return "";
-    if (ctx->N <= sd::kSmallApplyMax)
+    if (ctx->N <= ctx->small_apply_max)
         return ctx->precision == SD_PREC_F64 ? "small_apply_f64" : "small_apply_f32";
     return ctx->cfg.name;
 }

@@ -90,7 +90,8 @@ struct PairCoefT {
     S mu0r;   // mu0 / c1 = 4 / (3a)      (coincident centres; self term in the finalize kernel)
     S ovA;    // -3 / (8 a^2)             overlap branch: A = mu0r + ovA * r
     S ovB;    // 1 / (8 a^2)              overlap branch: B = ovB / r
-    S thr;    // slow-path threshold on r^2: 4a^2 for RPY, tiny for Oseen (only r == 0)
+    S thr;    // careful-pass threshold on r^2: 4a^2 for RPY, tiny for Oseen (only r == 0)
+    S clampv; // 4 a^2: lower clamp of r^2 in the careful pass (both tensors)
     // periodic cube of side L, nearest image only (PAPER.md:115 footnote 1); unused in free space
     S invL;   // 1 / L rounded to S
     S mL;     // -L

@@ -37,6 +37,10 @@ constexpr int kStages = 4;   // ring depth
 constexpr int kPrefetch = 2; // tiles in flight ahead of the one being consumed
 constexpr int kChunk = 32;   // j per compensation chunk
 constexpr int kUnrollJ = 4;  // j per unrolled loop body
+// measured crossovers of the particles-per-thread variants (profiles/r01c_sweep.md)
+constexpr int kIpt4Min = 12288;    // above: 4 particles per thread in fp32, 2 in fp64
+constexpr int kIpt8Min = 32768;    // above: 8 per thread in fp32
+constexpr int kIpt4Min64 = 24576;  // above: 4 per thread in fp64
 
 enum { TENSOR_RPY = 0, TENSOR_OSEEN = 1 };
 enum { ACC_KAHAN = 0, ACC_PLAIN = 1 };
@@ -103,12 +107,16 @@ __device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b) {
 // replaced by d - L n with n = rint(d / L) taken as (fma(d, 1/L, M) - M), M = 1.5 * 2^23: the
 // fma rounds the exact product d * fl(1/L) to an integer, ties to even (reading B2).
 // 3 more packed instructions per component: 29 per two pairs (Rotne-Prager), 26 (Oseen).
-template <int I2, int TENSOR, bool PBC>
+// CLAMP (the "careful" pass, see the kernel): r^2 is clamped from below to k.clampv = 4a^2
+// before the MUFUs, so that every pair -- the self pair and overlapping pairs included -- adds a
+// finite term of ordinary magnitude; the unclamped r^2 of every pair is returned in r2out and
+// the caller corrects the few pairs below the clamp.  Branch-free, 2 FMNMX per two pairs more.
+template <int I2, int TENSOR, bool PBC, bool CLAMP>
 __device__ __forceinline__ void pair_fast_staged(const f32x2 (&xi)[I2], const f32x2 (&yi)[I2],
                                                  const f32x2 (&zi)[I2], const float4 pj,
                                                  const float4 fj, const PairCoef& k,
                                                  f32x2 (&px)[I2], f32x2 (&py)[I2], f32x2 (&pz)[I2],
-                                                 float& mn) {
+                                                 float& mn, float (&r2out)[2 * I2]) {
     f32x2 dx[I2], dy[I2], dz[I2], r2[I2], inv[I2], inv2[I2], dF[I2], A[I2], Bd[I2];
     const f32x2 xj = bc2(pj.x), yj = bc2(pj.y), zj = bc2(pj.z);
     const f32x2 fx = bc2(fj.x), fy = bc2(fj.y), fz = bc2(fj.z);
@@ -138,8 +146,15 @@ __device__ __forceinline__ void pair_fast_staged(const f32x2 (&xi)[I2], const f3
     }
 #pragma unroll
     for (int m = 0; m < I2; ++m) {
-        const float a = lo2(r2[m]), b = hi2(r2[m]);
-        mn = fminf(mn, fminf(a, b));
+        float a = lo2(r2[m]), b = hi2(r2[m]);
+        if (CLAMP) {
+            r2out[2 * m] = a;
+            r2out[2 * m + 1] = b;
+            a = fmaxf(a, k.clampv);
+            b = fmaxf(b, k.clampv);
+        } else {
+            mn = fminf(mn, fminf(a, b));
+        }
         inv[m] = pk2(rsq_approx(a), rsq_approx(b));
         inv2[m] = pk2(rcp_approx(a), rcp_approx(b));
     }
@@ -225,6 +240,39 @@ __device__ __forceinline__ void pair_exact(const float xi, const float yi, const
     pz = fmaf(Bd, dz, pz);
 }
 
+// What the CLAMP body added for one (i, j) whose r^2 lies below the clamp: the far-field formula
+// evaluated with 1/r := 1/sqrt(clampv) on the true d.  Subtracted again by the careful pass (and
+// replaced by pair_exact unless the pair is the self pair).  d = 0 for the self pair: A_c F' only.
+template <int TENSOR, bool PBC>
+__device__ __forceinline__ void pair_clamped_sub(const float xi, const float yi, const float zi,
+                                                 const float4 pj, const float4 fj,
+                                                 const PairCoef& k, float& px, float& py,
+                                                 float& pz) {
+    float dx = xi - pj.x, dy = yi - pj.y, dz = zi - pj.z;
+    if (PBC) {
+        dx = __fmaf_rn(__fsub_rn(__fmaf_rn(dx, k.invL, k.magic), k.magic), k.mL, dx);
+        dy = __fmaf_rn(__fsub_rn(__fmaf_rn(dy, k.invL, k.magic), k.magic), k.mL, dy);
+        dz = __fmaf_rn(__fsub_rn(__fmaf_rn(dz, k.invL, k.magic), k.magic), k.mL, dz);
+    }
+    const float inv = rsq_approx(k.clampv), inv2 = rcp_approx(k.clampv);
+    const float inv3 = inv * inv2;
+    const float dF = fmaf(dz, fj.z, fmaf(dy, fj.y, dx * fj.x));
+    float A, Bd;
+    if (TENSOR == TENSOR_RPY) {
+        A = fmaf(inv3, k.k2, inv);
+        Bd = (inv3 * dF) * fmaf(inv2, k.m3k2, 1.0f);
+    } else {
+        A = inv;
+        Bd = inv3 * dF;
+    }
+    px = fmaf(-A, fj.x, px);
+    py = fmaf(-A, fj.y, py);
+    pz = fmaf(-A, fj.z, pz);
+    px = fmaf(-Bd, dx, px);
+    py = fmaf(-Bd, dy, py);
+    pz = fmaf(-Bd, dz, pz);
+}
+
 __device__ __forceinline__ void kahan_merge2(f32x2& s, f32x2& c, const f32x2 p) {
     const f32x2 y = sub2(p, c);
     const f32x2 t = add2(s, y);
@@ -233,7 +281,7 @@ __device__ __forceinline__ void kahan_merge2(f32x2& s, f32x2& c, const f32x2 p) 
 }
 
 template <int I2, int TENSOR, int ACC, bool PBC>
-__global__ void __launch_bounds__(kThreads, (I2 <= 2) ? 2 : 1)
+__global__ void __launch_bounds__(kThreads, (I2 == 1) ? 3 : ((I2 == 2) ? 2 : 1))
 pairs_f32_kernel(const float4* __restrict__ rec, float4* __restrict__ part, const Schedule sch,
                  const PairCoef k, const int N, const long long slot_stride) {
     constexpr int I = 2 * I2;
@@ -330,15 +378,25 @@ pairs_f32_kernel(const float4* __restrict__ rec, float4* __restrict__ part, cons
                     }
                 }
                 float mn = 3.0e38f;
+                float r2v[2 * I2];
+                const int j0 = jbase + ch * kChunk;
+                // the chunk that holds this warp's own particles (self pairs, r = 0)
+                const int rel = j0 - (i_first - lane);
+                const bool diag = rel >= 0 && (rel % kThreads) == 0 && rel < I * kThreads;
+                if (!diag) {
 #pragma unroll kUnrollJ
-                for (int jj = 0; jj < kChunk; ++jj) {
-                    const float4 pj = cj[2 * jj];
-                    const float4 fj = cj[2 * jj + 1];
-                    pair_fast_staged<I2, TENSOR, PBC>(xi, yi, zi, pj, fj, k, px, py, pz, mn);
+                    for (int jj = 0; jj < kChunk; ++jj) {
+                        const float4 pj = cj[2 * jj];
+                        const float4 fj = cj[2 * jj + 1];
+                        pair_fast_staged<I2, TENSOR, PBC, false>(xi, yi, zi, pj, fj, k, px, py, pz,
+                                                                 mn, r2v);
+                    }
                 }
-                if (mn < k.thr) {
-                    // an overlapping pair or the self pair sits in this chunk: redo it exactly
-                    const int j0 = jbase + ch * kChunk;
+                if (diag || mn < k.thr) {
+                    // careful pass: self pairs, overlapping pairs or coincident centres sit in this
+                    // chunk.  Every pair goes through the clamped packed body (finite terms of
+                    // ordinary size, so nothing cancels); the pairs below the clamp are then put
+                    // right one by one: clamped term out, exact term (none for the self pair) in.
 #pragma unroll
                     for (int m = 0; m < I2; ++m) {
                         if (ACC == ACC_KAHAN) {
@@ -349,26 +407,36 @@ pairs_f32_kernel(const float4* __restrict__ rec, float4* __restrict__ part, cons
                             pz[m] = qz[m];
                         }
                     }
-#pragma unroll 1
+#pragma unroll 2
                     for (int jj = 0; jj < kChunk; ++jj) {
                         const float4 pj = cj[2 * jj];
                         const float4 fj = cj[2 * jj + 1];
                         const int j = j0 + jj;
+                        pair_fast_staged<I2, TENSOR, PBC, true>(xi, yi, zi, pj, fj, k, px, py, pz,
+                                                                mn, r2v);
 #pragma unroll
                         for (int m = 0; m < I2; ++m) {
-                            const int i0 = i_first + (2 * m) * kThreads;
-                            float ax = lo2(px[m]), ay = lo2(py[m]), az = lo2(pz[m]);
-                            float bx = hi2(px[m]), by = hi2(py[m]), bz = hi2(pz[m]);
-                            // pad records (j >= N) are skipped here: under PBC their wrapped
-                            // image can land anywhere in the box
-                            pair_exact<TENSOR, PBC>(lo2(xi[m]), lo2(yi[m]), lo2(zi[m]),
-                                                    j == i0 || j >= N, pj, fj, k, ax, ay, az);
-                            pair_exact<TENSOR, PBC>(hi2(xi[m]), hi2(yi[m]), hi2(zi[m]),
-                                                    j == i0 + kThreads || j >= N, pj, fj, k, bx,
-                                                    by, bz);
-                            px[m] = pk2(ax, bx);
-                            py[m] = pk2(ay, by);
-                            pz[m] = pk2(az, bz);
+                            if (fminf(r2v[2 * m], r2v[2 * m + 1]) < k.clampv && j < N) {
+                                const int i0 = i_first + (2 * m) * kThreads;
+                                float ax = lo2(px[m]), ay = lo2(py[m]), az = lo2(pz[m]);
+                                float bx = hi2(px[m]), by = hi2(py[m]), bz = hi2(pz[m]);
+                                if (r2v[2 * m] < k.clampv) {
+                                    pair_clamped_sub<TENSOR, PBC>(lo2(xi[m]), lo2(yi[m]), lo2(zi[m]),
+                                                                  pj, fj, k, ax, ay, az);
+                                    pair_exact<TENSOR, PBC>(lo2(xi[m]), lo2(yi[m]), lo2(zi[m]),
+                                                            j == i0, pj, fj, k, ax, ay, az);
+                                }
+                                if (r2v[2 * m + 1] < k.clampv) {
+                                    pair_clamped_sub<TENSOR, PBC>(hi2(xi[m]), hi2(yi[m]), hi2(zi[m]),
+                                                                  pj, fj, k, bx, by, bz);
+                                    pair_exact<TENSOR, PBC>(hi2(xi[m]), hi2(yi[m]), hi2(zi[m]),
+                                                            j == i0 + kThreads, pj, fj, k, bx, by,
+                                                            bz);
+                                }
+                                px[m] = pk2(ax, bx);
+                                py[m] = pk2(ay, by);
+                                pz[m] = pk2(az, bz);
+                            }
                         }
                     }
                 }

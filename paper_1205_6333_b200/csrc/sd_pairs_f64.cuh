@@ -36,16 +36,22 @@ __device__ __forceinline__ double min_image_f64(const double d, const PairCoef64
     return fma(__dsub_rn(fma(d, k.invL, k.magic), k.magic), k.mL, d);
 }
 
-template <int TENSOR, bool PBC>
+// CLAMP: the careful pass of the fp32 kernel (sd_pairs_f32.cuh) in fp64: r^2 is clamped from
+// below to k.clampv before 1/r is formed; the true r^2 is returned in r2out.
+template <int TENSOR, bool PBC, bool CLAMP>
 __device__ __forceinline__ void pair_fast_f64(const double xi, const double yi, const double zi,
                                               const double4 pj, const double4 fj,
                                               const PairCoef64& k, double& px, double& py,
-                                              double& pz, float& mn) {
+                                              double& pz, float& mn, double& r2out) {
     const double dx = min_image_f64<PBC>(xi - pj.x, k), dy = min_image_f64<PBC>(yi - pj.y, k),
                  dz = min_image_f64<PBC>(zi - pj.z, k);
-    const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+    double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+    if (CLAMP) {
+        r2out = r2;
+        r2 = fmax(r2, k.clampv);
+    }
     const float r2f = static_cast<float>(r2);
-    mn = fminf(mn, r2f);
+    if (!CLAMP) mn = fminf(mn, r2f);
     const double inv = rsqrt_nr2(r2, r2f);
     const double dF = fma(dz, fj.z, fma(dy, fj.y, dx * fj.x));
     const double inv2 = inv * inv;
@@ -110,8 +116,36 @@ __device__ __forceinline__ void pair_exact_f64(const double xi, const double yi,
     pz = fma(Bd, dz, pz);
 }
 
+// the term the CLAMP body added for a pair below the clamp, subtracted again (see the fp32 kernel)
+template <int TENSOR, bool PBC>
+__device__ __forceinline__ void pair_clamped_sub_f64(const double xi, const double yi,
+                                                     const double zi, const double4 pj,
+                                                     const double4 fj, const PairCoef64& k,
+                                                     double& px, double& py, double& pz) {
+    const double dx = min_image_f64<PBC>(xi - pj.x, k), dy = min_image_f64<PBC>(yi - pj.y, k),
+                 dz = min_image_f64<PBC>(zi - pj.z, k);
+    const double inv = rsqrt_nr2(k.clampv, static_cast<float>(k.clampv));
+    const double dF = fma(dz, fj.z, fma(dy, fj.y, dx * fj.x));
+    const double inv2 = inv * inv;
+    const double inv3 = inv2 * inv;
+    double A, Bd;
+    if (TENSOR == TENSOR_RPY) {
+        A = fma(k.k2, inv3, inv);
+        Bd = fma(k.m3k2, inv2, 1.0) * (inv3 * dF);
+    } else {
+        A = inv;
+        Bd = inv3 * dF;
+    }
+    px = fma(-A, fj.x, px);
+    py = fma(-A, fj.y, py);
+    pz = fma(-A, fj.z, pz);
+    px = fma(-Bd, dx, px);
+    py = fma(-Bd, dy, py);
+    pz = fma(-Bd, dz, pz);
+}
+
 template <int I, int TENSOR, bool PBC>
-__global__ void __launch_bounds__(kThreads, (I <= 2) ? 2 : 1)
+__global__ void __launch_bounds__(kThreads, (I == 1) ? 3 : ((I == 2) ? 2 : 1))
 pairs_f64_kernel(const double4* __restrict__ rec, double4* __restrict__ part, const Schedule sch,
                  const PairCoef64 k, const float thr, const int N, const long long slot_stride) {
     constexpr int IB = kThreads * I;
@@ -191,33 +225,45 @@ pairs_f64_kernel(const double4* __restrict__ rec, double4* __restrict__ part, co
                     qz[m] = pz[m];
                 }
                 float mn = 3.0e38f;
+                double r2t;
+                const int j0 = jbase + ch * kChunk;
+                const int rel = j0 - (i_first - lane);  // chunk holding this warp's own particles?
+                const bool diag = rel >= 0 && (rel % kThreads) == 0 && rel < I * kThreads;
+                if (!diag) {
 #pragma unroll 4
-                for (int jj = 0; jj < kChunk; ++jj) {
-                    const double4 pj = cj[2 * jj];
-                    const double4 fj = cj[2 * jj + 1];
+                    for (int jj = 0; jj < kChunk; ++jj) {
+                        const double4 pj = cj[2 * jj];
+                        const double4 fj = cj[2 * jj + 1];
 #pragma unroll
-                    for (int m = 0; m < I; ++m)
-                        pair_fast_f64<TENSOR, PBC>(xi[m], yi[m], zi[m], pj, fj, k, px[m], py[m], pz[m],
-                                                   mn);
+                        for (int m = 0; m < I; ++m)
+                            pair_fast_f64<TENSOR, PBC, false>(xi[m], yi[m], zi[m], pj, fj, k, px[m],
+                                                              py[m], pz[m], mn, r2t);
+                    }
                 }
-                if (mn < thr) {
-                    const int j0 = jbase + ch * kChunk;
+                if (diag || mn < thr) {  // careful pass, as in the fp32 kernel
 #pragma unroll
                     for (int m = 0; m < I; ++m) {
                         px[m] = qx[m];
                         py[m] = qy[m];
                         pz[m] = qz[m];
                     }
-#pragma unroll 1
+#pragma unroll 2
                     for (int jj = 0; jj < kChunk; ++jj) {
                         const double4 pj = cj[2 * jj];
                         const double4 fj = cj[2 * jj + 1];
                         const int j = j0 + jj;
 #pragma unroll
-                        for (int m = 0; m < I; ++m)
-                            pair_exact_f64<TENSOR, PBC>(xi[m], yi[m], zi[m],
-                                                        j == i_first + m * kThreads || j >= N, pj,
-                                                        fj, k, px[m], py[m], pz[m]);
+                        for (int m = 0; m < I; ++m) {
+                            pair_fast_f64<TENSOR, PBC, true>(xi[m], yi[m], zi[m], pj, fj, k, px[m],
+                                                             py[m], pz[m], mn, r2t);
+                            if (r2t < k.clampv && j < N) {
+                                pair_clamped_sub_f64<TENSOR, PBC>(xi[m], yi[m], zi[m], pj, fj, k,
+                                                                  px[m], py[m], pz[m]);
+                                pair_exact_f64<TENSOR, PBC>(xi[m], yi[m], zi[m],
+                                                            j == i_first + m * kThreads, pj, fj, k,
+                                                            px[m], py[m], pz[m]);
+                            }
+                        }
                     }
                 }
             }

@@ -25,7 +25,7 @@
 
 namespace sd {
 
-constexpr int kSmallApplyMax = 4096;  // above this the tiled packed kernel wins (measured)
+constexpr int kSmallApplyMax = 2560;  // above this the tiled packed kernel wins (measured)
 constexpr int kStepperMax = 64;   // above this one launch per product is faster (measured)
 constexpr int kSmallThreads = 256;
 constexpr int kSmallTile = 256;

@@ -60,9 +60,12 @@ pack_kernel(const T4* __restrict__ pos, const T4* __restrict__ force, T4* __rest
     }
 }
 
+constexpr int kFinThreads = 128;
+constexpr int kFinBatch = 8;
+
 // fp32 modes.  part: [slot][Nrec][2] float4 (hi, lo), value = hi - lo.
 template <int MODE>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(kFinThreads)
 finalize_f32_kernel(const float4* __restrict__ part, const int* __restrict__ blk_nslots,
                     float4* __restrict__ rec, float4* __restrict__ vel, float4* __restrict__ pos,
                     float4* __restrict__ pos_lo, float4* __restrict__ pos_half, const double dt,
@@ -74,13 +77,26 @@ finalize_f32_kernel(const float4* __restrict__ part, const int* __restrict__ blk
     double vx = mu0r * static_cast<double>(f.x);   // self term mu0 F_i = (mu0 / c1) (c1 F_i)
     double vy = mu0r * static_cast<double>(f.y);
     double vz = mu0r * static_cast<double>(f.z);
-    for (int s = 0; s < nslots; ++s) {
-        const float4* p = part + (static_cast<size_t>(s) * slot_stride + i) * 2;
-        const float4 hi = p[0];
-        const float4 lo = p[1];
-        vx += static_cast<double>(hi.x) - static_cast<double>(lo.x);
-        vy += static_cast<double>(hi.y) - static_cast<double>(lo.y);
-        vz += static_cast<double>(hi.z) - static_cast<double>(lo.z);
+    // slots in batches of kFinBatch: the loads of a batch are in flight together (a small-N
+    // product has up to T slots per row and this kernel is pure latency); the sum keeps slot order
+    for (int s0 = 0; s0 < nslots; s0 += kFinBatch) {
+        float4 hi[kFinBatch], lo[kFinBatch];
+#pragma unroll
+        for (int q = 0; q < kFinBatch; ++q) {
+            if (s0 + q < nslots) {
+                const float4* p = part + (static_cast<size_t>(s0 + q) * slot_stride + i) * 2;
+                hi[q] = p[0];
+                lo[q] = p[1];
+            }
+        }
+#pragma unroll
+        for (int q = 0; q < kFinBatch; ++q) {
+            if (s0 + q < nslots) {
+                vx += static_cast<double>(hi[q].x) - static_cast<double>(lo[q].x);
+                vy += static_cast<double>(hi[q].y) - static_cast<double>(lo[q].y);
+                vz += static_cast<double>(hi[q].z) - static_cast<double>(lo[q].z);
+            }
+        }
     }
     vel[i] = make_float4(static_cast<float>(vx), static_cast<float>(vy), static_cast<float>(vz), 0.f);
     if (MODE == FIN_VEL) return;
@@ -104,7 +120,7 @@ finalize_f32_kernel(const float4* __restrict__ part, const int* __restrict__ blk
 
 // fp64 mode.  part: [slot][Nrec] double4.
 template <int MODE>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(kFinThreads)
 finalize_f64_kernel(const double4* __restrict__ part, const int* __restrict__ blk_nslots,
                     double4* __restrict__ rec, double4* __restrict__ vel,
                     double4* __restrict__ pos, double4* __restrict__ pos_half, const double dt,
@@ -114,11 +130,19 @@ finalize_f64_kernel(const double4* __restrict__ part, const int* __restrict__ bl
     const int nslots = blk_nslots[i / IB];
     const double4 f = rec[2 * static_cast<size_t>(i) + 1];
     double vx = mu0r * f.x, vy = mu0r * f.y, vz = mu0r * f.z;
-    for (int s = 0; s < nslots; ++s) {
-        const double4 p = part[static_cast<size_t>(s) * slot_stride + i];
-        vx += p.x;
-        vy += p.y;
-        vz += p.z;
+    for (int s0 = 0; s0 < nslots; s0 += kFinBatch) {
+        double4 p[kFinBatch];
+#pragma unroll
+        for (int q = 0; q < kFinBatch; ++q)
+            if (s0 + q < nslots) p[q] = part[static_cast<size_t>(s0 + q) * slot_stride + i];
+#pragma unroll
+        for (int q = 0; q < kFinBatch; ++q) {
+            if (s0 + q < nslots) {
+                vx += p[q].x;
+                vy += p[q].y;
+                vz += p[q].z;
+            }
+        }
     }
     vel[i] = make_double4(vx, vy, vz, 0.0);
     if (MODE == FIN_VEL) return;

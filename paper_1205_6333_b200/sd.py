@@ -33,6 +33,7 @@ SYMBOLS = {
     "sd_create": (_I, [ctypes.POINTER(_P), _LL, _D, _D]),
     "sd_set_tensor": (_I, [_P, _I]),
     "sd_set_precision": (_I, [_P, _I]),
+    "sd_set_dispatch": (_I, [_P, _LL, _I]),
     "sd_set_box": (_I, [_P, _D]),
     "sd_box": (_D, [_P]),
     "sd_mobility_apply": (_I, [_P, _P, _P, _P, _P]),
@@ -122,6 +123,11 @@ class Context:
     def set_precision(self, precision: int):
         self._check(self._lib.sd_set_precision(self._h, int(precision)))
         self.precision = int(precision)
+
+    def set_dispatch(self, small_apply_max: int = -1, particles_per_thread: int = 0):
+        """Dispatch knobs of the small-N path (ablations / tests); defaults = measured crossovers."""
+        self._check(self._lib.sd_set_dispatch(self._h, int(small_apply_max),
+                                              int(particles_per_thread)))
 
     def set_box(self, box_side: float):
         """Periodic cube of that side, nearest image only; 0 = free space."""

@@ -43,11 +43,13 @@ def box_as_seen(L, prec_name):
     return float(np.float32(L)) if prec_name != "PREC_F64" else float(L)
 
 
-def gpu_apply_box(torch, sd, pos, force, L, prec_name, tensor, expect_kernel=None):
+def gpu_apply_box(torch, sd, pos, force, L, prec_name, tensor, expect_kernel=None,
+                  dispatch=(-1, 0)):
     p, f = rounded(pos, prec_name), rounded(force, prec_name)
     ctx = sd.Context(pos.shape[0], wl.A, wl.ETA)
     ctx.set_precision(getattr(sd, prec_name))
     ctx.set_tensor(tensor)
+    ctx.set_dispatch(*dispatch)
     ctx.set_box(L)
     assert ctx.box == L
     if expect_kernel is not None:
@@ -68,7 +70,9 @@ def gpu_apply_box(torch, sd, pos, force, L, prec_name, tensor, expect_kernel=Non
 @pytest.mark.parametrize("prec_name", ["PREC_F32_KAHAN", "PREC_F64"])
 @pytest.mark.parametrize("tname", ["rpy", "oseen"])
 @pytest.mark.parametrize("forces", ["gravity", "normal"])
-def test_fcc_4000_small_path_all_rows(gpu, prec_name, tname, forces):
+@pytest.mark.parametrize("path", ["small_apply", "pairs_f"])
+def test_fcc_4000_all_rows(gpu, prec_name, tname, forces, path):
+    """N = 4000 through the one-launch kernel (forced) and through the tiled kernels (default)."""
     torch, sd = gpu
     cells = 10
     pos = wl.fcc_lattice(cells, 0.1, jitter_seed=wl.SEED_BASE + 20)
@@ -76,7 +80,8 @@ def test_fcc_4000_small_path_all_rows(gpu, prec_name, tname, forces):
     n = pos.shape[0]
     assert n == 4000
     F = wl.gravity_forces(n) if forces == "gravity" else wl.normal_forces(n, wl.SEED_BASE + 21)
-    got, p, f = gpu_apply_box(torch, sd, pos, F, L, prec_name, TENSOR[tname][0], "small_apply")
+    got, p, f = gpu_apply_box(torch, sd, pos, F, L, prec_name, TENSOR[tname][0], path,
+                              dispatch=(1 << 20, 0) if path == "small_apply" else (-1, 0))
     want = orc.apply(p, f, wl.A, wl.ETA, TENSOR[tname][1], box=box_as_seen(L, prec_name),
                      image=IMAGE[prec_name])
     assert rel_err(got, want) <= TOL[prec_name]
@@ -186,10 +191,12 @@ def test_large_box_is_free_space_and_box_can_be_switched_off(gpu):
                                                  ("PREC_F64", 1e-9, 1.02),
                                                  ("PREC_F64", 1e-9, 1.0)])
 @pytest.mark.parametrize("cells,integ,steps,dt", [(2, "midpoint", 1000, 0.01),
+                                                  (8, "midpoint", 30, 0.005),
                                                   (10, "euler", 100, 0.001),
-                                                  (11, "midpoint", 20, 0.005)])
+                                                  (16, "midpoint", 5, 0.005)])
 def test_step_in_periodic_box(gpu, prec_name, tol, scale, cells, integ, steps, dt):
-    """N = 32 (one-launch stepper), 4000 (one launch per product), 5324 (tiled kernels)."""
+    """N = 32 (one-launch stepper), 2048 (one launch per product), 4000 and 16384 (tiled kernels
+    with 2 and 4 particles per thread)."""
     torch, sd = gpu
     pos = wl.fcc_lattice(cells, 0.1, jitter_seed=wl.SEED_BASE + 31 + cells)
     L = scale * wl.fcc_box(cells, 0.1)

@@ -53,7 +53,7 @@ def gpu_apply(torch, sd, pos, force, prec, tensor, a=wl.A, eta=wl.ETA):
     torch.cuda.synchronize()
     out = dv.cpu().numpy()
     assert np.all(out[:, 3] == 0.0)  # pad lane written as 0
-    assert ctx.launch_count >= (1 if pos.shape[0] <= 4096 else 3)  # our kernels ran
+    assert ctx.launch_count >= (1 if pos.shape[0] <= 2560 else 3)  # our kernels ran
     ctx.close()
     return out[:, :3].astype(np.float64), p[:, :3].astype(np.float64), f[:, :3].astype(np.float64)
 
@@ -310,12 +310,14 @@ def test_ragged_sizes_large_kernels(gpu, n):
 
 
 @pytest.mark.parametrize("n,integ", [(4, "INT_EULER"), (33, "INT_MIDPOINT"), (64, "INT_EULER"),
-                                     (65, "INT_EULER"), (300, "INT_MIDPOINT"), (5000, "INT_EULER"),
-                                     (9000, "INT_MIDPOINT"), (9000, "INT_EULER")])
+                                     (65, "INT_EULER"), (300, "INT_MIDPOINT"), (2500, "INT_EULER"),
+                                     (2500, "INT_MIDPOINT"), (5000, "INT_EULER"),
+                                     (9000, "INT_MIDPOINT"), (9000, "INT_EULER"),
+                                     (14000, "INT_MIDPOINT")])
 @pytest.mark.parametrize("prec_name", ["PREC_F32_KAHAN", "PREC_F64"])
 def test_step_paths_agree_with_oracle(gpu, n, integ, prec_name):
     """sd_step through every dispatch path (persistent stepper N <= 64, one-launch-per-product
-    N <= 4096, tiled kernels above), odd step counts (ping-pong buffers), per-particle forces."""
+    N <= 2560, tiled kernels with 2 / 4 particles per thread above), odd step counts (ping-pong buffers), per-particle forces."""
     torch, sd = gpu
     prec = getattr(sd, prec_name)
     dtp = np_dtype(sd, prec)
@@ -448,3 +450,45 @@ def test_invalid_arguments_are_reported(gpu):
     ctx.step(t, 0.1, 0, sd.INT_EULER, gravity=(0, 0, -1))  # zero steps: no-op
     assert ctx.self_mobility == pytest.approx(1.0 / (6 * math.pi))
     ctx.close()
+
+
+# ---- dispatch knobs: every tiled variant on small clouds, all rows (careful pass coverage) ------
+
+@pytest.mark.parametrize("prec_name,tol", [("PREC_F32_KAHAN", TOL_F32), ("PREC_F64", TOL_F64)])
+@pytest.mark.parametrize("tname", ["TENSOR_RPY", "TENSOR_OSEEN"])
+@pytest.mark.parametrize("ipt", [2, 4, 8])
+def test_forced_tiled_kernels_on_dense_small_clouds(gpu, prec_name, tol, tname, ipt):
+    """sd_set_dispatch(0, ipt) sends small N through the tiled packed kernels.  Dense clouds
+    (phi = 0.2, overlaps allowed: ~1.6 overlapping neighbours per sphere, plus two coincident
+    centres) put self pairs, overlapping pairs and r = 0 pairs into most chunks, i.e. they
+    exercise the clamped careful pass and its per-pair corrections on every row."""
+    torch, sd = gpu
+    prec, tensor = getattr(sd, prec_name), getattr(sd, tname)
+    otensor = orc.TENSOR_RPY if tname == "TENSOR_RPY" else orc.TENSOR_OSEEN
+    for n in (257, 3000):
+        pos = wl.uniform_cube(n, 0.2, wl.SEED_BASE + 40 + n)
+        pos[n // 2] = pos[3]                       # coincident centres, j != i (reading A5)
+        force = wl.normal_forces(n, wl.SEED_BASE + 41 + n)
+        dt = np_dtype(sd, prec)
+        p, f = wl.to_xyzw(pos, dt), wl.to_xyzw(force, dt)
+        ctx = sd.Context(n, wl.A, wl.ETA)
+        ctx.set_precision(prec)
+        ctx.set_tensor(tensor)
+        ctx.set_dispatch(0, ipt)
+        assert "pairs_f" in ctx.kernel_name
+        dp, df = torch.from_numpy(p).cuda(), torch.from_numpy(f).cuda()
+        dv = torch.full_like(dp, float("nan"))
+        ctx.mobility_apply(dp, df, dv)
+        torch.cuda.synchronize()
+        got = dv.cpu().numpy()[:, :3].astype(np.float64)
+        want = orc.apply(p[:, :3].astype(np.float64), f[:, :3].astype(np.float64), wl.A, wl.ETA,
+                         otensor)
+        assert rel_err(got, want) <= tol
+        # default dispatch (one-launch kernel at this N) agrees as well
+        ctx.set_dispatch(-1, 0)
+        ctx.mobility_apply(dp, df, dv)
+        torch.cuda.synchronize()
+        assert rel_err(dv.cpu().numpy()[:, :3].astype(np.float64), want) <= tol
+        with pytest.raises(sd.SdError):
+            ctx.set_dispatch(0, 3)
+        ctx.close()
