@@ -48,6 +48,8 @@ def parse_args():
                     help="instead of the product: the paper's benchmark run (PAPER.md:231), fcc "
                          "lattice of 4 cells^3 spheres at n = 0.1 a^-3 in its periodic box, 100 "
                          "Euler steps of 0.001 tau_s per timed step; reports simulation steps/s")
+    ap.add_argument("--staging", choices=["bulk", "naive", "sync"], default="bulk",
+                    help="memory-access ablation (PAPER.md Appendix A): how j records reach the threads")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
 
@@ -61,7 +63,8 @@ def workload(n):
 def workload_name(args):
     return (f"sd_mobility_apply N={args.n} uniform cube phi=0.01, N(0,1) forces, "
             f"{args.tensor.upper()}, {'fp32-Kahan' if args.precision == 'f32' else 'fp64'}"
-            + (", periodic box (nearest image)" if args.box else ""))
+            + (", periodic box (nearest image)" if args.box else "")
+            + (f", staging={args.staging}" if args.staging != "bulk" else ""))
 
 
 def box_side(args, wl):
@@ -275,6 +278,7 @@ def main():
     ctx.set_precision(prec)
     ctx.set_tensor(tensor)
     ctx.set_box(box_side(args, wl))
+    ctx.set_staging({"bulk": 0, "naive": 1, "sync": 2}[args.staging])
     peak_probe = ctx.fma_peak_probe(prec)
 
     def barrier():

@@ -86,6 +86,16 @@ sd_status sd_set_precision(sd_ctx* ctx, sd_precision precision);
  * Reallocates the scratch buffers; synchronises the device. */
 sd_status sd_set_dispatch(sd_ctx* ctx, long long small_apply_max, int particles_per_thread);
 
+/* Ablation of the memory-access schemes the paper compares (PAPER.md:111-241 and Appendix A): how
+ * the j records reach the threads of the tiled kernel.
+ *   0  bulk asynchronous copies into a ring of shared-memory tiles (default, the product path)
+ *   1  "naive" (Alg. 1): every thread loads each record from global memory, one address per warp
+ *   2  "tiling" (Alg. 2): the block copies a tile into shared memory between two barriers
+ * Modes 1 and 2 exist for SD_TENSOR_RPY + SD_PREC_F32_KAHAN in free space only; otherwise, and
+ * for any later change away from that combination, SD_ERR_UNSUPPORTED is returned and the context
+ * is left unchanged.  Results are bit-identical across modes. */
+sd_status sd_set_staging(sd_ctx* ctx, int mode);
+
 /* Boundary conditions (footnote 1: "a simulation box with periodic boundaries and
  * include only hydrodynamic interactions from the nearest image of each particle").
  * box_side = 0 (default): free space.  box_side = L > 0: periodic cube of side L; every

@@ -47,6 +47,7 @@ struct sd_ctx {
     double box = 0.0;  // side of the periodic cube; 0 = free space
     long long small_apply_max = sd::kSmallApplyMax;  // N up to which the one-launch kernel runs
     int ipt_override = 0;                            // particles per thread; 0 = automatic
+    int staging = 0;                                 // sd::STAGE_* (ablation, fp32 RPY Kahan only)
     int device = 0;
     int num_sms = 0;
     Config cfg;
@@ -160,9 +161,27 @@ sd_status configure(sd_ctx* c) {
             cfg.kernel = pbc ? f32_pick<2, true>(rpy, plain) : f32_pick<2, false>(rpy, plain);
         else
             cfg.kernel = pbc ? f32_pick<1, true>(rpy, plain) : f32_pick<1, false>(rpy, plain);
+        if (c->staging != sd::STAGE_BULK) {  // ablation variants: RPY, Kahan, free space only
+            if (!rpy || plain || pbc)
+                return fail(c, SD_ERR_UNSUPPORTED,
+                            "staging ablation exists for RPY, fp32-Kahan, free space only: call sd_set_staging(ctx, 0) first");
+            const bool naive = c->staging == sd::STAGE_NAIVE;
+#define SD_STAGED(I2V)                                                                              \
+    (naive ? reinterpret_cast<const void*>(&sd::pairs_f32_kernel<I2V, 0, 0, false, sd::STAGE_NAIVE>) \
+           : reinterpret_cast<const void*>(&sd::pairs_f32_kernel<I2V, 0, 0, false, sd::STAGE_SYNC>))
+            cfg.kernel = (i2 == 4) ? SD_STAGED(4) : ((i2 == 2) ? SD_STAGED(2) : SD_STAGED(1));
+#undef SD_STAGED
+            static const char* snames[2][3] = {
+                {"pairs_f32x2_i2_rpy_kahan_naive", "pairs_f32x2_i4_rpy_kahan_naive", "pairs_f32x2_i8_rpy_kahan_naive"},
+                {"pairs_f32x2_i2_rpy_kahan_sync", "pairs_f32x2_i4_rpy_kahan_sync", "pairs_f32x2_i8_rpy_kahan_sync"}};
+            cfg.name = snames[naive ? 0 : 1][i2 == 4 ? 2 : (i2 == 2 ? 1 : 0)];
+        }
     } else {
         // 4 particles per thread (one CTA per SM) once 1024-particle i-blocks balance over the
         // SMs: one LDS.128 per pair instead of two; 2 and 1 below (measured crossovers)
+        if (c->staging != sd::STAGE_BULK)
+            return fail(c, SD_ERR_UNSUPPORTED,
+                        "staging ablation exists for RPY, fp32-Kahan, free space only: call sd_set_staging(ctx, 0) first");
         cfg.ipt = (c->N > sd::kIpt4Min64) ? 4 : (c->N > sd::kIpt4Min ? 2 : 1);
         if (c->ipt_override) cfg.ipt = std::max(1, c->ipt_override / 2);
         cfg.TJ = sd::kTJ64;
@@ -485,11 +504,22 @@ sd_status sd_create(sd_ctx** out, long long N, double a, double eta) {
     return SD_OK;
 }
 
+namespace {
+// with a non-default staging (ablation) only RPY + fp32-Kahan + free space exists
+bool staging_forbids(const sd_ctx* c, int tensor, int precision, double box) {
+    return c->staging != sd::STAGE_BULK &&
+           (tensor != SD_TENSOR_RPY || precision != SD_PREC_F32_KAHAN || box > 0.0);
+}
+const char* kStagingMsg =
+    "the staging ablation exists for RPY, fp32-Kahan, free space only: call sd_set_staging(ctx, 0) first";
+}  // namespace
+
 sd_status sd_set_tensor(sd_ctx* ctx, sd_tensor tensor) {
     if (!ctx) return fail(nullptr, SD_ERR_INVALID_ARG, "sd_set_tensor: ctx is NULL");
     if (tensor != SD_TENSOR_RPY && tensor != SD_TENSOR_OSEEN)
         return fail(ctx, SD_ERR_INVALID_ARG, "sd_set_tensor: unknown tensor");
     if (static_cast<int>(tensor) == ctx->tensor) return SD_OK;
+    if (staging_forbids(ctx, tensor, ctx->precision, ctx->box)) return fail(ctx, SD_ERR_UNSUPPORTED, kStagingMsg);
     cudaDeviceSynchronize();
     ctx->tensor = tensor;
     return configure(ctx);
@@ -500,6 +530,7 @@ sd_status sd_set_precision(sd_ctx* ctx, sd_precision precision) {
     if (precision != SD_PREC_F32_KAHAN && precision != SD_PREC_F64 && precision != SD_PREC_F32_PLAIN)
         return fail(ctx, SD_ERR_INVALID_ARG, "sd_set_precision: unknown precision");
     if (static_cast<int>(precision) == ctx->precision) return SD_OK;
+    if (staging_forbids(ctx, ctx->tensor, precision, ctx->box)) return fail(ctx, SD_ERR_UNSUPPORTED, kStagingMsg);
     cudaDeviceSynchronize();
     ctx->precision = precision;
     return configure(ctx);
@@ -516,12 +547,31 @@ sd_status sd_set_dispatch(sd_ctx* ctx, long long small_apply_max, int particles_
     return configure(ctx);
 }
 
+sd_status sd_set_staging(sd_ctx* ctx, int mode) {
+    if (!ctx) return fail(nullptr, SD_ERR_INVALID_ARG, "sd_set_staging: ctx is NULL");
+    if (mode != sd::STAGE_BULK && mode != sd::STAGE_NAIVE && mode != sd::STAGE_SYNC)
+        return fail(ctx, SD_ERR_INVALID_ARG, "sd_set_staging: mode must be 0 (bulk copies), 1 (naive) or 2 (tiled with barriers)");
+    if (mode == ctx->staging) return SD_OK;
+    cudaDeviceSynchronize();
+    const int old = ctx->staging;
+    ctx->staging = mode;
+    sd_status s = configure(ctx);
+    if (s != SD_OK) {  // unsupported combination: keep the context usable
+        const std::string msg = ctx->err;
+        ctx->staging = old;
+        configure(ctx);
+        ctx->err = msg;
+    }
+    return s;
+}
+
 sd_status sd_set_box(sd_ctx* ctx, double box_side) {
     if (!ctx) return fail(nullptr, SD_ERR_INVALID_ARG, "sd_set_box: ctx is NULL");
     if (!(box_side >= 0.0) || !std::isfinite(box_side))
         return fail(ctx, SD_ERR_INVALID_ARG, "sd_set_box: box side must be finite and >= 0 (0 = free space)");
     if (box_side > 0.0 && !(static_cast<float>(box_side) > 0.0f) )
         return fail(ctx, SD_ERR_INVALID_ARG, "sd_set_box: box side underflows in fp32");
+    if (staging_forbids(ctx, ctx->tensor, ctx->precision, box_side)) return fail(ctx, SD_ERR_UNSUPPORTED, kStagingMsg);
     const bool was = ctx->box > 0.0, is = box_side > 0.0;
     ctx->box = box_side;
     if (was == is) return SD_OK;  // same kernels, only the constants change

@@ -36,7 +36,10 @@ constexpr int kTJ = 128;     // j records per tile (4 KiB)
 constexpr int kStages = 4;   // ring depth
 constexpr int kPrefetch = 2; // tiles in flight ahead of the one being consumed
 constexpr int kChunk = 32;   // j per compensation chunk
-constexpr int kUnrollJ = 4;  // j per unrolled loop body
+#ifndef SD_UNROLL_J
+#define SD_UNROLL_J 4
+#endif
+constexpr int kUnrollJ = SD_UNROLL_J;  // j per unrolled loop body
 // measured crossovers of the particles-per-thread variants (profiles/r01c_sweep.md)
 constexpr int kIpt4Min = 12288;    // above: 4 particles per thread in fp32, 2 in fp64
 constexpr int kIpt8Min = 32768;    // above: 8 per thread in fp32
@@ -44,6 +47,13 @@ constexpr int kIpt4Min64 = 24576;  // above: 4 per thread in fp64
 
 enum { TENSOR_RPY = 0, TENSOR_OSEEN = 1 };
 enum { ACC_KAHAN = 0, ACC_PLAIN = 1 };
+// How the j records reach the threads (ablation of PAPER.md:111-241, Appendix A; sd_set_staging):
+//   STAGE_BULK  bulk async copies (TMA engine) into a ring of shared-memory tiles, mbarriers only
+//   STAGE_NAIVE no staging: every thread loads the record from global memory (one address per
+//               warp, broadcast through L1), the paper's "naive" scheme (Alg. 1)
+//   STAGE_SYNC  the CTA copies a tile into shared memory between two __syncthreads, the paper's
+//               "tiling" scheme (Alg. 2 generalised from one warp to the whole block)
+enum { STAGE_BULK = 0, STAGE_NAIVE = 1, STAGE_SYNC = 2 };
 
 __device__ __forceinline__ float rsq_approx(float x) {
     float y;
@@ -156,7 +166,11 @@ __device__ __forceinline__ void pair_fast_staged(const f32x2 (&xi)[I2], const f3
             mn = fminf(mn, fminf(a, b));
         }
         inv[m] = pk2(rsq_approx(a), rsq_approx(b));
+#ifdef SD_INV2_MUL
+        inv2[m] = mul2(inv[m], inv[m]);
+#else
         inv2[m] = pk2(rcp_approx(a), rcp_approx(b));
+#endif
     }
 #pragma unroll
     for (int m = 0; m < I2; ++m) dF[m] = mul2(dx[m], fx);
@@ -280,12 +294,13 @@ __device__ __forceinline__ void kahan_merge2(f32x2& s, f32x2& c, const f32x2 p) 
     s = t;
 }
 
-template <int I2, int TENSOR, int ACC, bool PBC>
+template <int I2, int TENSOR, int ACC, bool PBC, int STAGE = STAGE_BULK>
 __global__ void __launch_bounds__(kThreads, (I2 == 1) ? 3 : ((I2 == 2) ? 2 : 1))
 pairs_f32_kernel(const float4* __restrict__ rec, float4* __restrict__ part, const Schedule sch,
                  const PairCoef k, const int N, const long long slot_stride) {
     constexpr int I = 2 * I2;
     constexpr int IB = kThreads * I;
+    static_assert(kTJ * 2 == kThreads, "STAGE_SYNC copies one float4 of the tile per thread");
     __shared__ __align__(128) float4 tiles[kStages][kTJ * 2];
     __shared__ __align__(8) uint64_t full_bar[kStages];
     __shared__ __align__(8) uint64_t empty_bar[kStages];
@@ -320,7 +335,7 @@ pairs_f32_kernel(const float4* __restrict__ rec, float4* __restrict__ part, cons
         if (++pf_t == T) pf_t = 0;
     };
     if (tid == 0) {
-        for (int q = 0; q < kPrefetch && pf_n < n_units; ++q) produce();
+        for (int q = 0; STAGE == STAGE_BULK && q < kPrefetch && pf_n < n_units; ++q) produce();
     }
 
     int n = 0;  // tiles consumed so far by this CTA
@@ -357,10 +372,20 @@ pairs_f32_kernel(const float4* __restrict__ rec, float4* __restrict__ part, cons
         }
 
         for (int tt = 0; tt < nt; ++tt, ++n) {
-            if (tid == 0 && pf_n < n_units) produce();
             const int s = n % kStages;
-            mbar_wait(&full_bar[s], (n / kStages) & 1);
-            const float4* tile = &tiles[s][0];
+            const float4* tile;
+            if (STAGE == STAGE_BULK) {
+                if (tid == 0 && pf_n < n_units) produce();
+                mbar_wait(&full_bar[s], (n / kStages) & 1);
+                tile = &tiles[s][0];
+            } else if (STAGE == STAGE_NAIVE) {
+                tile = rec + static_cast<size_t>(t0 + tt) * (kTJ * 2);
+            } else {
+                __syncthreads();  // everybody is done with the previous tile
+                tiles[0][tid] = rec[static_cast<size_t>(t0 + tt) * (kTJ * 2) + tid];
+                __syncthreads();
+                tile = &tiles[0][0];
+            }
             const int jbase = (t0 + tt) * kTJ;
 
 #pragma unroll 1
@@ -449,8 +474,10 @@ pairs_f32_kernel(const float4* __restrict__ rec, float4* __restrict__ part, cons
                     }
                 }
             }
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&empty_bar[s]);
+            if (STAGE == STAGE_BULK) {
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&empty_bar[s]);
+            }
         }
 
         // partial sums of this segment: value = hi - lo

@@ -23,6 +23,7 @@ OK, ERR_INVALID_ARG, ERR_ALLOC, ERR_CUDA, ERR_UNSUPPORTED = 0, 1, 2, 3, 4
 TENSOR_RPY, TENSOR_OSEEN = 0, 1
 PREC_F32_KAHAN, PREC_F64, PREC_F32_PLAIN = 0, 1, 2
 INT_EULER, INT_MIDPOINT = 0, 1
+STAGE_BULK, STAGE_NAIVE, STAGE_SYNC = 0, 1, 2
 
 FORCE_FN = ctypes.CFUNCTYPE(ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_longlong,
                             ctypes.c_void_p, ctypes.c_void_p)
@@ -34,6 +35,7 @@ SYMBOLS = {
     "sd_set_tensor": (_I, [_P, _I]),
     "sd_set_precision": (_I, [_P, _I]),
     "sd_set_dispatch": (_I, [_P, _LL, _I]),
+    "sd_set_staging": (_I, [_P, _I]),
     "sd_set_box": (_I, [_P, _D]),
     "sd_box": (_D, [_P]),
     "sd_mobility_apply": (_I, [_P, _P, _P, _P, _P]),
@@ -128,6 +130,10 @@ class Context:
         """Dispatch knobs of the small-N path (ablations / tests); defaults = measured crossovers."""
         self._check(self._lib.sd_set_dispatch(self._h, int(small_apply_max),
                                               int(particles_per_thread)))
+
+    def set_staging(self, mode: int):
+        """Memory-access ablation (Appendix A): 0 bulk copies, 1 naive, 2 tiled + barriers."""
+        self._check(self._lib.sd_set_staging(self._h, int(mode)))
 
     def set_box(self, box_side: float):
         """Periodic cube of that side, nearest image only; 0 = free space."""

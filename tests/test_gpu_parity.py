@@ -492,3 +492,47 @@ def test_forced_tiled_kernels_on_dense_small_clouds(gpu, prec_name, tol, tname, 
         with pytest.raises(sd.SdError):
             ctx.set_dispatch(0, 3)
         ctx.close()
+
+
+# ---- memory-access ablation (Appendix A): same bits through every staging -----
+
+@pytest.mark.parametrize("n", [3000, 20000, 140000])
+def test_staging_modes_are_bit_identical_and_guarded(gpu, n):
+    """sd_set_staging: bulk-copy ring (default), naive global loads (Alg. 1), block tiling with
+    barriers (Alg. 2).  The arithmetic and its order do not depend on how a record arrives."""
+    torch, sd = gpu
+    pos = wl.uniform_cube(n, 0.05, wl.SEED_BASE + 60 + n)
+    force = wl.normal_forces(n, wl.SEED_BASE + 61 + n)
+    p, f = wl.to_xyzw(pos, np.float32), wl.to_xyzw(force, np.float32)
+    dp, df = torch.from_numpy(p).cuda(), torch.from_numpy(f).cuda()
+    ctx = sd.Context(n, wl.A, wl.ETA)
+    ctx.set_dispatch(0, 0)          # tiled kernels at every N
+    out = {}
+    for mode, tag in ((sd.STAGE_BULK, "kahan"), (sd.STAGE_NAIVE, "_naive"), (sd.STAGE_SYNC, "_sync")):
+        ctx.set_staging(mode)
+        assert ctx.kernel_name.endswith(tag), ctx.kernel_name
+        dv = torch.full_like(dp, float("nan"))
+        ctx.mobility_apply(dp, df, dv)
+        torch.cuda.synchronize()
+        out[mode] = dv.cpu().numpy()
+    assert np.array_equal(out[sd.STAGE_BULK], out[sd.STAGE_NAIVE])
+    assert np.array_equal(out[sd.STAGE_BULK], out[sd.STAGE_SYNC])
+    rows = wl.row_subset(n, 512, wl.SEED_BASE + 62)
+    want = orc.apply_rows(p[:, :3].astype(np.float64), f[:, :3].astype(np.float64), rows, wl.A, wl.ETA)
+    assert rel_err(out[sd.STAGE_SYNC][rows, :3].astype(np.float64), want) <= TOL_F32
+    # the ablation variants exist for RPY / fp32-Kahan / free space only, and say so
+    for bad in (lambda: ctx.set_tensor(sd.TENSOR_OSEEN), lambda: ctx.set_precision(sd.PREC_F64),
+                lambda: ctx.set_box(100.0), lambda: ctx.set_staging(3)):
+        with pytest.raises(sd.SdError):
+            bad()
+    ctx.mobility_apply(dp, df, dv)  # still usable after the refused calls
+    torch.cuda.synchronize()
+    assert np.array_equal(dv.cpu().numpy(), out[sd.STAGE_BULK])
+    ctx.set_staging(sd.STAGE_BULK)
+    ctx.set_tensor(sd.TENSOR_OSEEN)
+    with pytest.raises(sd.SdError):
+        ctx.set_staging(sd.STAGE_NAIVE)
+    ctx.mobility_apply(dp, df, dv)
+    torch.cuda.synchronize()
+    assert np.all(np.isfinite(dv.cpu().numpy()))
+    ctx.close()
