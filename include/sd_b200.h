@@ -133,6 +133,13 @@ sd_status sd_step(sd_ctx* ctx, void* pos, sd_force_fn fn, void* user, const void
 /* Copy the velocities of the last product into vel_out[N][4] (device). */
 sd_status sd_get_velocity(sd_ctx* ctx, void* vel_out, void* stream);
 
+/* Ablation of PAPER.md:253-263 ("single or double-single precision for ... (b) positions in the
+ * Euler integration"): on = 1 (default) carries positions as (hi, lo) float pairs in the fp32
+ * modes; on = 0 keeps them in plain fp32, r <- fl32(r + h v), low words held at zero.  No effect
+ * in SD_PREC_F64.  The accumulation of the velocities, (a) in the paper, is selected by
+ * sd_set_precision (SD_PREC_F32_KAHAN / SD_PREC_F32_PLAIN). */
+sd_status sd_set_position_compensation(sd_ctx* ctx, int on);
+
 /* Forget the position low words (call after editing pos between sd_step calls). */
 sd_status sd_reset_compensation(sd_ctx* ctx, void* stream);
 

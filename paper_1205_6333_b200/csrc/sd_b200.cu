@@ -48,6 +48,7 @@ struct sd_ctx {
     long long small_apply_max = sd::kSmallApplyMax;  // N up to which the one-launch kernel runs
     int ipt_override = 0;                            // particles per thread; 0 = automatic
     int staging = 0;                                 // sd::STAGE_* (ablation, fp32 RPY Kahan only)
+    int pos_comp = 1;                                // 0: plain fp32 positions (ablation)
     int device = 0;
     int num_sms = 0;
     Config cfg;
@@ -365,7 +366,8 @@ sd_status launch_finalize(sd_ctx* c, void* vel, void* pos, double dt, cudaStream
         sd::finalize_f32_kernel<MODE><<<blocks, sd::kFinThreads, 0, st>>>(
             static_cast<const float4*>(c->part), c->d_blk_nslots, static_cast<float4*>(c->rec),
             static_cast<float4*>(vel), static_cast<float4*>(pos), static_cast<float4*>(c->pos_lo),
-            static_cast<float4*>(c->pos_half), dt, 4.0 / (3.0 * c->a), n, c->cfg.IB, c->Nrec);
+            static_cast<float4*>(c->pos_half), dt, 4.0 / (3.0 * c->a), n, c->cfg.IB, c->Nrec,
+            c->pos_comp);
     return check_launch(c, "finalize_kernel");
 }
 
@@ -401,7 +403,7 @@ sd_status launch_small_apply_t(sd_ctx* c, const void* posx, const void* force, c
     sd::small_apply_kernel<T4, TEN, KAHAN, IPW><<<blocks, sd::kSmallThreads, 0, st>>>(             \
         static_cast<const T4*>(posx), static_cast<const T4*>(force), gx, gy, gz,                   \
         static_cast<T4*>(vel), static_cast<const T4*>(pos_base), static_cast<T4*>(c->pos_lo),      \
-        static_cast<T4*>(pos_out), dt, mode, k, n)
+        static_cast<T4*>(pos_out), dt, mode, k, n, c->pos_comp)
     if (rpy) {
         if (ipw == 2) SD_SMALL_LAUNCH(0, 2); else SD_SMALL_LAUNCH(0, 1);
     } else {
@@ -438,7 +440,7 @@ sd_status launch_stepper_t(sd_ctx* c, void* pos, const void* force, const double
 #define SD_STEP_LAUNCH(TEN, SUB)                                                                   \
     sd::small_stepper_kernel<T4, TEN, KAHAN, SUB><<<1, threads, 0, st>>>(                          \
         static_cast<T4*>(pos), static_cast<T4*>(c->pos_lo), static_cast<const T4*>(force), gx, gy, \
-        gz, static_cast<T4*>(c->vel), dt, ns, integrator, k, n)
+        gz, static_cast<T4*>(c->vel), dt, ns, integrator, k, n, c->pos_comp)
         if (rpy) {
             if (sub == 32) SD_STEP_LAUNCH(0, 32); else SD_STEP_LAUNCH(0, 16);
         } else {
@@ -545,6 +547,13 @@ sd_status sd_set_dispatch(sd_ctx* ctx, long long small_apply_max, int particles_
     ctx->small_apply_max = small_apply_max < 0 ? sd::kSmallApplyMax : small_apply_max;
     ctx->ipt_override = particles_per_thread;
     return configure(ctx);
+}
+
+sd_status sd_set_position_compensation(sd_ctx* ctx, int on) {
+    if (!ctx) return fail(nullptr, SD_ERR_INVALID_ARG, "sd_set_position_compensation: ctx is NULL");
+    ctx->pos_comp = on ? 1 : 0;
+    ctx->lo_valid = false;  // low words are re-zeroed before the next step
+    return SD_OK;
 }
 
 sd_status sd_set_staging(sd_ctx* ctx, int mode) {

@@ -131,6 +131,33 @@ __device__ __forceinline__ double lanes_sum(double v) {
     return v;
 }
 
+template <int WIDTH>
+__device__ __forceinline__ float lanes_sum_f32(float v) {
+#pragma unroll
+    for (int o = WIDTH / 2; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o, WIDTH);
+    return v;
+}
+
+// Cross-lane sum of the per-lane partial sums + self term mu0 F_i.  Compensated modes and fp64
+// combine in fp64; SD_PREC_F32_PLAIN stays in fp32 throughout, so that "single-precision
+// accumulation" means what it says even when a lane holds a single term.
+template <typename S, bool KAHAN, int WIDTH>
+__device__ __forceinline__ void combine_lanes(const Acc3<S, KAHAN>& acc, const S mu0, const S fx,
+                                              const S fy, const S fz, double& vx, double& vy,
+                                              double& vz) {
+    acc.value(vx, vy, vz);
+    if (!KAHAN && sizeof(S) == 4) {
+        const float m = static_cast<float>(mu0);
+        vx = fmaf(m, static_cast<float>(fx), lanes_sum_f32<WIDTH>(static_cast<float>(vx)));
+        vy = fmaf(m, static_cast<float>(fy), lanes_sum_f32<WIDTH>(static_cast<float>(vy)));
+        vz = fmaf(m, static_cast<float>(fz), lanes_sum_f32<WIDTH>(static_cast<float>(vz)));
+    } else {
+        vx = lanes_sum<WIDTH>(vx) + static_cast<double>(mu0) * static_cast<double>(fx);
+        vy = lanes_sum<WIDTH>(vy) + static_cast<double>(mu0) * static_cast<double>(fy);
+        vz = lanes_sum<WIDTH>(vz) + static_cast<double>(mu0) * static_cast<double>(fz);
+    }
+}
+
 // ---- one product per launch -----------------------------------------------------------------
 // posx: positions the distances are taken from; force: per-particle forces or NULL (uniform g).
 // MODE (sd_stream.cuh, run-time): FIN_VEL writes vel only; otherwise pos_base (+ pos_lo) + h v
@@ -141,7 +168,7 @@ small_apply_kernel(const T4* __restrict__ posx, const T4* __restrict__ force, co
                    const double gy, const double gz, T4* __restrict__ vel,
                    const T4* __restrict__ pos_base, T4* __restrict__ pos_lo,
                    T4* __restrict__ pos_out, const double dt, const int MODE,
-                   const CoefT<typename Vec4<T4>::S> k, const int N) {
+                   const CoefT<typename Vec4<T4>::S> k, const int N, const int pos_comp) {
     typedef typename Vec4<T4>::S S;
     __shared__ T4 sp[kSmallTile];
     __shared__ T4 sf[kSmallTile];
@@ -180,27 +207,20 @@ small_apply_kernel(const T4* __restrict__ posx, const T4* __restrict__ force, co
     }
 #pragma unroll
     for (int m = 0; m < IPW; ++m) {
-        double vx, vy, vz;
-        acc[m].value(vx, vy, vz);
-        vx = lanes_sum<32>(vx);
-        vy = lanes_sum<32>(vy);
-        vz = lanes_sum<32>(vz);
         const int i = i0 + m;
+        S sfx = S(gx), sfy = S(gy), sfz = S(gz);  // F_i of the self term
+        if (force) {
+            const T4 f = force[min(i, N - 1)];
+            sfx = f.x, sfy = f.y, sfz = f.z;
+        }
+        double vx, vy, vz;
+        combine_lanes<S, KAHAN, 32>(acc[m], k.mu0, sfx, sfy, sfz, vx, vy, vz);
         if (lane == 0 && i < N) {
-            double fx = gx, fy = gy, fz = gz;
-            if (force) {
-                const T4 f = force[i];
-                fx = f.x, fy = f.y, fz = f.z;
-            }
-            const double mu0 = static_cast<double>(k.mu0);
-            vx += mu0 * static_cast<double>(S(fx));
-            vy += mu0 * static_cast<double>(S(fy));
-            vz += mu0 * static_cast<double>(S(fz));
             vel[i] = Vec4<T4>::make(S(vx), S(vy), S(vz), S(0));
             if (MODE != FIN_VEL) {
                 const T4 ph = pos_base[i];
                 double X = ph.x, Y = ph.y, Z = ph.z;
-                if (sizeof(S) == 4) {
+                if (sizeof(S) == 4 && pos_comp) {
                     const T4 pl = pos_lo[i];
                     X += pl.x, Y += pl.y, Z += pl.z;
                 }
@@ -208,10 +228,11 @@ small_apply_kernel(const T4* __restrict__ posx, const T4* __restrict__ force, co
                 X += h * vx, Y += h * vy, Z += h * vz;
                 const S xh = S(X), yh = S(Y), zh = S(Z);
                 pos_out[i] = Vec4<T4>::make(xh, yh, zh, S(0));
-                if (MODE != FIN_HALF && sizeof(S) == 4)
-                    pos_lo[i] = Vec4<T4>::make(S(X - static_cast<double>(xh)),
-                                               S(Y - static_cast<double>(yh)),
-                                               S(Z - static_cast<double>(zh)), S(0));
+                if (MODE != FIN_HALF && sizeof(S) == 4)  // pos_comp = 0: plain fp32 positions
+                    pos_lo[i] = pos_comp ? Vec4<T4>::make(S(X - static_cast<double>(xh)),
+                                                          S(Y - static_cast<double>(yh)),
+                                                          S(Z - static_cast<double>(zh)), S(0))
+                                         : Vec4<T4>::make(S(0), S(0), S(0), S(0));
             }
         }
     }
@@ -226,7 +247,7 @@ __global__ void __launch_bounds__(1024)
 small_stepper_kernel(T4* __restrict__ pos, T4* __restrict__ pos_lo, const T4* __restrict__ force,
                      const double gx, const double gy, const double gz, T4* __restrict__ vel,
                      const double dt, const long long n_steps, const int integrator,
-                     const CoefT<typename Vec4<T4>::S> k, const int N) {
+                     const CoefT<typename Vec4<T4>::S> k, const int N, const int pos_comp) {
     typedef typename Vec4<T4>::S S;
     __shared__ double P[kStepperMax][3];   // current positions r_n
     __shared__ S X[kStepperMax][3];        // positions the distances are taken from (S-rounded)
@@ -237,7 +258,7 @@ small_stepper_kernel(T4* __restrict__ pos, T4* __restrict__ pos_lo, const T4* __
     if (owner) {
         const T4 p = pos[i];
         double x = p.x, y = p.y, z = p.z;
-        if (sizeof(S) == 4) {
+        if (sizeof(S) == 4 && pos_comp) {
             const T4 l = pos_lo[i];
             x += l.x, y += l.y, z += l.z;
         }
@@ -251,7 +272,6 @@ small_stepper_kernel(T4* __restrict__ pos, T4* __restrict__ pos_lo, const T4* __
         }
     }
     __syncthreads();
-    const double mu0 = static_cast<double>(k.mu0);
     double vx = 0.0, vy = 0.0, vz = 0.0;
     const int n_products = (integrator == 1) ? 2 : 1;
     for (long long step = 0; step < n_steps; ++step) {
@@ -266,20 +286,21 @@ small_stepper_kernel(T4* __restrict__ pos, T4* __restrict__ pos_lo, const T4* __
                     acc.add(tx, ty, tz);
                 }
             }
-            acc.value(vx, vy, vz);
-            vx = lanes_sum<SUB>(vx);
-            vy = lanes_sum<SUB>(vy);
-            vz = lanes_sum<SUB>(vz);
+            {
+                const int ii = (i < N) ? i : 0;
+                combine_lanes<S, KAHAN, SUB>(acc, k.mu0, F[ii][0], F[ii][1], F[ii][2], vx, vy, vz);
+            }
             __syncthreads();  // every lane has read X
             if (owner) {
-                vx += mu0 * static_cast<double>(F[i][0]);
-                vy += mu0 * static_cast<double>(F[i][1]);
-                vz += mu0 * static_cast<double>(F[i][2]);
                 const bool half = (n_products == 2) && (stage == 0);
                 const double h = half ? 0.5 * dt : dt;
                 const double x = P[i][0] + h * vx, y = P[i][1] + h * vy, z = P[i][2] + h * vz;
                 X[i][0] = S(x), X[i][1] = S(y), X[i][2] = S(z);
-                if (!half) P[i][0] = x, P[i][1] = y, P[i][2] = z;
+                if (!half) {  // pos_comp = 0: the position is kept in S only ("single")
+                    P[i][0] = pos_comp ? x : static_cast<double>(X[i][0]);
+                    P[i][1] = pos_comp ? y : static_cast<double>(X[i][1]);
+                    P[i][2] = pos_comp ? z : static_cast<double>(X[i][2]);
+                }
             }
             __syncthreads();
         }

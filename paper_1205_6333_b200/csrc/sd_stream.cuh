@@ -69,7 +69,8 @@ __global__ void __launch_bounds__(kFinThreads)
 finalize_f32_kernel(const float4* __restrict__ part, const int* __restrict__ blk_nslots,
                     float4* __restrict__ rec, float4* __restrict__ vel, float4* __restrict__ pos,
                     float4* __restrict__ pos_lo, float4* __restrict__ pos_half, const double dt,
-                    const double mu0r, const int N, const int IB, const long long slot_stride) {
+                    const double mu0r, const int N, const int IB, const long long slot_stride,
+                    const int pos_comp) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N) return;
     const int nslots = blk_nslots[i / IB];
@@ -101,7 +102,7 @@ finalize_f32_kernel(const float4* __restrict__ part, const int* __restrict__ blk
     vel[i] = make_float4(static_cast<float>(vx), static_cast<float>(vy), static_cast<float>(vz), 0.f);
     if (MODE == FIN_VEL) return;
     const float4 ph = pos[i];
-    const float4 pl = pos_lo[i];
+    const float4 pl = pos_comp ? pos_lo[i] : make_float4(0.f, 0.f, 0.f, 0.f);  // 0: plain fp32 positions
     const double h = (MODE == FIN_HALF) ? 0.5 * dt : dt;
     const double X = (static_cast<double>(ph.x) + static_cast<double>(pl.x)) + h * vx;
     const double Y = (static_cast<double>(ph.y) + static_cast<double>(pl.y)) + h * vy;
@@ -113,9 +114,10 @@ finalize_f32_kernel(const float4* __restrict__ part, const int* __restrict__ blk
         return;
     }
     pos[i] = make_float4(xh, yh, zh, 0.f);
-    pos_lo[i] = make_float4(static_cast<float>(X - static_cast<double>(xh)),
-                            static_cast<float>(Y - static_cast<double>(yh)),
-                            static_cast<float>(Z - static_cast<double>(zh)), 0.f);
+    pos_lo[i] = pos_comp ? make_float4(static_cast<float>(X - static_cast<double>(xh)),
+                                       static_cast<float>(Y - static_cast<double>(yh)),
+                                       static_cast<float>(Z - static_cast<double>(zh)), 0.f)
+                         : make_float4(0.f, 0.f, 0.f, 0.f);
 }
 
 // fp64 mode.  part: [slot][Nrec] double4.

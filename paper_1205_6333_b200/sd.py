@@ -43,6 +43,7 @@ SYMBOLS = {
     "sd_step": (_I, [_P, _P, FORCE_FN, _P, _P, ctypes.POINTER(_D), _D, _LL, _I, _P]),
     "sd_get_velocity": (_I, [_P, _P, _P]),
     "sd_reset_compensation": (_I, [_P, _P]),
+    "sd_set_position_compensation": (_I, [_P, _I]),
     "sd_num_particles": (_LL, [_P]),
     "sd_self_mobility": (_D, [_P]),
     "sd_launch_count": (_LL, [_P]),
@@ -172,6 +173,10 @@ class Context:
 
     def get_velocity(self, vel, stream=None):
         self._check(self._lib.sd_get_velocity(self._h, self._ptr(vel, "vel"), _stream_ptr(stream)))
+
+    def set_position_compensation(self, on: bool):
+        """False: plain fp32 positions in sd_step (ablation of PAPER.md:253-263)."""
+        self._check(self._lib.sd_set_position_compensation(self._h, 1 if on else 0))
 
     def reset_compensation(self, stream=None):
         self._check(self._lib.sd_reset_compensation(self._h, _stream_ptr(stream)))

@@ -57,3 +57,19 @@ def test_reference_arm_prints_contract_line():
     assert line["cpu_baseline"]["kind"] == "oracle" and line["cpu_baseline"]["cores"] >= 1
     assert line["e2e"]["h2d_bytes_per_step"] == 0 and line["e2e"]["d2h_bytes_per_step"] == 0
     assert line["steps"] == 2 and line["warmup"] == 1
+
+
+def test_stability_postprocessing_recovers_period_and_amplitude():
+    """paper_1205_6333_b200/stability.py, host side: parabolic fits to the extrema of a sampled
+    x_1(t) give cycle duration and amplitude of a known signal."""
+    import numpy as np
+    from paper_1205_6333_b200 import stability
+    dt, stride, T, A = 0.01, 100, 517.04, 4.2617
+    t = (np.arange(60000) + 1) * dt * stride
+    traj = np.zeros((t.size, 4, 4))
+    traj[:, 0, 0] = 6.57 + A * np.cos(2 * np.pi * t / T)
+    traj[:, 0, 1] = 1e-7 * np.sin(t)
+    rows, ncyc = stability.analyse(traj, dt, stride, window=1.0e4)
+    assert ncyc == int(t[-1] // T)
+    for lo, hi, n, dur, sd_, amp, ymax in rows[:-1]:
+        assert n >= 18 and abs(dur - T) < 1e-3 and abs(amp - A) < 1e-4 and ymax <= 1e-7
