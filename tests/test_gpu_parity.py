@@ -536,3 +536,55 @@ def test_staging_modes_are_bit_identical_and_guarded(gpu, n):
     torch.cuda.synchronize()
     assert np.all(np.isfinite(dv.cpu().numpy()))
     ctx.close()
+
+
+# ---- the pieces the stability experiment runs on -----------------------------
+
+def test_four_sphere_euler_2e5_steps_fp64_matches_oracle(gpu):
+    """Euler, dt = 0.01, 2e5 steps (~3.9 cycles) in the one-launch stepper, fp64, against sdo_step."""
+    torch, sd = gpu
+    pos, force = wl.four_sphere()
+    p = wl.to_xyzw(pos, np.float64)
+    ctx = sd.Context(4, wl.A, wl.ETA)
+    ctx.set_precision(sd.PREC_F64)
+    dp = torch.from_numpy(p).cuda()
+    for _ in range(4):  # several calls: the state carried between launches is complete
+        ctx.step(dp, 0.01, 50000, sd.INT_EULER, gravity=(0.0, 0.0, -1.0))
+    torch.cuda.synchronize()
+    want, _, _ = orc.step(pos, force, wl.A, wl.ETA, 0.01, 200000, orc.INT_EULER)
+    got = dp.cpu().numpy()[:, :3]
+    assert np.abs(got - want).max() <= 1e-8
+    assert np.all(got[[0, 2], 1] == 0.0) and np.all(got[[1, 3], 0] == 0.0)  # PAPER.md:251 symmetries
+    ctx.close()
+
+
+@pytest.mark.parametrize("n", [4, 300, 5000])
+def test_plain_fp32_positions_round_every_step(gpu, n):
+    """sd_set_position_compensation(0), reading B5: r <- fl32(r + dt v), nothing carried over.  One
+    Euler step from fp32 positions must land on the fp32 number nearest to r + dt v_oracle (1 ulp
+    of slack for the fp32 velocity error), and two such steps must differ from the compensated
+    run exactly by the low words that were dropped."""
+    torch, sd = gpu
+    pos = wl.uniform_cube(n, 0.05, wl.SEED_BASE + 80 + n) if n > 4 else wl.four_sphere()[0]
+    p = wl.to_xyzw(pos, np.float32)
+    F = wl.gravity_forces(n)
+    dt = 0.37
+    ctx = sd.Context(n, wl.A, wl.ETA)
+    ctx.set_position_compensation(False)
+    dp = torch.from_numpy(p).cuda()
+    ctx.step(dp, dt, 1, sd.INT_EULER, gravity=(0.0, 0.0, -1.0))
+    torch.cuda.synchronize()
+    got1 = dp.cpu().numpy()[:, :3].copy()
+    v = orc.apply(p[:, :3].astype(np.float64), F, wl.A, wl.ETA)
+    exact = p[:, :3].astype(np.float64) + dt * v
+    ulp = np.spacing(np.abs(exact).astype(np.float32)).astype(np.float64)
+    assert np.all(np.abs(got1.astype(np.float64) - exact) <= 0.5 * ulp + 1e-5 * dt * np.abs(v) + 1e-12)
+    # second step: plain mode restarts from the rounded positions, i.e. equals a fresh context
+    ctx.step(dp, dt, 1, sd.INT_EULER, gravity=(0.0, 0.0, -1.0))
+    ctx2 = sd.Context(n, wl.A, wl.ETA)
+    dq = torch.from_numpy(np.concatenate([got1, np.zeros((n, 1), np.float32)], axis=1)).cuda()
+    ctx2.step(dq, dt, 1, sd.INT_EULER, gravity=(0.0, 0.0, -1.0))
+    torch.cuda.synchronize()
+    assert np.array_equal(dp.cpu().numpy(), dq.cpu().numpy())
+    ctx.close()
+    ctx2.close()
