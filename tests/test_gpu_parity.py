@@ -578,7 +578,8 @@ def test_plain_fp32_positions_round_every_step(gpu, n):
     v = orc.apply(p[:, :3].astype(np.float64), F, wl.A, wl.ETA)
     exact = p[:, :3].astype(np.float64) + dt * v
     ulp = np.spacing(np.abs(exact).astype(np.float32)).astype(np.float64)
-    assert np.all(np.abs(got1.astype(np.float64) - exact) <= 0.5 * ulp + 1e-5 * dt * np.abs(v) + 1e-12)
+    assert np.all(np.abs(got1.astype(np.float64) - exact) <= 0.5 * ulp
+                  + 1e-5 * dt * np.linalg.norm(v, axis=1, keepdims=True) + 1e-12)
     # second step: plain mode restarts from the rounded positions, i.e. equals a fresh context
     ctx.step(dp, dt, 1, sd.INT_EULER, gravity=(0.0, 0.0, -1.0))
     ctx2 = sd.Context(n, wl.A, wl.ETA)
