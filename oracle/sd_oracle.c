@@ -43,6 +43,9 @@
  *     of the fp32 positions); the displacement d - L n itself is then formed in double.
  *     The variants differ only for pairs within rounding of |d_alpha| = L/2.
  *
+ *   - lubrication correction (Eq. 8): see the block comment above
+ *     sdo_lubrication; pinned in tests/test_oracle_lub_pins.py.
+ *
  * Pins (tests/test_oracle_pins.py, run with -m "not gpu"): single-sphere Stokes
  * velocity, closed-form two-sphere velocities, continuity and C1-continuity at r = 2a,
  * divergence-freeness, T = (1 + a^2/3 lap) G by finite differences, symmetry,
@@ -294,6 +297,103 @@ int sdo_step(double *pos, const double *force, long long N, double a, double eta
              double *vel_last) {
     return sdo_step_box(pos, force, N, a, eta, tensor, 0.0, SDO_IMAGE_DEFINITION, dt, n_steps,
                         integrator, traj, rec_stride, vel_last);
+}
+
+/* ---- lubrication correction (Eq. 8) --------------------
+ *
+ *   mu0 f_sing(r_ij) = [ 1/(4 s) - (9/40) ln s ] rr^ - (1/6) ln s (I - rr^),   s = r_ij / a - 2
+ *   C_i = sum'_j f_sing(r_ij) . (v_i - v_j)         (the term subtracted from F_i in step 2 of
+ *                                                    the paper's loop)
+ * Readings (C1-C4): the primed sum runs over j != i with r_ij < 3a ("we truncate ad hoc
+ * at s = 1 or r = 3a"); ln is the natural logarithm; s is clamped from below at SDO_LUB_SMIN (the
+ * paper never lets spheres touch; Eq. 8 diverges at s = 0 and is undefined for s < 0); periodic
+ * box as in sdo_apply_box.  decide_f32 != 0 takes the DECISION r < 3a the way the fp32 kernels
+ * do: on r^2 = fma(dz,dz,fma(dy,dy,dx*dx)) evaluated in float on float displacements, against
+ * (float)(9 a^2); the term itself is always evaluated in double.
+ */
+#define SDO_LUB_SMIN 1.0e-3
+
+static void sdo_lub_row(const double *pos, const double *vel, long long N, double a, double mu0,
+                        double L, int image, int decide_f32, long long i, double *c) {
+    long double sx = 0.0L, sy = 0.0L, sz = 0.0L;
+    for (long long j = 0; j < N; ++j) {
+        if (j == i) continue;
+        const double dx = sdo_min_image(pos[3 * i + 0], pos[3 * j + 0], L, image);
+        const double dy = sdo_min_image(pos[3 * i + 1], pos[3 * j + 1], L, image);
+        const double dz = sdo_min_image(pos[3 * i + 2], pos[3 * j + 2], L, image);
+        const double r2 = dx * dx + dy * dy + dz * dz;
+        int inside;
+        if (decide_f32) {
+            const float fx = (float)dx, fy = (float)dy, fz = (float)dz;
+            inside = fmaf(fz, fz, fmaf(fy, fy, fx * fx)) < (float)(9.0 * a * a);
+        } else {
+            inside = r2 < 9.0 * a * a;
+        }
+        if (!inside || r2 == 0.0) continue;
+        const double r = sqrt(r2);
+        double s = r / a - 2.0;
+        if (s < SDO_LUB_SMIN) s = SDO_LUB_SMIN;
+        const double ls = log(s);
+        const double par = (1.0 / (4.0 * s) - 9.0 / 40.0 * ls) / mu0; /* along rr^      */
+        const double per = (-ls / 6.0) / mu0;                         /* along I - rr^  */
+        const double wx = vel[3 * i + 0] - vel[3 * j + 0];
+        const double wy = vel[3 * i + 1] - vel[3 * j + 1];
+        const double wz = vel[3 * i + 2] - vel[3 * j + 2];
+        const double rw = (dx * wx + dy * wy + dz * wz) / r2;         /* (r^ . w) / r   */
+        sx += (long double)(per * wx + (par - per) * rw * dx);
+        sy += (long double)(per * wy + (par - per) * rw * dy);
+        sz += (long double)(per * wz + (par - per) * rw * dz);
+    }
+    c[0] = (double)sx;
+    c[1] = (double)sy;
+    c[2] = (double)sz;
+}
+
+/* corr[i] = C_i for all i.  vel: [N][3] velocities of the previous step. */
+int sdo_lubrication(const double *pos, const double *vel, long long N, double a, double eta,
+                    double L, int image, int decide_f32, double *corr) {
+    if (!sdo_args_ok(pos, vel, N, a, eta, SDO_TENSOR_RPY) || !corr || !sdo_box_ok(L, image)) return 1;
+    const double mu0 = sdo_mu0(a, eta);
+#pragma omp parallel for schedule(dynamic, 8) if (N >= 256)
+    for (long long i = 0; i < N; ++i)
+        sdo_lub_row(pos, vel, N, a, mu0, L, image, decide_f32, i, corr + 3 * i);
+    return 0;
+}
+
+/* The paper's loop with the lubrication-corrected forces, constant external
+ * forces fext:  F = fext - C(r, v_prev);  v = M(r) F;  Euler: r <- r + dt v.  Midpoint: both
+ * stages correct the forces with the velocities of the product evaluated last.  vel: in = the
+ * velocities "of the previous step" (zeros for a cold start), out = those of the last product. */
+int sdo_step_lub(double *pos, double *vel, const double *fext, long long N, double a, double eta,
+                 int tensor, double L, int image, int decide_f32, double dt, long long n_steps,
+                 int integrator) {
+    if (!sdo_args_ok(pos, fext, N, a, eta, tensor) || !vel || !isfinite(dt) || n_steps < 0) return 1;
+    if (!sdo_box_ok(L, image)) return 1;
+    if (integrator != SDO_INT_EULER && integrator != SDO_INT_MIDPOINT) return 1;
+    const size_t n3 = 3 * (size_t)N;
+    double *f = (double *)malloc(sizeof(double) * n3);
+    double *c = (double *)malloc(sizeof(double) * n3);
+    double *ph = (double *)malloc(sizeof(double) * n3);
+    if (!f || !c || !ph) {
+        free(f); free(c); free(ph);
+        return 2;
+    }
+    for (long long s = 0; s < n_steps; ++s) {
+        sdo_lubrication(pos, vel, N, a, eta, L, image, decide_f32, c);
+        for (size_t k = 0; k < n3; ++k) f[k] = fext[k] - c[k];
+        sdo_apply_box(pos, f, N, a, eta, tensor, L, image, vel);
+        if (integrator == SDO_INT_EULER) {
+            for (size_t k = 0; k < n3; ++k) pos[k] = pos[k] + dt * vel[k];
+        } else {
+            for (size_t k = 0; k < n3; ++k) ph[k] = pos[k] + 0.5 * dt * vel[k];
+            sdo_lubrication(ph, vel, N, a, eta, L, image, decide_f32, c);
+            for (size_t k = 0; k < n3; ++k) f[k] = fext[k] - c[k];
+            sdo_apply_box(ph, f, N, a, eta, tensor, L, image, vel);
+            for (size_t k = 0; k < n3; ++k) pos[k] = pos[k] + dt * vel[k];
+        }
+    }
+    free(f); free(c); free(ph);
+    return 0;
 }
 
 int sdo_num_threads(void) {

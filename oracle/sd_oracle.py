@@ -68,6 +68,10 @@ def _load():
     lib.sdo_assemble_box.argtypes = [dp, ll, dbl, dbl, ci, dbl, ci, dp]
     lib.sdo_step_box.restype = ci
     lib.sdo_step_box.argtypes = [dp, dp, ll, dbl, dbl, ci, dbl, ci, dbl, ll, ci, dp, ll, dp]
+    lib.sdo_lubrication.restype = ci
+    lib.sdo_lubrication.argtypes = [dp, dp, ll, dbl, dbl, dbl, ci, ci, dp]
+    lib.sdo_step_lub.restype = ci
+    lib.sdo_step_lub.argtypes = [dp, dp, dp, ll, dbl, dbl, ci, dbl, ci, ci, dbl, ll, ci]
     lib.sdo_num_threads.restype = ci
     lib.sdo_set_num_threads.argtypes = [ci]
     _lib = lib
@@ -152,6 +156,32 @@ def step(pos, force, a: float, eta: float, dt: float, n_steps: int, integrator: 
                               dt, n_steps, integrator, tp, max(rec_stride, 1), _dp(vel))
     _check(rc, "sdo_step_box")
     return pos, vel, traj
+
+
+LUB_SMIN = 1.0e-3  # lower clamp of the surface separation s (reading C2)
+
+
+def lubrication(pos, vel, a: float, eta: float, box: float = 0.0, image: int = IMAGE_DEFINITION,
+                decide_f32: bool = False) -> np.ndarray:
+    """C_i = sum'_j f_sing(r_ij).(v_i - v_j), Eq. (8) truncated at r = 3a."""
+    pos, vel = _as3(pos, "pos"), _as3(vel, "vel")
+    if pos.shape != vel.shape:
+        raise ValueError("pos and vel must have the same shape")
+    out = np.empty_like(pos)
+    _check(_load().sdo_lubrication(_dp(pos), _dp(vel), pos.shape[0], a, eta, float(box), int(image),
+                                   1 if decide_f32 else 0, _dp(out)), "sdo_lubrication")
+    return out
+
+
+def step_lub(pos, vel, fext, a: float, eta: float, dt: float, n_steps: int, integrator: int,
+             tensor: int = TENSOR_RPY, box: float = 0.0, image: int = IMAGE_DEFINITION,
+             decide_f32: bool = False):
+    """The paper's loop with lubrication-corrected forces.  Returns (pos_final, vel_last)."""
+    pos, vel, fext = _as3(pos, "pos").copy(), _as3(vel, "vel").copy(), _as3(fext, "fext")
+    rc = _load().sdo_step_lub(_dp(pos), _dp(vel), _dp(fext), pos.shape[0], a, eta, tensor,
+                              float(box), int(image), 1 if decide_f32 else 0, dt, n_steps, integrator)
+    _check(rc, "sdo_step_lub")
+    return pos, vel
 
 
 def num_threads() -> int:
