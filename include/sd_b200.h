@@ -130,6 +130,30 @@ sd_status sd_step(sd_ctx* ctx, void* pos, sd_force_fn fn, void* user, const void
                   const double gravity[3], double dt, long long n_steps,
                   sd_integrator integrator, void* stream);
 
+/* Lubrication correction.  Eq. (8), rotational terms ignored as in the paper:
+ *   mu0 f_sing(r_ij) = [1/(4s) - (9/40) ln s] rr^ - (1/6) ln s (I - rr^),   s = r_ij / a - 2,
+ *   force_out[i] = F_i^ext - sum'_j f_sing(r_ij) . (v_i - v_j)            (step 2)
+ * the primed sum running over j != i with r_ij < 3a ("we truncate ad hoc at s = 1").  s is clamped
+ * from below at 1e-3 (Eq. 8 diverges at contact and is undefined for overlapping spheres; the
+ * paper never lets spheres touch); coincident centres contribute nothing.  F^ext is f_ext[N][4]
+ * or, when f_ext is NULL, the uniform force gravity[3] (NULL: zero).  pos, vel, f_ext, force_out
+ * are device arrays of the context's element type; force_out may be f_ext, not pos or vel.  The
+ * neighbour search is a hashed cell grid rebuilt on every call (context-owned, allocated on first
+ * use); results do not depend on thread scheduling.  With sd_set_box the nearest image is used
+ * and the box side must be at least 9a (SD_ERR_UNSUPPORTED otherwise).  The cut-off is decided in
+ * the context's arithmetic, the accepted pairs are evaluated in fp64. */
+sd_status sd_lubrication_apply(sd_ctx* ctx, const void* pos, const void* vel, const void* f_ext,
+                               const double gravity[3], void* force_out, void* stream);
+
+/* on != 0: sd_step runs the paper's full loop: before every product the forces
+ * (gravity / force / the callback's) are corrected by sd_lubrication_apply with the velocities of
+ * the product evaluated last (zero after sd_create; see sd_set_velocity).  Default off. */
+sd_status sd_set_lubrication(sd_ctx* ctx, int on);
+
+/* Set the "velocities of the previous step" the next lubrication correction uses: vel[N][4]
+ * (device), or NULL for zero. */
+sd_status sd_set_velocity(sd_ctx* ctx, const void* vel, void* stream);
+
 /* Copy the velocities of the last product into vel_out[N][4] (device). */
 sd_status sd_get_velocity(sd_ctx* ctx, void* vel_out, void* stream);
 

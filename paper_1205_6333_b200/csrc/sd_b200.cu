@@ -18,6 +18,7 @@
 #include "sd_common.cuh"
 #include "sd_pairs_f32.cuh"
 #include "sd_pairs_f64.cuh"
+#include "sd_lub.cuh"
 #include "sd_small.cuh"
 #include "sd_stream.cuh"
 
@@ -49,6 +50,16 @@ struct sd_ctx {
     int ipt_override = 0;                            // particles per thread; 0 = automatic
     int staging = 0;                                 // sd::STAGE_* (ablation, fp32 RPY Kahan only)
     int pos_comp = 1;                                // 0: plain fp32 positions (ablation)
+    int lubrication = 0;                             // sd_step corrects the forces by Eq. (8)
+    // lubrication cell grid (allocated on first use)
+    int4* lub_cell = nullptr;
+    unsigned* lub_count = nullptr;   // [H + 1] bucket histogram
+    unsigned* lub_start = nullptr;   // [H + 1] exclusive scan of it
+    unsigned* lub_cursor = nullptr;  // [H]
+    int* lub_order = nullptr;        // [N] particle indices grouped by bucket
+    void* lub_tmp = nullptr;         // cub scan scratch
+    size_t lub_tmp_bytes = 0;
+    unsigned lub_H = 0;
     int device = 0;
     int num_sms = 0;
     Config cfg;
@@ -118,6 +129,14 @@ void free_buffers(sd_ctx* c) {
         if (*b) cudaFree(*b);
         *b = nullptr;
     }
+    void** lub[] = {reinterpret_cast<void**>(&c->lub_cell), reinterpret_cast<void**>(&c->lub_count),
+                    reinterpret_cast<void**>(&c->lub_start), reinterpret_cast<void**>(&c->lub_cursor),
+                    reinterpret_cast<void**>(&c->lub_order), &c->lub_tmp};
+    for (void** b : lub) {
+        if (*b) cudaFree(*b);
+        *b = nullptr;
+    }
+    c->lub_H = 0;
     if (c->d_cta_u0) cudaFree(c->d_cta_u0);
     if (c->d_blk_first) cudaFree(c->d_blk_first);
     if (c->d_blk_nslots) cudaFree(c->d_blk_nslots);
@@ -462,6 +481,70 @@ sd_status launch_stepper(sd_ctx* c, void* pos, const void* force, const double g
     return launch_stepper_t<float4, true>(c, pos, force, g, dt, n_steps, integrator, st);
 }
 
+// force_out = F^ext - C(pos, vel)  (sd_lub.cuh).  fext NULL: uniform force g.
+sd_status launch_lubrication(sd_ctx* c, const void* pos, const void* vel, const void* fext,
+                             const double g[3], void* force_out, cudaStream_t st) {
+    const int n = static_cast<int>(c->N);
+    sd::LubGrid grid;
+    grid.inv_cell = 1.0 / (3.0 * c->a);
+    grid.L = c->box;
+    grid.invL = c->box > 0.0 ? 1.0 / c->box : 0.0;
+    grid.nc = 0;
+    if (c->box > 0.0) {
+        // the fp32 kernels see the box side rounded to float (as the pair kernels do)
+        if (c->precision != SD_PREC_F64) {
+            grid.L = static_cast<double>(static_cast<float>(c->box));
+            grid.invL = 1.0 / grid.L;
+        }
+        grid.nc = static_cast<int>(std::floor(grid.L / (3.0 * c->a)));
+        if (grid.nc < 3)
+            return fail(c, SD_ERR_UNSUPPORTED, "lubrication in a periodic box needs a box side of at least 9 a");
+        grid.nc = std::min(grid.nc, 1024);
+    }
+    if (!c->lub_cell) {
+        unsigned H = 1024;
+        while (H < 2u * static_cast<unsigned>(n)) H <<= 1;
+        c->lub_H = H;
+        SD_CUDA(c, cudaMalloc(&c->lub_cell, sizeof(int4) * n));
+        SD_CUDA(c, cudaMalloc(&c->lub_count, sizeof(unsigned) * (H + 1)));
+        SD_CUDA(c, cudaMalloc(&c->lub_start, sizeof(unsigned) * (H + 1)));
+        SD_CUDA(c, cudaMalloc(&c->lub_cursor, sizeof(unsigned) * H));
+        SD_CUDA(c, cudaMalloc(&c->lub_order, sizeof(int) * n));
+        SD_CUDA(c, cub::DeviceScan::ExclusiveSum(nullptr, c->lub_tmp_bytes, c->lub_count, c->lub_start,
+                                                 static_cast<int>(H + 1), st));
+        SD_CUDA(c, cudaMalloc(&c->lub_tmp, c->lub_tmp_bytes));
+    }
+    const unsigned H = c->lub_H;
+    grid.mask = H - 1;
+    SD_CUDA(c, cudaMemsetAsync(c->lub_count, 0, sizeof(unsigned) * (H + 1), st));
+    SD_CUDA(c, cudaMemsetAsync(c->lub_cursor, 0, sizeof(unsigned) * H, st));
+    const int nb = (n + 255) / 256;
+    const double gx = g ? g[0] : 0.0, gy = g ? g[1] : 0.0, gz = g ? g[2] : 0.0;
+    sd_status s;
+#define SD_LUB(T4)                                                                                  \
+    sd::lub_count_kernel<T4><<<nb, 256, 0, st>>>(static_cast<const T4*>(pos), c->lub_cell,          \
+                                                 c->lub_count, grid, n);                           \
+    if ((s = check_launch(c, "lub_count_kernel")) != SD_OK) return s;                               \
+    SD_CUDA(c, cub::DeviceScan::ExclusiveSum(c->lub_tmp, c->lub_tmp_bytes, c->lub_count,            \
+                                             c->lub_start, static_cast<int>(H + 1), st));          \
+    sd::lub_scatter_kernel<<<nb, 256, 0, st>>>(c->lub_cell, c->lub_start, c->lub_cursor,            \
+                                               c->lub_order, n);                                   \
+    if ((s = check_launch(c, "lub_scatter_kernel")) != SD_OK) return s;                             \
+    sd::lub_sort_kernel<<<(H + 255) / 256, 256, 0, st>>>(c->lub_start, c->lub_order, H);            \
+    if ((s = check_launch(c, "lub_sort_kernel")) != SD_OK) return s;                                \
+    sd::lub_force_kernel<T4><<<(n + 127) / 128, 128, 0, st>>>(                                      \
+        static_cast<const T4*>(pos), static_cast<const T4*>(vel), static_cast<const T4*>(fext), gx, \
+        gy, gz, c->lub_cell, c->lub_start, c->lub_order, static_cast<T4*>(force_out), grid, c->a,  \
+        c->mu0, n);                                                                                \
+    return check_launch(c, "lub_force_kernel")
+    if (c->precision == SD_PREC_F64) {
+        SD_LUB(double4);
+    } else {
+        SD_LUB(float4);
+    }
+#undef SD_LUB
+}
+
 bool misaligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) & (a - 1)) != 0; }
 
 }  // namespace
@@ -646,27 +729,40 @@ sd_status sd_step(sd_ctx* ctx, void* pos, sd_force_fn fn, void* user, const void
         SD_CUDA(ctx, cudaMemsetAsync(ctx->pos_lo, 0, static_cast<size_t>(ctx->Nrec) * al, st));
         ctx->lo_valid = true;
     }
-    if (!fn && ctx->N <= sd::kStepperMax)  // all steps in one launch
+    const bool lub = ctx->lubrication != 0;
+    if (!fn && !lub && ctx->N <= sd::kStepperMax)  // all steps in one launch
         return launch_stepper(ctx, pos, force, gravity, dt, n_steps, integrator, st);
+    // Forces that change from product to product (a caller callback and / or the lubrication
+    // correction with the velocities of the previous product) are rebuilt in
+    // the context's force buffer before every product.
+    const bool dynamic = fn || lub;
+    auto fill = [&](const void* p) -> sd_status {
+        const void* fe = force;
+        const double* gg = gravity;
+        if (fn) {
+            if (fn(p, ctx->force_buf, ctx->N, user, stream) != 0)
+                return fail(ctx, SD_ERR_INVALID_ARG, "sd_step: force callback failed");
+            fe = ctx->force_buf;
+        }
+        if (lub) return launch_lubrication(ctx, p, ctx->vel, fe, fe ? nullptr : gg, ctx->force_buf, st);
+        return SD_OK;
+    };
     if (ctx->N <= ctx->small_apply_max) {    // one launch per product
-        const void* fptr = fn ? ctx->force_buf : force;
-        const double* g = (fn || force) ? nullptr : gravity;
+        const void* fptr = dynamic ? ctx->force_buf : force;
+        const double* g = (dynamic || force) ? nullptr : gravity;
         void* cur = pos;
         void* other = ctx->pos_alt;
         for (long long step = 0; step < n_steps; ++step) {
             if (integrator == SD_INT_EULER) {
-                if (fn && fn(cur, ctx->force_buf, ctx->N, user, stream) != 0)
-                    return fail(ctx, SD_ERR_INVALID_ARG, "sd_step: force callback failed");
+                if (dynamic && (s = fill(cur)) != SD_OK) return s;
                 s = launch_small_apply(ctx, cur, fptr, g, ctx->vel, cur, other, dt, sd::FIN_EULER, st);
                 if (s != SD_OK) return s;
                 std::swap(cur, other);
             } else {
-                if (fn && fn(pos, ctx->force_buf, ctx->N, user, stream) != 0)
-                    return fail(ctx, SD_ERR_INVALID_ARG, "sd_step: force callback failed");
+                if (dynamic && (s = fill(pos)) != SD_OK) return s;
                 s = launch_small_apply(ctx, pos, fptr, g, ctx->vel, pos, ctx->pos_half, dt, sd::FIN_HALF, st);
                 if (s != SD_OK) return s;
-                if (fn && fn(ctx->pos_half, ctx->force_buf, ctx->N, user, stream) != 0)
-                    return fail(ctx, SD_ERR_INVALID_ARG, "sd_step: force callback failed");
+                if (dynamic && (s = fill(ctx->pos_half)) != SD_OK) return s;
                 s = launch_small_apply(ctx, ctx->pos_half, fptr, g, ctx->vel, pos, pos, dt, sd::FIN_FULL, st);
                 if (s != SD_OK) return s;
             }
@@ -676,14 +772,14 @@ sd_status sd_step(sd_ctx* ctx, void* pos, sd_force_fn fn, void* user, const void
                                          cudaMemcpyDeviceToDevice, st));
         return SD_OK;
     }
-    // constant forces are packed once; callback forces before every product
-    const int force_what = fn ? 0 : (force ? sd::PACK_FORCE : sd::PACK_GRAVITY);
+    // constant forces are packed once; dynamic forces before every product
+    const int force_what = dynamic ? 0 : (force ? sd::PACK_FORCE : sd::PACK_GRAVITY);
     s = launch_pack(ctx, pos, force, sd::PACK_POS | force_what, gravity, st);
     if (s != SD_OK) return s;
     auto callback = [&](const void* p) -> sd_status {
-        if (!fn) return SD_OK;
-        if (fn(p, ctx->force_buf, ctx->N, user, stream) != 0)
-            return fail(ctx, SD_ERR_INVALID_ARG, "sd_step: force callback failed");
+        if (!dynamic) return SD_OK;
+        sd_status r = fill(p);
+        if (r != SD_OK) return r;
         return launch_pack(ctx, nullptr, ctx->force_buf, sd::PACK_FORCE, nullptr, st);
     };
     for (long long step = 0; step < n_steps; ++step) {
@@ -699,6 +795,34 @@ sd_status sd_step(sd_ctx* ctx, void* pos, sd_force_fn fn, void* user, const void
         }
     }
     return SD_OK;
+}
+
+sd_status sd_set_lubrication(sd_ctx* ctx, int on) {
+    if (!ctx) return fail(nullptr, SD_ERR_INVALID_ARG, "sd_set_lubrication: ctx is NULL");
+    ctx->lubrication = on ? 1 : 0;
+    return SD_OK;
+}
+
+sd_status sd_set_velocity(sd_ctx* ctx, const void* vel, void* stream) {
+    if (!ctx) return fail(nullptr, SD_ERR_INVALID_ARG, "sd_set_velocity: ctx is NULL");
+    const size_t bytes = static_cast<size_t>(ctx->N) * 4 * elem_size(ctx->precision);
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (vel) SD_CUDA(ctx, cudaMemcpyAsync(ctx->vel, vel, bytes, cudaMemcpyDeviceToDevice, st));
+    else SD_CUDA(ctx, cudaMemsetAsync(ctx->vel, 0, bytes, st));
+    return SD_OK;
+}
+
+sd_status sd_lubrication_apply(sd_ctx* ctx, const void* pos, const void* vel, const void* f_ext,
+                               const double gravity[3], void* force_out, void* stream) {
+    if (!ctx) return fail(nullptr, SD_ERR_INVALID_ARG, "sd_lubrication_apply: ctx is NULL");
+    if (!pos || !vel || !force_out) return fail(ctx, SD_ERR_INVALID_ARG, "sd_lubrication_apply: NULL pointer");
+    const size_t al = 4 * elem_size(ctx->precision);
+    if (misaligned(pos, al) || misaligned(vel, al) || misaligned(force_out, al) || (f_ext && misaligned(f_ext, al)))
+        return fail(ctx, SD_ERR_INVALID_ARG, "sd_lubrication_apply: misaligned records");
+    if (force_out == pos || force_out == vel)
+        return fail(ctx, SD_ERR_INVALID_ARG, "sd_lubrication_apply: force_out aliases pos or vel");
+    return launch_lubrication(ctx, pos, vel, f_ext, f_ext ? nullptr : gravity, force_out,
+                              static_cast<cudaStream_t>(stream));
 }
 
 sd_status sd_get_velocity(sd_ctx* ctx, void* vel_out, void* stream) {

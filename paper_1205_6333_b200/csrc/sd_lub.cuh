@@ -1,0 +1,188 @@
+// sd_lub.cuh -- lubrication correction of the forces.
+//
+//   mu0 f_sing(r_ij) = [ 1/(4 s) - (9/40) ln s ] rr^ - (1/6) ln s (I - rr^) ,  s = r_ij / a - 2   Eq. (8)
+//   F_i <- F_i^ext - sum'_j f_sing(r_ij) . (v_i - v_j)         step 2 of the paper's loop
+//
+// with the velocities of the previous product and the primed sum over j != i with r_ij < 3a
+// ("we truncate ad hoc at s = 1 or r = 3a").  The paper points to Verlet lists and particle
+// reordering for this O(N) step; here it is a hashed cell grid rebuilt on
+// every call, four small launches, no host synchronisation, deterministic:
+//   lub_count_kernel    cell (3 ints, side >= 3a) and bucket (spatial hash, H = 2^k >= 2N) of
+//                       every particle; bucket histogram by atomicAdd
+//   exclusive scan      cub::DeviceScan over the H counters (library primitive, plumbing)
+//   lub_scatter_kernel  particle indices into their buckets (atomic cursor), then
+//   lub_sort_kernel     each bucket sorted by particle index: the summation order below, and
+//                       with it every bit of the result, does not depend on the atomics
+//   lub_force_kernel    one thread per particle i: 27 neighbour cells -> buckets -> candidates j
+//                       (a candidate whose cell differs is a hash collision and is skipped);
+//                       the cut-off r^2 < 9a^2 is decided in the arithmetic of the context
+//                       (fp32 fma chain in the fp32 modes, reading C3); an accepted
+//                       pair is evaluated in fp64 on the exact difference of the stored
+//                       coordinates (s = r/a - 2 loses all digits in fp32 when the gap closes);
+//                       sums in fp64; writes F^ext - C rounded to the element type.
+// Memory-bound: ~60 B per particle read + 27 bucket probes; the pair terms are a few per
+// particle.  Periodic box: cells = floor(L / 3a) per edge (>= 3 required), neighbour cells wrap,
+// displacements take the nearest image by the rule of the pair kernels.
+#pragma once
+#include <cub/device/device_scan.cuh>
+
+#include "sd_common.cuh"
+#include "sd_stream.cuh"
+
+namespace sd {
+
+constexpr double kLubSmin = 1.0e-3;  // lower clamp of s (reading C2: Eq. 8 diverges at contact)
+
+struct LubGrid {
+    double inv_cell;  // 1 / cell side
+    double L, invL;   // periodic cube (0: free space)
+    int nc;           // cells per edge in the box (0: free space, unbounded integer cells)
+    unsigned mask;    // H - 1
+};
+
+__device__ __forceinline__ unsigned lub_hash(int cx, int cy, int cz, unsigned mask) {
+    return ((static_cast<unsigned>(cx) * 73856093u) ^ (static_cast<unsigned>(cy) * 19349663u) ^
+            (static_cast<unsigned>(cz) * 83492791u)) & mask;
+}
+
+__device__ __forceinline__ int lub_cell_coord(double x, const LubGrid& g) {
+    if (g.nc > 0) {
+        double u = x * g.invL;
+        u -= floor(u);  // [0, 1)
+        const int c = static_cast<int>(u * g.nc);
+        return c < g.nc ? c : g.nc - 1;
+    }
+    return static_cast<int>(floor(x * g.inv_cell));
+}
+
+template <typename T4>
+__global__ void __launch_bounds__(256)
+lub_count_kernel(const T4* __restrict__ pos, int4* __restrict__ cell, unsigned* __restrict__ count,
+                 const LubGrid g, const int N) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const T4 p = pos[i];
+    const int cx = lub_cell_coord(p.x, g), cy = lub_cell_coord(p.y, g), cz = lub_cell_coord(p.z, g);
+    const unsigned h = lub_hash(cx, cy, cz, g.mask);
+    cell[i] = make_int4(cx, cy, cz, static_cast<int>(h));
+    atomicAdd(&count[h], 1u);
+}
+
+__global__ void __launch_bounds__(256)
+lub_scatter_kernel(const int4* __restrict__ cell, const unsigned* __restrict__ start,
+                   unsigned* __restrict__ cursor, int* __restrict__ order, const int N) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const unsigned h = static_cast<unsigned>(cell[i].w);
+    order[start[h] + atomicAdd(&cursor[h], 1u)] = i;
+}
+
+// one thread per bucket: insertion sort by particle index (buckets hold a handful of particles)
+__global__ void __launch_bounds__(256)
+lub_sort_kernel(const unsigned* __restrict__ start, int* __restrict__ order, const unsigned H) {
+    const unsigned h = blockIdx.x * blockDim.x + threadIdx.x;
+    if (h >= H) return;
+    const unsigned b = start[h], e = start[h + 1];
+    for (unsigned k = b + 1; k < e; ++k) {
+        const int v = order[k];
+        unsigned m = k;
+        while (m > b && order[m - 1] > v) {
+            order[m] = order[m - 1];
+            --m;
+        }
+        order[m] = v;
+    }
+}
+
+// nearest-image displacement of one component as a double, by the rule of the pair kernels
+// (reading B2): fp32 modes decide n on the fp32 difference, fp64 on the double one.
+template <typename S>
+__device__ __forceinline__ double lub_disp(const S xi, const S xj, const LubGrid& g);
+template <>
+__device__ __forceinline__ double lub_disp<float>(const float xi, const float xj, const LubGrid& g) {
+    if (g.nc == 0) return static_cast<double>(xi) - static_cast<double>(xj);
+    const float d = __fsub_rn(xi, xj);
+    const float Lf = static_cast<float>(g.L);
+    const float n = __fsub_rn(__fmaf_rn(d, __fdiv_rn(1.0f, Lf), 12582912.0f), 12582912.0f);
+    return static_cast<double>(d) - static_cast<double>(n) * static_cast<double>(Lf);
+}
+template <>
+__device__ __forceinline__ double lub_disp<double>(const double xi, const double xj, const LubGrid& g) {
+    const double d = xi - xj;
+    if (g.nc == 0) return d;
+    const double n = __dsub_rn(fma(d, g.invL, 6755399441055744.0), 6755399441055744.0);
+    return __dsub_rn(d, __dmul_rn(n, g.L));
+}
+
+// r^2 < 9 a^2 decided in the arithmetic of the context (reading C3)
+__device__ __forceinline__ bool lub_inside(float, double dx, double dy, double dz, double nine_a2) {
+    const float fx = static_cast<float>(dx), fy = static_cast<float>(dy), fz = static_cast<float>(dz);
+    return __fmaf_rn(fz, fz, __fmaf_rn(fy, fy, __fmul_rn(fx, fx))) < static_cast<float>(nine_a2);
+}
+__device__ __forceinline__ bool lub_inside(double, double dx, double dy, double dz, double nine_a2) {
+    return __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz)) < nine_a2;
+}
+
+// force_out = F^ext - C.  fext: per-particle external forces or NULL (uniform g); fext may be
+// force_out itself (each thread reads its own element before it writes it).
+template <typename T4>
+__global__ void __launch_bounds__(128)
+lub_force_kernel(const T4* __restrict__ pos, const T4* __restrict__ vel, const T4* fext,
+                 const double gx, const double gy, const double gz, const int4* __restrict__ cell,
+                 const unsigned* __restrict__ start, const int* __restrict__ order,
+                 T4* force_out, const LubGrid g, const double a, const double mu0,
+                 const int N) {
+    typedef typename Vec4<T4>::S S;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const T4 pi = pos[i];
+    const T4 vi = vel[i];
+    const int4 ci = cell[i];
+    const double nine_a2 = 9.0 * a * a, inv_a = 1.0 / a, inv_mu0 = 1.0 / mu0;
+    double cx = 0.0, cy = 0.0, cz = 0.0;
+    for (int oz = -1; oz <= 1; ++oz)
+        for (int oy = -1; oy <= 1; ++oy)
+            for (int ox = -1; ox <= 1; ++ox) {
+                int nx = ci.x + ox, ny = ci.y + oy, nz = ci.z + oz;
+                if (g.nc > 0) {
+                    nx = (nx + g.nc) % g.nc;
+                    ny = (ny + g.nc) % g.nc;
+                    nz = (nz + g.nc) % g.nc;
+                }
+                const unsigned h = lub_hash(nx, ny, nz, g.mask);
+                const unsigned e = start[h + 1];
+                for (unsigned k = start[h]; k < e; ++k) {
+                    const int j = order[k];
+                    const int4 cj = cell[j];
+                    if (j == i || cj.x != nx || cj.y != ny || cj.z != nz) continue;  // self / collision
+                    const T4 pj = pos[j];
+                    const double dx = lub_disp<S>(pi.x, pj.x, g), dy = lub_disp<S>(pi.y, pj.y, g),
+                                 dz = lub_disp<S>(pi.z, pj.z, g);
+                    if (!lub_inside(S(0), dx, dy, dz, nine_a2)) continue;
+                    const double r2 = dx * dx + dy * dy + dz * dz;
+                    if (r2 == 0.0) continue;  // coincident centres: no direction, no term
+                    const double r = sqrt(r2);
+                    double s = r * inv_a - 2.0;
+                    s = s < kLubSmin ? kLubSmin : s;
+                    const double ls = log(s);
+                    const double par = (0.25 / s - 0.225 * ls) * inv_mu0;
+                    const double per = (-ls * (1.0 / 6.0)) * inv_mu0;
+                    const T4 vj = vel[j];
+                    const double wx = static_cast<double>(vi.x) - static_cast<double>(vj.x);
+                    const double wy = static_cast<double>(vi.y) - static_cast<double>(vj.y);
+                    const double wz = static_cast<double>(vi.z) - static_cast<double>(vj.z);
+                    const double rw = (dx * wx + dy * wy + dz * wz) / r2;
+                    cx += per * wx + (par - per) * rw * dx;
+                    cy += per * wy + (par - per) * rw * dy;
+                    cz += per * wz + (par - per) * rw * dz;
+                }
+            }
+    double fx = gx, fy = gy, fz = gz;
+    if (fext) {
+        const T4 f = fext[i];
+        fx = f.x, fy = f.y, fz = f.z;
+    }
+    force_out[i] = Vec4<T4>::make(S(fx - cx), S(fy - cy), S(fz - cz), S(0));
+}
+
+}  // namespace sd

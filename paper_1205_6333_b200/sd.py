@@ -42,6 +42,9 @@ SYMBOLS = {
     "sd_mobility_apply_host": (_I, [_P, _P, _P, _P, _P]),
     "sd_step": (_I, [_P, _P, FORCE_FN, _P, _P, ctypes.POINTER(_D), _D, _LL, _I, _P]),
     "sd_get_velocity": (_I, [_P, _P, _P]),
+    "sd_lubrication_apply": (_I, [_P, _P, _P, _P, ctypes.POINTER(_D), _P, _P]),
+    "sd_set_lubrication": (_I, [_P, _I]),
+    "sd_set_velocity": (_I, [_P, _P, _P]),
     "sd_reset_compensation": (_I, [_P, _P]),
     "sd_set_position_compensation": (_I, [_P, _I]),
     "sd_num_particles": (_LL, [_P]),
@@ -170,6 +173,21 @@ class Context:
                                       ctypes.c_void_p(user or 0),
                                       self._ptr(force, "force", allow_none=True), g, float(dt),
                                       int(n_steps), int(integrator), _stream_ptr(stream)))
+
+    def lubrication_apply(self, pos, vel, force_out, f_ext=None, gravity=None, stream=None):
+        """force_out = F_ext - sum' f_sing.(v_i - v_j), Eq. (8) truncated at 3a."""
+        g = (ctypes.c_double * 3)(*[float(x) for x in gravity]) if gravity is not None else None
+        self._check(self._lib.sd_lubrication_apply(
+            self._h, self._ptr(pos, "pos"), self._ptr(vel, "vel"),
+            self._ptr(f_ext, "f_ext", allow_none=True), g, self._ptr(force_out, "force_out"),
+            _stream_ptr(stream)))
+
+    def set_lubrication(self, on: bool):
+        self._check(self._lib.sd_set_lubrication(self._h, 1 if on else 0))
+
+    def set_velocity(self, vel=None, stream=None):
+        self._check(self._lib.sd_set_velocity(self._h, self._ptr(vel, "vel", allow_none=True),
+                                              _stream_ptr(stream)))
 
     def get_velocity(self, vel, stream=None):
         self._check(self._lib.sd_get_velocity(self._h, self._ptr(vel, "vel"), _stream_ptr(stream)))

@@ -1,0 +1,144 @@
+"""GPU parity of the lubrication correction (Eq. 8) and of the
+paper's full loop (forces corrected with the previous velocities) against the
+CPU oracle, through the C ABI (`sd_lubrication_apply`, `sd_set_lubrication` + `sd_step`).
+
+The cut-off r < 3a is a decision taken by floating point: both sides take it in the kernel's
+arithmetic (reading C3; oracle `decide_f32`).  Accepted pairs are evaluated in fp64 on
+both sides, so the only fp32 error is the rounding of the stored inputs and of the output.
+"""
+import numpy as np
+import pytest
+
+from oracle import sd_oracle as orc
+from paper_1205_6333_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+IMAGE = {"PREC_F32_KAHAN": orc.IMAGE_F32, "PREC_F64": orc.IMAGE_F64}
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    import torch
+    from paper_1205_6333_b200 import sd
+    assert torch.cuda.is_available()
+    torch.cuda.set_device(0)
+    sd.load_library()
+    return torch, sd
+
+
+def _dt(prec_name):
+    return np.float64 if prec_name == "PREC_F64" else np.float32
+
+
+def _row_err(got, want):
+    scale = np.maximum(np.linalg.norm(want, axis=1), 1.0)
+    return float(np.max(np.linalg.norm(got - want, axis=1) / scale))
+
+
+@pytest.mark.parametrize("prec_name,tol", [("PREC_F32_KAHAN", 2e-7), ("PREC_F64", 1e-12)])
+@pytest.mark.parametrize("boxed", [False, True])
+@pytest.mark.parametrize("n,phi", [(50, 0.1), (3000, 0.05), (40000, 0.05)])
+def test_lubrication_apply_all_rows(gpu, prec_name, tol, boxed, n, phi):
+    """Uniform clouds with overlaps allowed: pairs inside 3a (about 27 phi per sphere), in contact,
+    overlapping (s clamped) and, when boxed, through the faces; per-particle external forces."""
+    torch, sd = gpu
+    dt = _dt(prec_name)
+    L = wl.cube_side(n, phi)
+    pos = wl.uniform_cube(n, phi, wl.SEED_BASE + 300 + n)
+    if boxed:  # a third of the particles live in neighbouring periodic copies
+        sh = np.random.Generator(np.random.PCG64(wl.SEED_BASE + 301)).integers(-1, 2, size=(n, 3))
+        pos = pos + L * sh * (np.arange(n) % 3 == 0)[:, None]
+    vel = wl.normal_forces(n, wl.SEED_BASE + 302 + n)
+    fext = wl.normal_forces(n, wl.SEED_BASE + 303 + n)
+    p, v, f = wl.to_xyzw(pos, dt), wl.to_xyzw(vel, dt), wl.to_xyzw(fext, dt)
+    ctx = sd.Context(n, wl.A, wl.ETA)
+    ctx.set_precision(getattr(sd, prec_name))
+    if boxed:
+        ctx.set_box(L)
+    dp, dv, df = (torch.from_numpy(x).cuda() for x in (p, v, f))
+    out = torch.full_like(dp, float("nan"))
+    ctx.lubrication_apply(dp, dv, out, f_ext=df)
+    out2 = torch.full_like(dp, float("nan"))
+    ctx.lubrication_apply(dp, dv, out2, f_ext=df)
+    torch.cuda.synchronize()
+    got = out.cpu().numpy()
+    assert np.array_equal(got, out2.cpu().numpy())            # deterministic despite the atomics
+    assert np.all(got[:, 3] == 0.0)
+    Ls = (float(np.float32(L)) if dt == np.float32 else L) if boxed else 0.0
+    corr = orc.lubrication(p[:, :3].astype(np.float64), v[:, :3].astype(np.float64), wl.A, wl.ETA,
+                           box=Ls, image=IMAGE[prec_name], decide_f32=(dt == np.float32))
+    want = f[:, :3].astype(np.float64) - corr
+    assert np.count_nonzero(np.abs(corr).sum(axis=1)) > 0.5 * n * min(1.0, 27 * phi * 0.5)
+    assert _row_err(got[:, :3].astype(np.float64), want) <= tol
+    # in place (force_out = f_ext) and with a uniform force instead of an array
+    ctx.lubrication_apply(dp, dv, df, f_ext=df)
+    out3 = torch.empty_like(dp)
+    ctx.lubrication_apply(dp, dv, out3, gravity=(0.0, 0.0, -1.0))
+    torch.cuda.synchronize()
+    assert np.array_equal(df.cpu().numpy(), got)
+    wantg = np.array([0.0, 0.0, -1.0]) - corr
+    assert _row_err(out3.cpu().numpy()[:, :3].astype(np.float64), wantg) <= tol
+    ctx.close()
+
+
+def test_lubrication_needs_a_box_of_nine_radii(gpu):
+    torch, sd = gpu
+    ctx = sd.Context(8, wl.A, wl.ETA)
+    ctx.set_box(8.5)
+    z = torch.zeros((8, 4), device="cuda")
+    with pytest.raises(sd.SdError) as e:
+        ctx.lubrication_apply(z, z.clone(), z.clone())
+    assert e.value.status == sd.ERR_UNSUPPORTED
+    ctx.set_box(9.5)
+    ctx.lubrication_apply(z, z.clone(), z.clone())
+    torch.cuda.synchronize()
+    ctx.close()
+
+
+@pytest.mark.parametrize("prec_name,ptol,vtol", [("PREC_F32_KAHAN", 2e-5, 1e-4), ("PREC_F64", 1e-10, 1e-9)])
+@pytest.mark.parametrize("n,integ,steps", [(2, "euler", 60), (300, "midpoint", 6), (300, "euler", 7),
+                                           (3000, "euler", 5), (3000, "midpoint", 3)])
+def test_step_with_lubrication_matches_the_papers_loop(gpu, prec_name, ptol, vtol, n, integ, steps):
+    """sd_set_lubrication + sd_step against sdo_step_lub: N = 2 and 300 through the one-launch-per-
+    product kernel, 3000 through the tiled kernels; random sequential addition with centre distances
+    >= 2.6 a (every gap s >= 0.6: the paper's lagged-velocity scheme v_n = mu (F - zeta v_{n-1})
+    diverges once |mu zeta| > 1, i.e. for gaps well below half a radius, on either side of the
+    comparison), ~2 neighbours inside 3a per sphere, gravity + random forces; cold start."""
+    torch, sd = gpu
+    dt_np = _dt(prec_name)
+    if n == 2:
+        pos = np.array([[0.0, 0.0, 1.3], [0.0, 0.0, -1.3]])
+        fext = np.array([[0.0, 0.0, -1.0], [0.0, 0.0, 1.0]])     # pushed together, gap 0.6 a
+    else:
+        pos = wl.rsa_cube(n, 0.25, wl.SEED_BASE + 310 + n, a=1.3)
+        fext = wl.gravity_forces(n) + 0.5 * wl.normal_forces(n, wl.SEED_BASE + 311 + n)
+    p, f = wl.to_xyzw(pos, dt_np), wl.to_xyzw(fext, dt_np)
+    dt = 0.01
+    ctx = sd.Context(n, wl.A, wl.ETA)
+    ctx.set_precision(getattr(sd, prec_name))
+    ctx.set_lubrication(True)
+    dp, df = torch.from_numpy(p).cuda(), torch.from_numpy(f).cuda()
+    gi = sd.INT_EULER if integ == "euler" else sd.INT_MIDPOINT
+    oi = orc.INT_EULER if integ == "euler" else orc.INT_MIDPOINT
+    ctx.step(dp, dt, steps, gi, force=df)
+    dv = torch.empty_like(dp)
+    ctx.get_velocity(dv)
+    torch.cuda.synchronize()
+    p64, f64 = p[:, :3].astype(np.float64), f[:, :3].astype(np.float64)
+    want_p, want_v = orc.step_lub(p64, np.zeros_like(p64), f64, wl.A, wl.ETA, dt, steps, oi,
+                                  decide_f32=(dt_np == np.float32))
+    got_p = dp.cpu().numpy()[:, :3].astype(np.float64)
+    got_v = dv.cpu().numpy()[:, :3].astype(np.float64)
+    assert np.abs(got_p - want_p).max() <= ptol
+    assert _row_err(got_v, want_v) <= vtol
+    # the correction is not a no-op on this input
+    free_p, _, _ = orc.step(p64, f64, wl.A, wl.ETA, dt, steps, oi)
+    assert np.abs(free_p - want_p).max() > 20 * ptol
+    # continuing from the carried velocities == one longer run (state between calls is complete)
+    ctx.step(dp, dt, 2, gi, force=df)
+    torch.cuda.synchronize()
+    want_p2, _ = orc.step_lub(p64, np.zeros_like(p64), f64, wl.A, wl.ETA, dt, steps + 2, oi,
+                              decide_f32=(dt_np == np.float32))
+    assert np.abs(dp.cpu().numpy()[:, :3].astype(np.float64) - want_p2).max() <= 2 * ptol
+    ctx.close()
