@@ -50,6 +50,9 @@ def parse_args():
                          "Euler steps of 0.001 tau_s per timed step; reports simulation steps/s")
     ap.add_argument("--staging", choices=["bulk", "naive", "sync"], default="bulk",
                     help="memory-access ablation (PAPER.md Appendix A): how j records reach the threads")
+    ap.add_argument("--lub", action="store_true",
+                    help="instead of the product: the lubrication correction of the forces (Eq. 8, "
+                         "PAPER.md:80-104) on N uniform points at phi = 0.05; reports particles/s")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
 
@@ -237,6 +240,119 @@ def run_fcc_steps(args, rank):
     print(json.dumps(line), flush=True)
 
 
+def run_lub(args, rank):
+    """Lubrication correction (sd_lubrication_apply): an O(N) neighbour-list step, memory bound.
+    value = particles/s; roofline against the measured HBM copy bandwidth with 64 B (fp32) / 128 B
+    (fp64) algorithmic bytes per particle (pos, vel, F_ext in, force out, each once)."""
+    if rank != 0:
+        return
+    from paper_1205_6333_b200 import workloads as wl
+    n, phi = args.n, 0.05
+    f64mode = args.precision == "f64"
+    npdt = np.float64 if f64mode else np.float32
+    pos = wl.uniform_cube(n, phi, wl.SEED_BASE + 300 + n)
+    vel = wl.normal_forces(n, wl.SEED_BASE + 302 + n)
+    fext = wl.normal_forces(n, wl.SEED_BASE + 303 + n)
+    name = (f"sd_lubrication_apply N={n} uniform cube phi={phi} (overlaps allowed, ~1.35 neighbours "
+            f"inside 3a per sphere), N(0,1) velocities and forces, {'fp64' if f64mode else 'fp32'}"
+            + (", periodic box" if args.box else ""))
+    base = {"metric": "particles/s (lubrication correction of the forces, Eq. 8)", "unit": "particles/s",
+            "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "data": "synthetic"}
+    box = wl.cube_side(n, phi) if args.box else 0.0
+    if args.impl == "reference":
+        from oracle import sd_oracle as orc
+        m = min(n, 30000)  # the oracle is O(N^2): a bounded sub-cloud of the same density
+        p64 = wl.to_xyzw(wl.uniform_cube(m, phi, wl.SEED_BASE + 300 + n), npdt)[:, :3].astype(np.float64)
+        v64 = vel[:m]
+        for _ in range(args.warmup):
+            orc.lubrication(p64, v64, wl.A, wl.ETA, box=wl.cube_side(m, phi) if args.box else 0.0)
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            orc.lubrication(p64, v64, wl.A, wl.ETA, box=wl.cube_side(m, phi) if args.box else 0.0)
+        t = time.perf_counter() - t0
+        value = args.steps * m / t
+        desc = f"all-pairs oracle on a {m}-particle cloud of the same density per step"
+        print(json.dumps(dict(base, impl="reference", value=value, ms_per_step=1e3 * t / args.steps,
+                              dtype="f64", config={"workload": name, "step": desc},
+                              cpu_baseline={"value": value, "unit": "particles/s",
+                                            "cores": orc.num_threads(), "kind": "oracle", "sample": desc},
+                              e2e={"value": value, "unit": "particles/s", "h2d_bytes_per_step": 0,
+                                   "d2h_bytes_per_step": 0}, gpu_launches=0)), flush=True)
+        return
+    import torch
+    from paper_1205_6333_b200 import benchutil, sd
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product has no CPU fallback")
+    torch.cuda.set_device(0)
+    sd.load_library()
+    hp, hv, hf = (torch.from_numpy(wl.to_xyzw(x, npdt)).pin_memory() for x in (pos, vel, fext))
+    hout = torch.empty_like(hp).pin_memory()
+    dp, dv, df = hp.cuda(), hv.cuda(), hf.cuda()
+    dout = torch.empty_like(dp)
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")
+    ctx = sd.Context(n, wl.A, wl.ETA)
+    ctx.set_precision(sd.PREC_F64 if f64mode else sd.PREC_F32_KAHAN)
+    ctx.set_box(box)
+    for _ in range(args.warmup):
+        ctx.lubrication_apply(dp, dv, dout, f_ext=df)
+    torch.cuda.synchronize()
+    launches0 = ctx.launch_count
+    sampler = benchutil.ClockSampler(0)
+    sampler.start()
+    evs = []
+    for _ in range(args.steps):
+        flush.zero_()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        ctx.lubrication_apply(dp, dv, dout, f_ext=df)
+        e1.record()
+        evs.append((e0, e1))
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    secs = sum(a.elapsed_time(b) for a, b in evs) * 1e-3
+    gpu_launches = ctx.launch_count - launches0
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        dp.copy_(hp, non_blocking=True)
+        dv.copy_(hv, non_blocking=True)
+        df.copy_(hf, non_blocking=True)
+        ctx.lubrication_apply(dp, dv, dout, f_ext=df)
+        hout.copy_(dout, non_blocking=True)
+        torch.cuda.synchronize()
+    e2e = time.perf_counter() - t0
+    rec = n * 4 * (8 if f64mode else 4)
+    peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    hbm, src = 6550.0, "fallback 6550 GB/s (B200_PROFILING.md)"
+    if os.path.exists(peaks_path):
+        with open(peaks_path) as f:
+            hbm = float(json.load(f).get("hbm_gbs", hbm))
+            src = "MEASURED_PEAKS.json hbm_gbs (burst copy)"
+    achieved = 4.0 * rec * args.steps / secs / 1e9
+    line = dict(base, value=args.steps * n / secs, ms_per_step=1e3 * secs / args.steps,
+                dtype="f64" if f64mode else "f32",
+                config={"workload": name, "kernel": "lub_count + cub scan + lub_scatter + lub_sort + lub_force",
+                        "parallelism": "1 GPU", "l2": "L2 flushed with a 256 MiB write between timed iterations"},
+                clocks=clocks, gpu_launches=gpu_launches,
+                e2e={"value": args.steps * n / e2e, "unit": "particles/s", "h2d_bytes_per_step": 3 * rec,
+                     "d2h_bytes_per_step": rec},
+                roofline={"bound": "hbm", "kernel": "whole lubrication step (5 launches)", "achieved": achieved,
+                          "peak": hbm, "unit": "GB/s", "frac": achieved / hbm, "traffic": None,
+                          "peak_source": src, "bytes_per_particle": 4 * rec // n})
+    if not args.no_cpu_baseline:
+        from oracle import sd_oracle as orc
+        m = min(n, 30000)
+        p64 = wl.to_xyzw(wl.uniform_cube(m, phi, wl.SEED_BASE + 300 + n), npdt)[:, :3].astype(np.float64)
+        t0 = time.perf_counter()
+        orc.lubrication(p64, vel[:m], wl.A, wl.ETA)
+        t = time.perf_counter() - t0
+        line["cpu_baseline"] = {"value": m / t, "unit": "particles/s", "cores": orc.num_threads(),
+                                "kind": "oracle", "sample": f"all-pairs oracle on a {m}-particle cloud of "
+                                                            f"the same density, {t:.1f} s"}
+    ctx.close()
+    print(json.dumps(line), flush=True)
+
+
 def main():
     args = parse_args()
     rank = int(os.environ.get("RANK", "0"))
@@ -244,6 +360,9 @@ def main():
     world = int(os.environ.get("WORLD_SIZE", "1"))
     if args.fcc_cells > 0:
         run_fcc_steps(args, rank)
+        return
+    if args.lub:
+        run_lub(args, rank)
         return
     if args.impl == "reference":
         run_reference(args, rank)

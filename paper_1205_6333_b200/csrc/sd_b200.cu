@@ -57,6 +57,9 @@ struct sd_ctx {
     unsigned* lub_start = nullptr;   // [H + 1] exclusive scan of it
     unsigned* lub_cursor = nullptr;  // [H]
     int* lub_order = nullptr;        // [N] particle indices grouped by bucket
+    void* lub_spos = nullptr;        // [N] positions, velocities, cells in bucket order
+    void* lub_svel = nullptr;
+    int4* lub_scell = nullptr;
     void* lub_tmp = nullptr;         // cub scan scratch
     size_t lub_tmp_bytes = 0;
     unsigned lub_H = 0;
@@ -131,7 +134,8 @@ void free_buffers(sd_ctx* c) {
     }
     void** lub[] = {reinterpret_cast<void**>(&c->lub_cell), reinterpret_cast<void**>(&c->lub_count),
                     reinterpret_cast<void**>(&c->lub_start), reinterpret_cast<void**>(&c->lub_cursor),
-                    reinterpret_cast<void**>(&c->lub_order), &c->lub_tmp};
+                    reinterpret_cast<void**>(&c->lub_order), &c->lub_tmp, &c->lub_spos, &c->lub_svel,
+                    reinterpret_cast<void**>(&c->lub_scell)};
     for (void** b : lub) {
         if (*b) cudaFree(*b);
         *b = nullptr;
@@ -502,9 +506,12 @@ sd_status launch_lubrication(sd_ctx* c, const void* pos, const void* vel, const 
         grid.nc = std::min(grid.nc, 1024);
     }
     if (!c->lub_cell) {
-        unsigned H = 1024;
-        while (H < 2u * static_cast<unsigned>(n)) H <<= 1;
+        unsigned H = 512;  // 2^(3 bits) buckets, at least one per particle
+        while (H < static_cast<unsigned>(n)) H <<= 3;
         c->lub_H = H;
+        SD_CUDA(c, cudaMalloc(&c->lub_spos, 4 * elem_size(c->precision) * n));
+        SD_CUDA(c, cudaMalloc(&c->lub_svel, 4 * elem_size(c->precision) * n));
+        SD_CUDA(c, cudaMalloc(&c->lub_scell, sizeof(int4) * n));
         SD_CUDA(c, cudaMalloc(&c->lub_cell, sizeof(int4) * n));
         SD_CUDA(c, cudaMalloc(&c->lub_count, sizeof(unsigned) * (H + 1)));
         SD_CUDA(c, cudaMalloc(&c->lub_start, sizeof(unsigned) * (H + 1)));
@@ -515,7 +522,9 @@ sd_status launch_lubrication(sd_ctx* c, const void* pos, const void* vel, const 
         SD_CUDA(c, cudaMalloc(&c->lub_tmp, c->lub_tmp_bytes));
     }
     const unsigned H = c->lub_H;
-    grid.mask = H - 1;
+    unsigned bits = 0;
+    while ((1u << (3 * (bits + 1))) <= H) ++bits;
+    grid.mask = (1u << bits) - 1u;
     SD_CUDA(c, cudaMemsetAsync(c->lub_count, 0, sizeof(unsigned) * (H + 1), st));
     SD_CUDA(c, cudaMemsetAsync(c->lub_cursor, 0, sizeof(unsigned) * H, st));
     const int nb = (n + 255) / 256;
@@ -532,10 +541,14 @@ sd_status launch_lubrication(sd_ctx* c, const void* pos, const void* vel, const 
     if ((s = check_launch(c, "lub_scatter_kernel")) != SD_OK) return s;                             \
     sd::lub_sort_kernel<<<(H + 255) / 256, 256, 0, st>>>(c->lub_start, c->lub_order, H);            \
     if ((s = check_launch(c, "lub_sort_kernel")) != SD_OK) return s;                                \
+    sd::lub_gather_kernel<T4><<<nb, 256, 0, st>>>(                                                  \
+        static_cast<const T4*>(pos), static_cast<const T4*>(vel), c->lub_cell, c->lub_order,        \
+        static_cast<T4*>(c->lub_spos), static_cast<T4*>(c->lub_svel), c->lub_scell, n);             \
+    if ((s = check_launch(c, "lub_gather_kernel")) != SD_OK) return s;                              \
     sd::lub_force_kernel<T4><<<(n + 127) / 128, 128, 0, st>>>(                                      \
-        static_cast<const T4*>(pos), static_cast<const T4*>(vel), static_cast<const T4*>(fext), gx, \
-        gy, gz, c->lub_cell, c->lub_start, c->lub_order, static_cast<T4*>(force_out), grid, c->a,  \
-        c->mu0, n);                                                                                \
+        static_cast<const T4*>(c->lub_spos), static_cast<const T4*>(c->lub_svel),                   \
+        static_cast<const T4*>(fext), gx, gy, gz, c->lub_scell, c->lub_start,                       \
+        static_cast<T4*>(force_out), grid, c->a, c->mu0, n);                                       \
     return check_launch(c, "lub_force_kernel")
     if (c->precision == SD_PREC_F64) {
         SD_LUB(double4);

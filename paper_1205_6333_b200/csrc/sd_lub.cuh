@@ -13,7 +13,7 @@
 //   lub_scatter_kernel  particle indices into their buckets (atomic cursor), then
 //   lub_sort_kernel     each bucket sorted by particle index: the summation order below, and
 //                       with it every bit of the result, does not depend on the atomics
-//   lub_force_kernel    one thread per particle i: 27 neighbour cells -> buckets -> candidates j
+//   lub_force_kernel    one thread per particle i, taken in bucket order: 27 neighbour cells -> buckets -> candidates j
 //                       (a candidate whose cell differs is a hash collision and is skipped);
 //                       the cut-off r^2 < 9a^2 is decided in the arithmetic of the context
 //                       (fp32 fma chain in the fp32 modes, reading C3); an accepted
@@ -37,12 +37,23 @@ struct LubGrid {
     double inv_cell;  // 1 / cell side
     double L, invL;   // periodic cube (0: free space)
     int nc;           // cells per edge in the box (0: free space, unbounded integer cells)
-    unsigned mask;    // H - 1
+    unsigned mask;    // 2^bits - 1: low bits of a cell coordinate that enter the bucket index
 };
 
+// Bucket of a cell: Morton code of the low `bits` bits of its three coordinates (H = 2^(3 bits)
+// buckets).  Neighbouring cells land in neighbouring buckets, so the 27 probes of a particle and
+// the candidates they list are close in memory; cells 2^bits apart alias into one bucket and are
+// told apart by the stored cell coordinates.
+__device__ __forceinline__ unsigned lub_spread(unsigned v) {  // 10 bits -> every third bit
+    v = (v | (v << 16)) & 0x030000FFu;
+    v = (v | (v << 8)) & 0x0300F00Fu;
+    v = (v | (v << 4)) & 0x030C30C3u;
+    v = (v | (v << 2)) & 0x09249249u;
+    return v;
+}
 __device__ __forceinline__ unsigned lub_hash(int cx, int cy, int cz, unsigned mask) {
-    return ((static_cast<unsigned>(cx) * 73856093u) ^ (static_cast<unsigned>(cy) * 19349663u) ^
-            (static_cast<unsigned>(cz) * 83492791u)) & mask;
+    return lub_spread(static_cast<unsigned>(cx) & mask) | (lub_spread(static_cast<unsigned>(cy) & mask) << 1) |
+           (lub_spread(static_cast<unsigned>(cz) & mask) << 2);
 }
 
 __device__ __forceinline__ int lub_cell_coord(double x, const LubGrid& g) {
@@ -94,6 +105,22 @@ lub_sort_kernel(const unsigned* __restrict__ start, int* __restrict__ order, con
     }
 }
 
+// sorted copies: particle data in bucket order, so that the force kernel reads contiguous runs
+template <typename T4>
+__global__ void __launch_bounds__(256)
+lub_gather_kernel(const T4* __restrict__ pos, const T4* __restrict__ vel, const int4* __restrict__ cell,
+                  const int* __restrict__ order, T4* __restrict__ spos, T4* __restrict__ svel,
+                  int4* __restrict__ scell, const int N) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= N) return;
+    const int i = order[k];
+    spos[k] = pos[i];
+    svel[k] = vel[i];
+    int4 c = cell[i];
+    c.w = i;  // the particle's own index travels with its cell
+    scell[k] = c;
+}
+
 // nearest-image displacement of one component as a double, by the rule of the pair kernels
 // (reading B2): fp32 modes decide n on the fp32 difference, fp64 on the double one.
 template <typename S>
@@ -127,17 +154,19 @@ __device__ __forceinline__ bool lub_inside(double, double dx, double dy, double 
 // force_out itself (each thread reads its own element before it writes it).
 template <typename T4>
 __global__ void __launch_bounds__(128)
-lub_force_kernel(const T4* __restrict__ pos, const T4* __restrict__ vel, const T4* fext,
-                 const double gx, const double gy, const double gz, const int4* __restrict__ cell,
-                 const unsigned* __restrict__ start, const int* __restrict__ order,
-                 T4* force_out, const LubGrid g, const double a, const double mu0,
-                 const int N) {
+lub_force_kernel(const T4* __restrict__ spos, const T4* __restrict__ svel, const T4* fext,
+                 const double gx, const double gy, const double gz, const int4* __restrict__ scell,
+                 const unsigned* __restrict__ start, T4* force_out, const LubGrid g, const double a,
+                 const double mu0, const int N) {
     typedef typename Vec4<T4>::S S;
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= N) return;
-    const T4 pi = pos[i];
-    const T4 vi = vel[i];
-    const int4 ci = cell[i];
+    const int k0 = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k0 >= N) return;
+    // thread k0 owns the k0-th particle in bucket order: the lanes of a warp sit in the same or in
+    // neighbouring cells, probe the same buckets and read the same runs of the sorted copies
+    const T4 pi = spos[k0];
+    const T4 vi = svel[k0];
+    const int4 ci = scell[k0];
+    const int i = ci.w;
     const double nine_a2 = 9.0 * a * a, inv_a = 1.0 / a, inv_mu0 = 1.0 / mu0;
     double cx = 0.0, cy = 0.0, cz = 0.0;
     for (int oz = -1; oz <= 1; ++oz)
@@ -152,10 +181,9 @@ lub_force_kernel(const T4* __restrict__ pos, const T4* __restrict__ vel, const T
                 const unsigned h = lub_hash(nx, ny, nz, g.mask);
                 const unsigned e = start[h + 1];
                 for (unsigned k = start[h]; k < e; ++k) {
-                    const int j = order[k];
-                    const int4 cj = cell[j];
-                    if (j == i || cj.x != nx || cj.y != ny || cj.z != nz) continue;  // self / collision
-                    const T4 pj = pos[j];
+                    const int4 cj = scell[k];
+                    if (cj.w == i || cj.x != nx || cj.y != ny || cj.z != nz) continue;  // self / alias
+                    const T4 pj = spos[k];
                     const double dx = lub_disp<S>(pi.x, pj.x, g), dy = lub_disp<S>(pi.y, pj.y, g),
                                  dz = lub_disp<S>(pi.z, pj.z, g);
                     if (!lub_inside(S(0), dx, dy, dz, nine_a2)) continue;
@@ -167,7 +195,7 @@ lub_force_kernel(const T4* __restrict__ pos, const T4* __restrict__ vel, const T
                     const double ls = log(s);
                     const double par = (0.25 / s - 0.225 * ls) * inv_mu0;
                     const double per = (-ls * (1.0 / 6.0)) * inv_mu0;
-                    const T4 vj = vel[j];
+                    const T4 vj = svel[k];
                     const double wx = static_cast<double>(vi.x) - static_cast<double>(vj.x);
                     const double wy = static_cast<double>(vi.y) - static_cast<double>(vj.y);
                     const double wz = static_cast<double>(vi.z) - static_cast<double>(vj.z);
