@@ -30,7 +30,7 @@ FLOPS_PER_PAIR = {"rpy": 34, "oseen": 29}       # algorithmic flops (DESIGN.md, 
 FLOPS_NEAREST_IMAGE = 15                        # + 3 x (fma, add, fma) per pair in a periodic box
 FP32_LANES_PER_SM, FP64_LANES_PER_SM = 128, 64  # CUDA-core FMA lanes per SM (measured: ubench)
 # DRAM bytes per pair-kernel launch from the ncu --set full capture named in profiles/README.md
-NCU_TRAFFIC_BYTES = {(1048576, "f32", "rpy"): 43.9e6}  # profiles/r01_pairs_f32_ncu_full.md
+NCU_TRAFFIC_BYTES = {(1048576, "f32", "rpy"): 43.7e6}  # profiles/r01c_pairs_f32_ncu_full.md
 
 
 def parse_args():
