@@ -19,13 +19,24 @@ namespace sd {
 constexpr int kTJ64 = 64;  // j records per tile (4 KiB)
 
 // y0 = MUFU.RSQ(float(r2)) has relative error e0 <~ 2^-22; one Halley step
-//   e = 1 - r2 y0^2 ,  y = y0 (1 + e/2 + 3 e^2/8)
-// leaves ~0.3 e0^3 ~ 1e-21, i.e. rounding level, in 5 fp64 instructions.
+//   e = 1 - r2 y0^2 ,  y = y0 + y0 e (1/2 + 3 e/8)
+// leaves ~0.3 e0^3 ~ 1e-21, i.e. rounding level, in 5 fp64 instructions.  Evaluating the small
+// correction y0 e (1/2 + 3e/8) on the idle FP32 pipe (-DSD_F64_HALLEY_IN_F32: 24 instead of 26
+// fp64 instructions per pair, two more F2F conversions on the XU pipe) is accurate enough but
+// measured 3.4 % SLOWER at N = 1 M (5.55e11 vs 5.745e11 pairs/s): the conversions cost more issue
+// slots than the two DFMAs they replace.
 __device__ __forceinline__ double rsqrt_nr2(const double r2, const float r2f) {
-    const double y = static_cast<double>(rsq_approx(r2f));
+    const float yf = rsq_approx(r2f);
+    const double y = static_cast<double>(yf);
     const double e = fma(-r2, y * y, 1.0);
+#ifdef SD_F64_HALLEY_IN_F32
+    const float ef = static_cast<float>(e);
+    const float corr = (yf * ef) * fmaf(0.375f, ef, 0.5f);
+    return y + static_cast<double>(corr);
+#else
     const double p = fma(0.375, e, 0.5);
     return fma(y * e, p, y);
+#endif
 }
 
 // PBC: nearest image as in the fp32 kernel, d <- d - L rint(d / L) with rint taken as

@@ -249,3 +249,23 @@ def test_fp32_euler_steps_on_the_commensurate_lattice_step_by_step(gpu, cells):
         got = dp.cpu().numpy()[:, :3].astype(np.float64)
         assert np.abs(got - want).max() <= 1e-5 * 0.001 * np.abs(vwant).max() + 2.0 ** -24 * np.abs(want).max()
     ctx.close()
+
+
+def test_box_at_bench_size_sampled_rows(gpu):
+    """`bench.py --box` configuration (N = 1,048,576, fp32-Kahan, RPY, box = the cloud's own cube):
+    4096 seeded rows against the oracle, plus a property that holds at any size: moving every
+    particle by one box length along x leaves the velocities unchanged up to fp32 rounding."""
+    torch, sd = gpu
+    n = 1048576
+    pos, force = wl.sweep(n)
+    L = wl.cube_side(n, 0.01)
+    got, p, f = gpu_apply_box(torch, sd, pos, force, L, "PREC_F32_KAHAN", 0, "i8_rpy_kahan_pbc")
+    rows = wl.row_subset(n, 4096, wl.SEED_BASE + 90)
+    want = orc.apply_rows(p, f, rows, wl.A, wl.ETA, box=float(np.float32(L)), image=orc.IMAGE_F32)
+    assert rel_err(got[rows], want) <= TOL["PREC_F32_KAHAN"]
+    assert np.all(np.isfinite(got))
+    shifted = pos.copy()
+    shifted[:, 0] += float(np.float32(L))
+    got2, _, _ = gpu_apply_box(torch, sd, shifted, force, L, "PREC_F32_KAHAN", 0)
+    # the shifted coordinates round differently in fp32 (|x| up to 1.5 L): input rounding, ~1e-4 a
+    assert rel_err(got2[rows], got[rows]) <= 2e-3
