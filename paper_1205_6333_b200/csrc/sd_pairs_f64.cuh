@@ -5,9 +5,8 @@
 //  * 64-byte records {x, y, z, 0 | Fx, Fy, Fz, 0} of doubles, 64 j per 4 KiB tile;
 //  * no packed arithmetic (there is no DFMA2); one thread owns I particles (4 at large N with
 //    one CTA per SM, 2 with two CTAs per SM below: halves the LDS.128 per pair);
-//  * 1/r: MUFU.RSQ on the fp32-rounded r^2 as a 22-bit seed, then one third-order (Halley) step
-//    in fp64 (relative error ~2e-7 -> ~1e-21, i.e. rounding level); no fp64 division or sqrt
-//    in the loop;
+//  * 1/r: MUFU.RSQ on the fp32-rounded r^2 as a 22-bit seed, then one Newton step in fp64
+//    (relative error ~2e-7 -> <= 8.6e-14, see rsqrt_nr2); no fp64 division or sqrt in the loop;
 //  * fp64 sums need no compensation (measured 2e-13 vs the oracle's long-double rows at
 //    N = 65536); min r^2 is tracked on the fp32 copy of r^2 that the seed needs anyway.
 #pragma once
@@ -18,24 +17,28 @@ namespace sd {
 
 constexpr int kTJ64 = 64;  // j records per tile (4 KiB)
 
-// y0 = MUFU.RSQ(float(r2)) has relative error e0 <~ 2^-22; one Halley step
-//   e = 1 - r2 y0^2 ,  y = y0 + y0 e (1/2 + 3 e/8)
-// leaves ~0.3 e0^3 ~ 1e-21, i.e. rounding level, in 5 fp64 instructions.  Evaluating the small
-// correction y0 e (1/2 + 3e/8) on the idle FP32 pipe (-DSD_F64_HALLEY_IN_F32: 24 instead of 26
-// fp64 instructions per pair, two more F2F conversions on the XU pipe) is accurate enough but
-// measured 3.4 % SLOWER at N = 1 M (5.55e11 vs 5.745e11 pairs/s): the conversions cost more issue
-// slots than the two DFMAs they replace.
+// y0 = MUFU.RSQ(float(r2)) has relative error d0 <= 2^-22.4 + 2^-24 (MUFU + the rounding of r2 to
+// float) ~ 2.4e-7.  With e = 1 - r2 y0^2 ~ -2 d0 (a cancellation: fp64), one Newton step
+//   y = y0 + y0 e / 2
+// leaves a relative error of 3/8 e^2 <= 8.6e-14 in 1/r (always too small), i.e. <= 2.6e-13 in the
+// 1/r^3 terms: 40x below the 1e-11 tolerance of this path, in 4 fp64 instructions.  The kernel is
+// bound by the FP64 pipe (80 % active, 2 cycles per warp instruction), so the count matters:
+//   Newton (shipped)                      25 fp64 instructions per pair   5.985e11 pairs/s at N = 1 M
+//   Halley, y0 e (1/2 + 3e/8)  (-DSD_F64_HALLEY)      26, error ~1e-21    5.736e11
+//   Halley with the correction in fp32 (-DSD_F64_HALLEY_IN_F32)  24 + 2 F2F   5.549e11
 __device__ __forceinline__ double rsqrt_nr2(const double r2, const float r2f) {
     const float yf = rsq_approx(r2f);
     const double y = static_cast<double>(yf);
     const double e = fma(-r2, y * y, 1.0);
-#ifdef SD_F64_HALLEY_IN_F32
+#if defined(SD_F64_HALLEY_IN_F32)
     const float ef = static_cast<float>(e);
     const float corr = (yf * ef) * fmaf(0.375f, ef, 0.5f);
     return y + static_cast<double>(corr);
-#else
+#elif defined(SD_F64_HALLEY)
     const double p = fma(0.375, e, 0.5);
     return fma(y * e, p, y);
+#else
+    return fma(y * e, 0.5, y);
 #endif
 }
 
