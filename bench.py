@@ -50,6 +50,9 @@ def parse_args():
                          "Euler steps of 0.001 tau_s per timed step; reports simulation steps/s")
     ap.add_argument("--staging", choices=["bulk", "naive", "sync"], default="bulk",
                     help="memory-access ablation (PAPER.md Appendix A): how j records reach the threads")
+    ap.add_argument("--full-loop", action="store_true",
+                    help="with --fcc-cells: run the paper's whole step (PAPER.md:96-109), i.e. switch the "
+                         "lubrication correction of the forces on (sd_set_lubrication)")
     ap.add_argument("--lub", action="store_true",
                     help="instead of the product: the lubrication correction of the forces (Eq. 8, "
                          "PAPER.md:80-104) on N uniform points at phi = 0.05; reports particles/s")
@@ -147,7 +150,8 @@ def run_fcc_steps(args, rank):
     npdt = np.float64 if f64mode else np.float32
     name = (f"sd_step N={n} fcc lattice n=0.1/a^3 (+1e-2 a seeded jitter) in its periodic box "
             f"L={L:.3f} a, nearest image, gravity, Euler dt=0.001, {sim_steps} steps per timed step, "
-            f"{args.tensor.upper()}, {'fp64' if f64mode else 'fp32-Kahan'}")
+            f"{args.tensor.upper()}, {'fp64' if f64mode else 'fp32-Kahan'}"
+            + (", lubrication correction on (Eq. 8, previous-step velocities)" if args.full_loop else ""))
     base = {"metric": "simulation steps/s at N (Euler step = one mobility product + update)",
             "unit": "steps/s", "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "data": "synthetic",
@@ -158,15 +162,19 @@ def run_fcc_steps(args, rank):
         otensor = orc.TENSOR_RPY if args.tensor == "rpy" else orc.TENSOR_OSEEN
         p64 = wl.to_xyzw(pos, npdt)[:, :3].astype(np.float64)
         F = wl.gravity_forces(n)
+        def ostep(k):
+            if args.full_loop:
+                return orc.step_lub(p64, np.zeros_like(p64), F, wl.A, wl.ETA, dt, k, orc.INT_EULER, otensor, box=L)
+            return orc.step(p64, F, wl.A, wl.ETA, dt, k, orc.INT_EULER, otensor, box=L)
         t0 = time.perf_counter()
-        orc.step(p64, F, wl.A, wl.ETA, dt, 1, orc.INT_EULER, otensor, box=L)
+        ostep(1)
         per = max(time.perf_counter() - t0, 1e-6)
         k = int(max(1, min(sim_steps, 2.0 / per)))  # ~2 s per timed step
         for _ in range(args.warmup):
-            orc.step(p64, F, wl.A, wl.ETA, dt, k, orc.INT_EULER, otensor, box=L)
+            ostep(k)
         t0 = time.perf_counter()
         for _ in range(args.steps):
-            orc.step(p64, F, wl.A, wl.ETA, dt, k, orc.INT_EULER, otensor, box=L)
+            ostep(k)
         t = time.perf_counter() - t0
         value = args.steps * k / t
         desc = f"{k} Euler steps of all {n} rows per timed step"
@@ -193,11 +201,13 @@ def run_fcc_steps(args, rank):
     ctx.set_precision(sd.PREC_F64 if f64mode else sd.PREC_F32_KAHAN)
     ctx.set_tensor(sd.TENSOR_RPY if args.tensor == "rpy" else sd.TENSOR_OSEEN)
     ctx.set_box(L)
+    ctx.set_lubrication(args.full_loop)
     g = (0.0, 0.0, -1.0)
 
     def one_run():
         d_pos.copy_(d_pos0)
         ctx.reset_compensation()
+        ctx.set_velocity(None)
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record()
         ctx.step(d_pos, dt, sim_steps, sd.INT_EULER, gravity=g)

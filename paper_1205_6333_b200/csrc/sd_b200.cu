@@ -39,6 +39,18 @@ struct Config {
 
 }  // namespace
 
+namespace {
+constexpr long long kGraphSteps = 16;  // even: the small-N Euler path ping-pongs two buffers
+struct GraphKey {  // everything a captured step sequence has baked in (besides the context state)
+    void* pos;
+    const void* force;
+    double gx, gy, gz;
+    bool has_gravity;
+    double dt;
+    int integrator;
+};
+}  // namespace
+
 struct sd_ctx {
     long long N = 0;
     long long Nrec = 0;
@@ -63,6 +75,11 @@ struct sd_ctx {
     void* lub_tmp = nullptr;         // cub scan scratch
     size_t lub_tmp_bytes = 0;
     unsigned lub_H = 0;
+    // CUDA graph of kGraphSteps steps of the full loop (constant forces + lubrication)
+    cudaStream_t cap_stream = nullptr;
+    cudaGraphExec_t gexec = nullptr;
+    GraphKey gkey{};
+    long long graph_launches = 0;
     int device = 0;
     int num_sms = 0;
     Config cfg;
@@ -125,7 +142,13 @@ const void* f64_pick(bool rpy) {
     return rpy ? f64_kernel<I, 0, PBC>() : f64_kernel<I, 1, PBC>();
 }
 
+void drop_graph(sd_ctx* c) {
+    if (c->gexec) cudaGraphExecDestroy(c->gexec);
+    c->gexec = nullptr;
+}
+
 void free_buffers(sd_ctx* c) {
+    drop_graph(c);
     void** bufs[] = {&c->rec,       &c->part,        &c->vel,       &c->pos_lo, &c->pos_half, &c->pos_alt,
                      &c->force_buf, &c->stage_pos,   &c->stage_force, &c->stage_vel, &c->probe};
     for (void** b : bufs) {
@@ -485,6 +508,29 @@ sd_status launch_stepper(sd_ctx* c, void* pos, const void* force, const double g
     return launch_stepper_t<float4, true>(c, pos, force, g, dt, n_steps, integrator, st);
 }
 
+// cell-grid scratch of the lubrication step (allocated on first use, never inside a stream capture)
+sd_status ensure_lub_buffers(sd_ctx* c) {
+    if (!c->lub_cell) {
+        const int n = static_cast<int>(c->N);
+        cudaStream_t st = nullptr;
+        unsigned H = 512;  // 2^(3 bits) buckets, at least one per particle
+        while (H < static_cast<unsigned>(n)) H <<= 3;
+        c->lub_H = H;
+        SD_CUDA(c, cudaMalloc(&c->lub_spos, 4 * elem_size(c->precision) * n));
+        SD_CUDA(c, cudaMalloc(&c->lub_svel, 4 * elem_size(c->precision) * n));
+        SD_CUDA(c, cudaMalloc(&c->lub_scell, sizeof(int4) * n));
+        SD_CUDA(c, cudaMalloc(&c->lub_cell, sizeof(int4) * n));
+        SD_CUDA(c, cudaMalloc(&c->lub_count, sizeof(unsigned) * (H + 1)));
+        SD_CUDA(c, cudaMalloc(&c->lub_start, sizeof(unsigned) * (H + 1)));
+        SD_CUDA(c, cudaMalloc(&c->lub_cursor, sizeof(unsigned) * H));
+        SD_CUDA(c, cudaMalloc(&c->lub_order, sizeof(int) * n));
+        SD_CUDA(c, cub::DeviceScan::ExclusiveSum(nullptr, c->lub_tmp_bytes, c->lub_count, c->lub_start,
+                                                 static_cast<int>(H + 1), st));
+        SD_CUDA(c, cudaMalloc(&c->lub_tmp, c->lub_tmp_bytes));
+    }
+    return SD_OK;
+}
+
 // force_out = F^ext - C(pos, vel)  (sd_lub.cuh).  fext NULL: uniform force g.
 sd_status launch_lubrication(sd_ctx* c, const void* pos, const void* vel, const void* fext,
                              const double g[3], void* force_out, cudaStream_t st) {
@@ -505,21 +551,9 @@ sd_status launch_lubrication(sd_ctx* c, const void* pos, const void* vel, const 
             return fail(c, SD_ERR_UNSUPPORTED, "lubrication in a periodic box needs a box side of at least 9 a");
         grid.nc = std::min(grid.nc, 1024);
     }
-    if (!c->lub_cell) {
-        unsigned H = 512;  // 2^(3 bits) buckets, at least one per particle
-        while (H < static_cast<unsigned>(n)) H <<= 3;
-        c->lub_H = H;
-        SD_CUDA(c, cudaMalloc(&c->lub_spos, 4 * elem_size(c->precision) * n));
-        SD_CUDA(c, cudaMalloc(&c->lub_svel, 4 * elem_size(c->precision) * n));
-        SD_CUDA(c, cudaMalloc(&c->lub_scell, sizeof(int4) * n));
-        SD_CUDA(c, cudaMalloc(&c->lub_cell, sizeof(int4) * n));
-        SD_CUDA(c, cudaMalloc(&c->lub_count, sizeof(unsigned) * (H + 1)));
-        SD_CUDA(c, cudaMalloc(&c->lub_start, sizeof(unsigned) * (H + 1)));
-        SD_CUDA(c, cudaMalloc(&c->lub_cursor, sizeof(unsigned) * H));
-        SD_CUDA(c, cudaMalloc(&c->lub_order, sizeof(int) * n));
-        SD_CUDA(c, cub::DeviceScan::ExclusiveSum(nullptr, c->lub_tmp_bytes, c->lub_count, c->lub_start,
-                                                 static_cast<int>(H + 1), st));
-        SD_CUDA(c, cudaMalloc(&c->lub_tmp, c->lub_tmp_bytes));
+    {
+        sd_status a = ensure_lub_buffers(c);
+        if (a != SD_OK) return a;
     }
     const unsigned H = c->lub_H;
     unsigned bits = 0;
@@ -530,6 +564,10 @@ sd_status launch_lubrication(sd_ctx* c, const void* pos, const void* vel, const 
     const int nb = (n + 255) / 256;
     const double gx = g ? g[0] : 0.0, gy = g ? g[1] : 0.0, gz = g ? g[2] : 0.0;
     sd_status s;
+#define SD_LUB_FORCE_ARGS(T4)                                                                       \
+    static_cast<const T4*>(c->lub_spos), static_cast<const T4*>(c->lub_svel),                       \
+        static_cast<const T4*>(fext), gx, gy, gz, c->lub_scell, c->lub_start,                       \
+        static_cast<T4*>(force_out), grid, c->a, c->mu0, n
 #define SD_LUB(T4)                                                                                  \
     sd::lub_count_kernel<T4><<<nb, 256, 0, st>>>(static_cast<const T4*>(pos), c->lub_cell,          \
                                                  c->lub_count, grid, n);                           \
@@ -545,10 +583,12 @@ sd_status launch_lubrication(sd_ctx* c, const void* pos, const void* vel, const 
         static_cast<const T4*>(pos), static_cast<const T4*>(vel), c->lub_cell, c->lub_order,        \
         static_cast<T4*>(c->lub_spos), static_cast<T4*>(c->lub_svel), c->lub_scell, n);             \
     if ((s = check_launch(c, "lub_gather_kernel")) != SD_OK) return s;                              \
-    sd::lub_force_kernel<T4><<<(n + 127) / 128, 128, 0, st>>>(                                      \
-        static_cast<const T4*>(c->lub_spos), static_cast<const T4*>(c->lub_svel),                   \
-        static_cast<const T4*>(fext), gx, gy, gz, c->lub_scell, c->lub_start,                       \
-        static_cast<T4*>(force_out), grid, c->a, c->mu0, n);                                       \
+    if (n >= 262144)                                                                                \
+        sd::lub_force_kernel<T4, 1><<<(n + 127) / 128, 128, 0, st>>>(SD_LUB_FORCE_ARGS(T4));        \
+    else if (n >= 32768)                                                                            \
+        sd::lub_force_kernel<T4, 8><<<(n * 8 + 127) / 128, 128, 0, st>>>(SD_LUB_FORCE_ARGS(T4));    \
+    else                                                                                            \
+        sd::lub_force_kernel<T4, 32><<<(n * 32 + 127) / 128, 128, 0, st>>>(SD_LUB_FORCE_ARGS(T4));  \
     return check_launch(c, "lub_force_kernel")
     if (c->precision == SD_PREC_F64) {
         SD_LUB(double4);
@@ -648,6 +688,7 @@ sd_status sd_set_dispatch(sd_ctx* ctx, long long small_apply_max, int particles_
 sd_status sd_set_position_compensation(sd_ctx* ctx, int on) {
     if (!ctx) return fail(nullptr, SD_ERR_INVALID_ARG, "sd_set_position_compensation: ctx is NULL");
     ctx->pos_comp = on ? 1 : 0;
+    drop_graph(ctx);
     ctx->lo_valid = false;  // low words are re-zeroed before the next step
     return SD_OK;
 }
@@ -679,6 +720,7 @@ sd_status sd_set_box(sd_ctx* ctx, double box_side) {
     if (staging_forbids(ctx, ctx->tensor, ctx->precision, box_side)) return fail(ctx, SD_ERR_UNSUPPORTED, kStagingMsg);
     const bool was = ctx->box > 0.0, is = box_side > 0.0;
     ctx->box = box_side;
+    drop_graph(ctx);
     if (was == is) return SD_OK;  // same kernels, only the constants change
     cudaDeviceSynchronize();
     return configure(ctx);
@@ -745,6 +787,10 @@ sd_status sd_step(sd_ctx* ctx, void* pos, sd_force_fn fn, void* user, const void
     const bool lub = ctx->lubrication != 0;
     if (!fn && !lub && ctx->N <= sd::kStepperMax)  // all steps in one launch
         return launch_stepper(ctx, pos, force, gravity, dt, n_steps, integrator, st);
+
+    // `count` steps enqueued on stream `st` (also used under stream capture, see below)
+    auto run_steps = [&](cudaStream_t st, long long count) -> sd_status {
+        sd_status s;
     // Forces that change from product to product (a caller callback and / or the lubrication
     // correction with the velocities of the previous product) are rebuilt in
     // the context's force buffer before every product.
@@ -753,7 +799,7 @@ sd_status sd_step(sd_ctx* ctx, void* pos, sd_force_fn fn, void* user, const void
         const void* fe = force;
         const double* gg = gravity;
         if (fn) {
-            if (fn(p, ctx->force_buf, ctx->N, user, stream) != 0)
+            if (fn(p, ctx->force_buf, ctx->N, user, static_cast<void*>(st)) != 0)
                 return fail(ctx, SD_ERR_INVALID_ARG, "sd_step: force callback failed");
             fe = ctx->force_buf;
         }
@@ -765,7 +811,7 @@ sd_status sd_step(sd_ctx* ctx, void* pos, sd_force_fn fn, void* user, const void
         const double* g = (dynamic || force) ? nullptr : gravity;
         void* cur = pos;
         void* other = ctx->pos_alt;
-        for (long long step = 0; step < n_steps; ++step) {
+        for (long long step = 0; step < count; ++step) {
             if (integrator == SD_INT_EULER) {
                 if (dynamic && (s = fill(cur)) != SD_OK) return s;
                 s = launch_small_apply(ctx, cur, fptr, g, ctx->vel, cur, other, dt, sd::FIN_EULER, st);
@@ -795,7 +841,7 @@ sd_status sd_step(sd_ctx* ctx, void* pos, sd_force_fn fn, void* user, const void
         if (r != SD_OK) return r;
         return launch_pack(ctx, nullptr, ctx->force_buf, sd::PACK_FORCE, nullptr, st);
     };
-    for (long long step = 0; step < n_steps; ++step) {
+    for (long long step = 0; step < count; ++step) {
         if ((s = callback(pos)) != SD_OK) return s;
         if ((s = launch_pairs(ctx, st)) != SD_OK) return s;
         if (integrator == SD_INT_EULER) {
@@ -808,11 +854,58 @@ sd_status sd_step(sd_ctx* ctx, void* pos, sd_force_fn fn, void* user, const void
         }
     }
     return SD_OK;
+    };
+
+    // The lubrication step is eight small launches: with it the loop is bound by the host's launch
+    // rate (~100 us per step at any N), not by the GPU.  Constant-force runs are a fixed sequence of
+    // launches, so kGraphSteps steps are captured once into a CUDA graph and replayed.
+    if (lub && !fn && !ctx->profiling && n_steps >= 2 * kGraphSteps) {
+        GraphKey key;
+        std::memset(&key, 0, sizeof(key));  // padding bytes take part in the memcmp below
+        key.pos = pos;
+        key.force = force;
+        if (gravity) key.gx = gravity[0], key.gy = gravity[1], key.gz = gravity[2];
+        key.has_gravity = gravity != nullptr;
+        key.dt = dt;
+        key.integrator = static_cast<int>(integrator);
+        if (!ctx->gexec || std::memcmp(&key, &ctx->gkey, sizeof(GraphKey)) != 0) {
+            drop_graph(ctx);
+            if ((s = ensure_lub_buffers(ctx)) != SD_OK) return s;
+            if (!ctx->cap_stream) SD_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->cap_stream, cudaStreamNonBlocking));
+            const long long launches0 = ctx->launches;
+            SD_CUDA(ctx, cudaStreamBeginCapture(ctx->cap_stream, cudaStreamCaptureModeThreadLocal));
+            s = run_steps(ctx->cap_stream, kGraphSteps);
+            cudaGraph_t graph = nullptr;
+            cudaError_t e = cudaStreamEndCapture(ctx->cap_stream, &graph);
+            if (s != SD_OK || e != cudaSuccess) {
+                if (graph) cudaGraphDestroy(graph);
+                cudaGetLastError();
+                return s != SD_OK ? s : fail(ctx, SD_ERR_CUDA, std::string("sd_step: graph capture: ") + cudaGetErrorString(e));
+            }
+            ctx->graph_launches = ctx->launches - launches0;
+            ctx->launches = launches0;
+            e = cudaGraphInstantiate(&ctx->gexec, graph, 0);
+            cudaGraphDestroy(graph);
+            if (e != cudaSuccess) {
+                ctx->gexec = nullptr;
+                return fail(ctx, SD_ERR_CUDA, std::string("sd_step: graph instantiate: ") + cudaGetErrorString(e));
+            }
+            ctx->gkey = key;
+        }
+        long long done = 0;
+        for (; done + kGraphSteps <= n_steps; done += kGraphSteps) {
+            SD_CUDA(ctx, cudaGraphLaunch(ctx->gexec, st));
+            ctx->launches += ctx->graph_launches;
+        }
+        return done < n_steps ? run_steps(st, n_steps - done) : SD_OK;
+    }
+    return run_steps(st, n_steps);
 }
 
 sd_status sd_set_lubrication(sd_ctx* ctx, int on) {
     if (!ctx) return fail(nullptr, SD_ERR_INVALID_ARG, "sd_set_lubrication: ctx is NULL");
     ctx->lubrication = on ? 1 : 0;
+    drop_graph(ctx);
     return SD_OK;
 }
 
@@ -932,6 +1025,7 @@ void sd_destroy(sd_ctx* ctx) {
             cudaEventDestroy(ev.second);
         }
     free_buffers(ctx);
+    if (ctx->cap_stream) cudaStreamDestroy(ctx->cap_stream);
     delete ctx;
 }
 
