@@ -125,8 +125,9 @@ sd_status fail(sd_ctx* ctx, sd_status code, const std::string& msg) {
     } while (0)
 
 template <int I2, int TENSOR, int ACC, bool PBC>
-const void* f32_kernel() {
-    return reinterpret_cast<const void*>(&sd::pairs_f32_kernel<I2, TENSOR, ACC, PBC>);
+const void* f32_kernel() {  // the 2-particle-per-thread variant works on 32-record tiles
+    return reinterpret_cast<const void*>(
+        &sd::pairs_f32_kernel<I2, TENSOR, ACC, PBC, sd::STAGE_BULK, (I2 == 1) ? sd::kTJSmall : sd::kTJ>);
 }
 template <int I, int TENSOR, bool PBC>
 const void* f64_kernel() {
@@ -187,7 +188,7 @@ sd_status configure(sd_ctx* c) {
         int i2 = (c->N > sd::kIpt8Min) ? 4 : (c->N > sd::kIpt4Min ? 2 : 1);
         if (c->ipt_override) i2 = c->ipt_override / 2;
         cfg.ipt = 2 * i2;
-        cfg.TJ = sd::kTJ;
+        cfg.TJ = (i2 == 1) ? sd::kTJSmall : sd::kTJ;
         static const char* names[3][2][2][2] = {
             {{{"pairs_f32x2_i2_rpy_kahan", "pairs_f32x2_i2_rpy_kahan_pbc"},
               {"pairs_f32x2_i2_rpy_plain", "pairs_f32x2_i2_rpy_plain_pbc"}},
@@ -214,8 +215,10 @@ sd_status configure(sd_ctx* c) {
                             "staging ablation exists for RPY, fp32-Kahan, free space only: call sd_set_staging(ctx, 0) first");
             const bool naive = c->staging == sd::STAGE_NAIVE;
 #define SD_STAGED(I2V)                                                                              \
-    (naive ? reinterpret_cast<const void*>(&sd::pairs_f32_kernel<I2V, 0, 0, false, sd::STAGE_NAIVE>) \
-           : reinterpret_cast<const void*>(&sd::pairs_f32_kernel<I2V, 0, 0, false, sd::STAGE_SYNC>))
+    (naive ? reinterpret_cast<const void*>(                                                         \
+                 &sd::pairs_f32_kernel<I2V, 0, 0, false, sd::STAGE_NAIVE, (I2V == 1) ? sd::kTJSmall : sd::kTJ>) \
+           : reinterpret_cast<const void*>(                                                         \
+                 &sd::pairs_f32_kernel<I2V, 0, 0, false, sd::STAGE_SYNC, (I2V == 1) ? sd::kTJSmall : sd::kTJ>))
             cfg.kernel = (i2 == 4) ? SD_STAGED(4) : ((i2 == 2) ? SD_STAGED(2) : SD_STAGED(1));
 #undef SD_STAGED
             static const char* snames[2][3] = {

@@ -5,24 +5,28 @@
 //
 // with the velocities of the previous product and the primed sum over j != i with r_ij < 3a
 // ("we truncate ad hoc at s = 1 or r = 3a").  The paper points to Verlet lists and particle
-// reordering for this O(N) step; here it is a hashed cell grid rebuilt on
-// every call, four small launches, no host synchronisation, deterministic:
-//   lub_count_kernel    cell (3 ints, side >= 3a) and bucket (spatial hash, H = 2^k >= 2N) of
-//                       every particle; bucket histogram by atomicAdd
+// reordering for this O(N) step; here it is a cell grid rebuilt on every
+// call, no host synchronisation, deterministic:
+//   lub_count_kernel    cell (3 ints, side >= 3a) and bucket (Morton code of the cell's low bits,
+//                       H = 8^k >= N buckets) of every particle; bucket histogram by atomicAdd
 //   exclusive scan      cub::DeviceScan over the H counters (library primitive, plumbing)
 //   lub_scatter_kernel  particle indices into their buckets (atomic cursor), then
 //   lub_sort_kernel     each bucket sorted by particle index: the summation order below, and
 //                       with it every bit of the result, does not depend on the atomics
-//   lub_force_kernel    one thread per particle i, taken in bucket order: 27 neighbour cells -> buckets -> candidates j
-//                       (a candidate whose cell differs is a hash collision and is skipped);
-//                       the cut-off r^2 < 9a^2 is decided in the arithmetic of the context
-//                       (fp32 fma chain in the fp32 modes, reading C3); an accepted
-//                       pair is evaluated in fp64 on the exact difference of the stored
+//   lub_gather_kernel   positions, velocities and cells copied into bucket order (the paper's
+//                       "particle reordering"): neighbouring cells are neighbouring memory
+//   lub_force_kernel    1 / 8 / 32 lanes per particle (by N), particles in bucket order: 27
+//                       neighbour cells -> buckets -> candidates j (a candidate whose cell differs
+//                       is a bucket alias and is skipped); the cut-off r^2 < 9a^2 is decided in
+//                       the arithmetic of the context (fp32 fma chain in the fp32 modes,
+//                       DESIGN.md reading C3), in fp32 contexts before any fp64 instruction; an
+//                       accepted pair is evaluated in fp64 on the exact difference of the stored
 //                       coordinates (s = r/a - 2 loses all digits in fp32 when the gap closes);
-//                       sums in fp64; writes F^ext - C rounded to the element type.
-// Memory-bound: ~60 B per particle read + 27 bucket probes; the pair terms are a few per
-// particle.  Periodic box: cells = floor(L / 3a) per edge (>= 3 required), neighbour cells wrap,
-// displacements take the nearest image by the rule of the pair kernels.
+//                       sums in fp64 in a fixed order; writes F^ext - C rounded to the element type.
+// Latency-bound (dependent loads bucket -> candidate -> position), 2 % of the HBM roofline at
+// N = 1 M (profiles/r01d_lubrication.md).  Periodic box: cells = floor(L / 3a) per edge (>= 3
+// required), neighbour cells wrap, displacements take the nearest image by the rule of the pair
+// kernels.
 #pragma once
 #include <cub/device/device_scan.cuh>
 

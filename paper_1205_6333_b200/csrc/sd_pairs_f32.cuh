@@ -33,6 +33,10 @@ namespace sd {
 constexpr int kThreads = 256;
 constexpr int kWarps = kThreads / 32;
 constexpr int kTJ = 128;     // j records per tile (4 KiB)
+// tile of the 2-particle-per-thread variant.  32-record tiles (finer work units at small N) were
+// measured: N = 6000 73.8 -> 57.8 us per product, N = 12000 157.7 -> 148.1, but N = 3000 29.0 -> 38.9
+// (four times the slots to reduce and barriers to cross); kept at 128.
+constexpr int kTJSmall = 128;
 constexpr int kStages = 4;   // ring depth
 constexpr int kPrefetch = 2; // tiles in flight ahead of the one being consumed
 constexpr int kChunk = 32;   // j per compensation chunk
@@ -294,14 +298,15 @@ __device__ __forceinline__ void kahan_merge2(f32x2& s, f32x2& c, const f32x2 p) 
     s = t;
 }
 
-template <int I2, int TENSOR, int ACC, bool PBC, int STAGE = STAGE_BULK>
+template <int I2, int TENSOR, int ACC, bool PBC, int STAGE = STAGE_BULK, int TJ = kTJ>
 __global__ void __launch_bounds__(kThreads, (I2 == 1) ? 3 : ((I2 == 2) ? 2 : 1))
 pairs_f32_kernel(const float4* __restrict__ rec, float4* __restrict__ part, const Schedule sch,
                  const PairCoef k, const int N, const long long slot_stride) {
     constexpr int I = 2 * I2;
     constexpr int IB = kThreads * I;
-    static_assert(kTJ * 2 == kThreads, "STAGE_SYNC copies one float4 of the tile per thread");
-    __shared__ __align__(128) float4 tiles[kStages][kTJ * 2];
+    static_assert(TJ * 2 <= kThreads, "STAGE_SYNC copies at most one float4 of the tile per thread");
+    static_assert(TJ % kChunk == 0, "a tile is a whole number of compensation chunks");
+    __shared__ __align__(128) float4 tiles[kStages][TJ * 2];
     __shared__ __align__(8) uint64_t full_bar[kStages];
     __shared__ __align__(8) uint64_t empty_bar[kStages];
 
@@ -329,8 +334,8 @@ pairs_f32_kernel(const float4* __restrict__ rec, float4* __restrict__ part, cons
         const int s = pf_n % kStages;
         const int q = pf_n / kStages;
         if (q > 0) mbar_wait(&empty_bar[s], (q - 1) & 1);
-        mbar_arrive_expect_tx(&full_bar[s], kTJ * 32);
-        bulk_load(&tiles[s][0], rec + static_cast<size_t>(pf_t) * (kTJ * 2), kTJ * 32, &full_bar[s]);
+        mbar_arrive_expect_tx(&full_bar[s], TJ * 32);
+        bulk_load(&tiles[s][0], rec + static_cast<size_t>(pf_t) * (TJ * 2), TJ * 32, &full_bar[s]);
         ++pf_n;
         if (++pf_t == T) pf_t = 0;
     };
@@ -379,17 +384,17 @@ pairs_f32_kernel(const float4* __restrict__ rec, float4* __restrict__ part, cons
                 mbar_wait(&full_bar[s], (n / kStages) & 1);
                 tile = &tiles[s][0];
             } else if (STAGE == STAGE_NAIVE) {
-                tile = rec + static_cast<size_t>(t0 + tt) * (kTJ * 2);
+                tile = rec + static_cast<size_t>(t0 + tt) * (TJ * 2);
             } else {
                 __syncthreads();  // everybody is done with the previous tile
-                tiles[0][tid] = rec[static_cast<size_t>(t0 + tt) * (kTJ * 2) + tid];
+                if (tid < TJ * 2) tiles[0][tid] = rec[static_cast<size_t>(t0 + tt) * (TJ * 2) + tid];
                 __syncthreads();
                 tile = &tiles[0][0];
             }
-            const int jbase = (t0 + tt) * kTJ;
+            const int jbase = (t0 + tt) * TJ;
 
 #pragma unroll 1
-            for (int ch = 0; ch < kTJ / kChunk; ++ch) {
+            for (int ch = 0; ch < TJ / kChunk; ++ch) {
                 const float4* cj = tile + ch * (kChunk * 2);
                 f32x2 qx[I2], qy[I2], qz[I2];  // value of p at chunk start (PLAIN only)
 #pragma unroll
