@@ -73,7 +73,8 @@ typedef int (*sd_force_fn)(const void* pos, void* force, long long N, void* user
 sd_status sd_create(sd_ctx** out, long long N, double a, double eta);
 
 /* Select the pair tensor / the arithmetic.  Changing the precision changes the element type
- * expected of pos/force/vel and resets the position compensation. */
+ * expected of pos/force/vel, resets the position compensation and zeroes the velocities of the
+ * last product; every other setter keeps them (the lubrication correction reads them). */
 sd_status sd_set_tensor(sd_ctx* ctx, sd_tensor tensor);
 sd_status sd_set_precision(sd_ctx* ctx, sd_precision precision);
 

@@ -87,6 +87,7 @@ struct sd_ctx {
     void* rec = nullptr;        // packed records
     void* part = nullptr;       // segment partial sums
     void* vel = nullptr;        // velocities of the last product
+    size_t vel_bytes = 0;
     void* pos_lo = nullptr;     // low words of the positions (fp32 modes)
     void* pos_half = nullptr;   // midpoint positions (for force callbacks)
     void* pos_alt = nullptr;    // ping-pong partner of pos (small-N Euler)
@@ -175,7 +176,16 @@ void free_buffers(sd_ctx* c) {
 // Pick the kernel variant for (N, precision, tensor), build the static schedule and
 // (re)allocate every scratch buffer.
 sd_status configure(sd_ctx* c) {
+    // the velocities of the last product survive a reconfiguration that keeps their element type
+    // (sd_set_box, sd_set_tensor, sd_set_dispatch, ...): the lubrication correction needs them
+    void* keep_vel = nullptr;
+    const size_t vel_bytes = static_cast<size_t>(c->Nrec) * 4 * elem_size(c->precision);
+    if (c->vel && c->vel_bytes == vel_bytes) {
+        keep_vel = c->vel;
+        c->vel = nullptr;
+    }
     free_buffers(c);
+    c->vel = keep_vel;
     Config cfg;
     const bool f64 = c->precision == SD_PREC_F64;
     const bool rpy = c->tensor == SD_TENSOR_RPY;
@@ -277,13 +287,15 @@ sd_status configure(sd_ctx* c) {
     SD_CUDA(c, cudaMalloc(&c->rec, nrec * 2 * v4));
     const size_t part_per_slot = f64 ? nrec * v4 : nrec * 2 * v4;
     SD_CUDA(c, cudaMalloc(&c->part, part_per_slot * cfg.max_slots));
-    SD_CUDA(c, cudaMalloc(&c->vel, nrec * v4));
+    if (!c->vel) {
+        SD_CUDA(c, cudaMalloc(&c->vel, nrec * v4));
+            c->vel_bytes = nrec * v4;
+    }
     SD_CUDA(c, cudaMalloc(&c->pos_lo, nrec * v4));
     SD_CUDA(c, cudaMalloc(&c->pos_half, nrec * v4));
     SD_CUDA(c, cudaMalloc(&c->pos_alt, nrec * v4));
     SD_CUDA(c, cudaMalloc(&c->force_buf, nrec * v4));
     SD_CUDA(c, cudaMemset(c->pos_lo, 0, nrec * v4));
-    SD_CUDA(c, cudaMemset(c->vel, 0, nrec * v4));
     SD_CUDA(c, cudaMalloc(&c->d_cta_u0, sizeof(long long) * (cfg.G + 1)));
     SD_CUDA(c, cudaMalloc(&c->d_blk_first, sizeof(int) * cfg.B));
     SD_CUDA(c, cudaMalloc(&c->d_blk_nslots, sizeof(int) * cfg.B));

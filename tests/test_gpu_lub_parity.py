@@ -156,3 +156,51 @@ def test_step_with_lubrication_matches_the_papers_loop(gpu, prec_name, ptol, vto
     if not (steps > 30 and dt_np == np.float32):
         assert np.abs(dp.cpu().numpy()[:, :3].astype(np.float64) - want_p2).max() <= 2 * ptol
     ctx.close()
+
+
+def test_graph_replay_follows_changes_of_arguments_and_settings(gpu):
+    """sd_step replays a captured CUDA graph of 16 steps when the lubrication correction is on and
+    the forces are constant.  Everything a capture bakes in -- dt, the position buffer, the force
+    array / gravity, the integrator, the box, the position compensation -- must trigger a new
+    capture when it changes.  fp64, N = 300, 34 steps per call, each call checked against the oracle
+    continued from the state it left."""
+    torch, sd = gpu
+    n = 300
+    pos = wl.rsa_cube(n, 0.25, wl.SEED_BASE + 310 + n, a=1.3)
+    fext = wl.gravity_forces(n) + 0.5 * wl.normal_forces(n, wl.SEED_BASE + 311 + n)
+    L = 1.5 * wl.cube_side(n, 0.25, a=1.3)
+    ctx = sd.Context(n, wl.A, wl.ETA)
+    ctx.set_precision(sd.PREC_F64)
+    ctx.set_lubrication(True)
+    state = {"p": pos.copy(), "v": np.zeros_like(pos)}
+
+    def run(dp, dt, integ, force=None, gravity=None, box=0.0):
+        f64 = fext if force is not None else wl.gravity_forces(n, gravity)
+        ctx.step(dp, dt, 34, integ, force=force, gravity=gravity)
+        torch.cuda.synchronize()
+        oi = orc.INT_EULER if integ == sd.INT_EULER else orc.INT_MIDPOINT
+        state["p"], state["v"] = orc.step_lub(state["p"], state["v"], f64, wl.A, wl.ETA, dt, 34, oi,
+                                              box=box, image=orc.IMAGE_F64)
+        state["calls"] = state.get("calls", 0) + 1
+        err = np.abs(dp.cpu().numpy()[:, :3] - state["p"]).max()
+        assert err <= 1e-9, f"call {state['calls']}: {err:.3e}"
+
+    dp = torch.from_numpy(wl.to_xyzw(pos, np.float64)).cuda()
+    df = torch.from_numpy(wl.to_xyzw(fext, np.float64)).cuda()
+    run(dp, 0.002, sd.INT_EULER, force=df)
+    run(dp, 0.002, sd.INT_EULER, force=df)                 # same key: replay
+    run(dp, 0.001, sd.INT_EULER, force=df)                 # new dt
+    run(dp, 0.001, sd.INT_MIDPOINT, force=df)              # new integrator
+    dq = dp.clone()                                        # new position buffer
+    run(dq, 0.001, sd.INT_MIDPOINT, force=df)
+    run(dq, 0.001, sd.INT_EULER, gravity=(0.0, 0.3, -1.0))   # gravity instead of the force array
+    run(dq, 0.001, sd.INT_EULER, gravity=(0.0, -0.3, -1.0))
+    ctx.set_box(L)                                         # same kernels, new constants
+    run(dq, 0.001, sd.INT_EULER, gravity=(0.0, -0.3, -1.0), box=L)
+    ctx.set_lubrication(False)                             # and off again: plain loop
+    ctx.step(dq, 0.001, 34, sd.INT_EULER, gravity=(0.0, -0.3, -1.0))
+    torch.cuda.synchronize()
+    want, _, _ = orc.step(state["p"], wl.gravity_forces(n, (0.0, -0.3, -1.0)), wl.A, wl.ETA, 0.001, 34,
+                          orc.INT_EULER, box=L, image=orc.IMAGE_F64)
+    assert np.abs(dq.cpu().numpy()[:, :3] - want).max() <= 1e-9
+    ctx.close()
