@@ -99,6 +99,7 @@ struct sd_ctx {
     long long* d_cta_u0 = nullptr;
     int* d_blk_first = nullptr;
     int* d_blk_nslots = nullptr;
+    int* d_cta_piece = nullptr;
     bool lo_valid = false;
     long long launches = 0;
     bool profiling = false;
@@ -169,6 +170,8 @@ void free_buffers(sd_ctx* c) {
     if (c->d_cta_u0) cudaFree(c->d_cta_u0);
     if (c->d_blk_first) cudaFree(c->d_blk_first);
     if (c->d_blk_nslots) cudaFree(c->d_blk_nslots);
+    if (c->d_cta_piece) cudaFree(c->d_cta_piece);
+    c->d_cta_piece = nullptr;
     c->d_cta_u0 = nullptr;
     c->d_blk_first = c->d_blk_nslots = nullptr;
 }
@@ -194,7 +197,7 @@ sd_status configure(sd_ctx* c) {
         const bool plain = c->precision == SD_PREC_F32_PLAIN;
         // particles per thread: 8 once there is enough work to balance 2048-particle i-blocks
         // over the SMs (more operand reuse per j record), 4 and 2 below that (measured
-        // crossovers, profiles/r01c_sweep.md).  N <= small_apply_max never reaches this kernel.
+        // crossovers, profiles/r01d_sweep.md).  N <= small_apply_max never reaches this kernel.
         int i2 = (c->N > sd::kIpt8Min) ? 4 : (c->N > sd::kIpt4Min ? 2 : 1);
         if (c->ipt_override) i2 = c->ipt_override / 2;
         cfg.ipt = 2 * i2;
@@ -242,7 +245,7 @@ sd_status configure(sd_ctx* c) {
         if (c->staging != sd::STAGE_BULK)
             return fail(c, SD_ERR_UNSUPPORTED,
                         "staging ablation exists for RPY, fp32-Kahan, free space only: call sd_set_staging(ctx, 0) first");
-        cfg.ipt = (c->N > sd::kIpt4Min64) ? 4 : (c->N > sd::kIpt4Min ? 2 : 1);
+        cfg.ipt = (c->N > sd::kIpt4Min64) ? 4 : (c->N > sd::kIpt2Min64 ? 2 : 1);
         if (c->ipt_override) cfg.ipt = std::max(1, c->ipt_override / 2);
         cfg.TJ = sd::kTJ64;
         static const char* names64[3][2][2] = {
@@ -299,6 +302,21 @@ sd_status configure(sd_ctx* c) {
     SD_CUDA(c, cudaMalloc(&c->d_cta_u0, sizeof(long long) * (cfg.G + 1)));
     SD_CUDA(c, cudaMalloc(&c->d_blk_first, sizeof(int) * cfg.B));
     SD_CUDA(c, cudaMalloc(&c->d_blk_nslots, sizeof(int) * cfg.B));
+    // Pieces differ by one unit.  The CTAs of the first (and only) wave land on SM blockIdx % #SM,
+    // so CTA k, k + #SM, k + 2 #SM share an SM; when U / G resonates with #SM (N = 6000: U / G =
+    // 1.27, period 3.7 = 148 / 40) the long pieces of a plain blockIdx -> piece map pile up on the
+    // same SMs (6 units on some, 3 on others: 73.8 us instead of 57).  Giving the CTAs of one SM
+    // consecutive pieces balances the SMs to within one unit.
+    std::vector<int> piece(cfg.G);
+    {
+        const int nsm = c->num_sms;
+        std::vector<int> first_of_sm(nsm + 1, 0);
+        for (int sm = 0; sm < nsm; ++sm)
+            first_of_sm[sm + 1] = first_of_sm[sm] + cfg.G / nsm + (sm < cfg.G % nsm ? 1 : 0);
+        for (int b = 0; b < cfg.G; ++b) piece[b] = first_of_sm[b % nsm] + b / nsm;
+    }
+    SD_CUDA(c, cudaMalloc(&c->d_cta_piece, sizeof(int) * cfg.G));
+    SD_CUDA(c, cudaMemcpy(c->d_cta_piece, piece.data(), sizeof(int) * cfg.G, cudaMemcpyHostToDevice));
     SD_CUDA(c, cudaMemcpy(c->d_cta_u0, u0.data(), sizeof(long long) * (cfg.G + 1), cudaMemcpyHostToDevice));
     SD_CUDA(c, cudaMemcpy(c->d_blk_first, first.data(), sizeof(int) * cfg.B, cudaMemcpyHostToDevice));
     SD_CUDA(c, cudaMemcpy(c->d_blk_nslots, nslots.data(), sizeof(int) * cfg.B, cudaMemcpyHostToDevice));
@@ -311,6 +329,7 @@ sd::Schedule schedule_of(const sd_ctx* c) {
     s.cta_u0 = c->d_cta_u0;
     s.blk_first_cta = c->d_blk_first;
     s.blk_nslots = c->d_blk_nslots;
+    s.cta_piece = c->d_cta_piece;
     s.T = c->cfg.T;
     s.B = c->cfg.B;
     s.G = c->cfg.G;

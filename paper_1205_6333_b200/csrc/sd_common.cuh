@@ -73,6 +73,7 @@ struct Schedule {
     const long long* cta_u0;   // [G + 1]
     const int* blk_first_cta;  // [B]
     const int* blk_nslots;     // [B]
+    const int* cta_piece;      // [G] piece (index into cta_u0) of CTA blockIdx.x, see sd_b200.cu
     int T;                     // j-tiles
     int B;                     // i-blocks
     int G;                     // CTAs

@@ -44,10 +44,11 @@ constexpr int kChunk = 32;   // j per compensation chunk
 #define SD_UNROLL_J 4
 #endif
 constexpr int kUnrollJ = SD_UNROLL_J;  // j per unrolled loop body
-// measured crossovers of the particles-per-thread variants (profiles/r01c_sweep.md)
-constexpr int kIpt4Min = 12288;    // above: 4 particles per thread in fp32, 2 in fp64
+// measured crossovers of the particles-per-thread variants (profiles/r01d_sweep.md)
+constexpr int kIpt4Min = 20480;    // above: 4 particles per thread in fp32
+constexpr int kIpt2Min64 = 12288;  // above: 2 particles per thread in fp64
 constexpr int kIpt8Min = 32768;    // above: 8 per thread in fp32
-constexpr int kIpt4Min64 = 24576;  // above: 4 per thread in fp64
+constexpr int kIpt4Min64 = 40960;  // above: 4 per thread in fp64
 
 enum { TENSOR_RPY = 0, TENSOR_OSEEN = 1 };
 enum { ACC_KAHAN = 0, ACC_PLAIN = 1 };
@@ -312,7 +313,7 @@ pairs_f32_kernel(const float4* __restrict__ rec, float4* __restrict__ part, cons
 
     const int tid = threadIdx.x;
     const int lane = tid & 31;
-    const int c = blockIdx.x;
+    const int c = sch.cta_piece[blockIdx.x];  // pieces of one SM's CTAs are consecutive (balance)
     const long long u_begin = sch.cta_u0[c];
     const long long u_end = sch.cta_u0[c + 1];
     const int n_units = static_cast<int>(u_end - u_begin);

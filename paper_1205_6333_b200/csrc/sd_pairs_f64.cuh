@@ -169,7 +169,7 @@ pairs_f64_kernel(const double4* __restrict__ rec, double4* __restrict__ part, co
 
     const int tid = threadIdx.x;
     const int lane = tid & 31;
-    const int c = blockIdx.x;
+    const int c = sch.cta_piece[blockIdx.x];  // pieces of one SM's CTAs are consecutive (balance)
     const long long u_begin = sch.cta_u0[c];
     const long long u_end = sch.cta_u0[c + 1];
     const int n_units = static_cast<int>(u_end - u_begin);
