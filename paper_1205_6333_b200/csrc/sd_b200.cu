@@ -893,7 +893,9 @@ sd_status sd_step(sd_ctx* ctx, void* pos, sd_force_fn fn, void* user, const void
     // The lubrication step is eight small launches: with it the loop is bound by the host's launch
     // rate (~100 us per step at any N), not by the GPU.  Constant-force runs are a fixed sequence of
     // launches, so kGraphSteps steps are captured once into a CUDA graph and replayed.
-    if (lub && !fn && !ctx->profiling && n_steps >= 2 * kGraphSteps) {
+    // The one-launch-per-product loop of small systems is launch-bound as well (6 us per step at
+    // N = 256 for a 3 us kernel) and is replayed the same way.
+    if ((lub || ctx->N <= ctx->small_apply_max) && !fn && !ctx->profiling && n_steps >= 2 * kGraphSteps) {
         GraphKey key;
         std::memset(&key, 0, sizeof(key));  // padding bytes take part in the memcmp below
         key.pos = pos;
@@ -904,7 +906,7 @@ sd_status sd_step(sd_ctx* ctx, void* pos, sd_force_fn fn, void* user, const void
         key.integrator = static_cast<int>(integrator);
         if (!ctx->gexec || std::memcmp(&key, &ctx->gkey, sizeof(GraphKey)) != 0) {
             drop_graph(ctx);
-            if ((s = ensure_lub_buffers(ctx)) != SD_OK) return s;
+            if (lub && (s = ensure_lub_buffers(ctx)) != SD_OK) return s;
             if (!ctx->cap_stream) SD_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->cap_stream, cudaStreamNonBlocking));
             const long long launches0 = ctx->launches;
             SD_CUDA(ctx, cudaStreamBeginCapture(ctx->cap_stream, cudaStreamCaptureModeThreadLocal));

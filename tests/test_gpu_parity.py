@@ -589,3 +589,30 @@ def test_plain_fp32_positions_round_every_step(gpu, n):
     assert np.array_equal(dp.cpu().numpy(), dq.cpu().numpy())
     ctx.close()
     ctx2.close()
+
+
+@pytest.mark.parametrize("prec_name,tol", [("PREC_F32_KAHAN", 2e-5), ("PREC_F64", 1e-10)])
+@pytest.mark.parametrize("n,integ,steps", [(70, "INT_EULER", 45), (300, "INT_MIDPOINT", 37),
+                                           (1200, "INT_EULER", 33)])
+def test_small_system_loop_replayed_from_a_cuda_graph(gpu, prec_name, tol, n, integ, steps):
+    """64 < N <= 2560 with constant forces and 32 steps or more: sd_step captures 16 steps of the
+    one-launch-per-product loop into a CUDA graph and replays it (Euler ping-pongs two position
+    buffers: an even number of steps per replay), then runs the odd tail directly."""
+    torch, sd = gpu
+    prec = getattr(sd, prec_name)
+    dtp = np_dtype(sd, prec)
+    pos = wl.uniform_cube(n, 0.05, wl.SEED_BASE + 950 + n)
+    force = wl.normal_forces(n, wl.SEED_BASE + 951 + n)
+    p, f = wl.to_xyzw(pos, dtp), wl.to_xyzw(force, dtp)
+    ctx = sd.Context(n, wl.A, wl.ETA)
+    ctx.set_precision(prec)
+    dp, df = torch.from_numpy(p).cuda(), torch.from_numpy(f).cuda()
+    oint = orc.INT_EULER if integ == "INT_EULER" else orc.INT_MIDPOINT
+    p64, f64 = p[:, :3].astype(np.float64), f[:, :3].astype(np.float64)
+    ctx.step(dp, 0.01, steps, getattr(sd, integ), force=df)
+    ctx.step(dp, 0.005, steps, getattr(sd, integ), force=df)      # new dt: new capture
+    torch.cuda.synchronize()
+    w1, _, _ = orc.step(p64, f64, wl.A, wl.ETA, 0.01, steps, oint)
+    w2, _, _ = orc.step(w1, f64, wl.A, wl.ETA, 0.005, steps, oint)
+    assert np.abs(dp.cpu().numpy()[:, :3].astype(np.float64) - w2).max() <= tol * wl.cube_side(n, 0.05)
+    ctx.close()
