@@ -41,6 +41,7 @@ struct Config {
 
 namespace {
 constexpr long long kGraphSteps = 16;  // even: the small-N Euler path ping-pongs two buffers
+constexpr long long kGraphMaxN = 32768; // below: the gaps between launches are a measurable share of a step
 struct GraphKey {  // everything a captured step sequence has baked in (besides the context state)
     void* pos;
     const void* force;
@@ -198,7 +199,7 @@ sd_status configure(sd_ctx* c) {
         // particles per thread: 8 once there is enough work to balance 2048-particle i-blocks
         // over the SMs (more operand reuse per j record), 4 and 2 below that (measured
         // crossovers, profiles/r01d_sweep.md).  N <= small_apply_max never reaches this kernel.
-        int i2 = (c->N > sd::kIpt8Min) ? 4 : (c->N > sd::kIpt4Min ? 2 : 1);
+        int i2 = (c->N > sd::kIpt8Min) ? 4 : (c->N > (pbc ? sd::kIpt4MinBox : sd::kIpt4Min) ? 2 : 1);
         if (c->ipt_override) i2 = c->ipt_override / 2;
         cfg.ipt = 2 * i2;
         cfg.TJ = (i2 == 1) ? sd::kTJSmall : sd::kTJ;
@@ -895,7 +896,7 @@ sd_status sd_step(sd_ctx* ctx, void* pos, sd_force_fn fn, void* user, const void
     // launches, so kGraphSteps steps are captured once into a CUDA graph and replayed.
     // The one-launch-per-product loop of small systems is launch-bound as well (6 us per step at
     // N = 256 for a 3 us kernel) and is replayed the same way.
-    if ((lub || ctx->N <= ctx->small_apply_max) && !fn && !ctx->profiling && n_steps >= 2 * kGraphSteps) {
+    if ((lub || ctx->N <= kGraphMaxN) && !fn && !ctx->profiling && n_steps >= 2 * kGraphSteps) {
         GraphKey key;
         std::memset(&key, 0, sizeof(key));  // padding bytes take part in the memcmp below
         key.pos = pos;

@@ -46,6 +46,7 @@ constexpr int kChunk = 32;   // j per compensation chunk
 constexpr int kUnrollJ = SD_UNROLL_J;  // j per unrolled loop body
 // measured crossovers of the particles-per-thread variants (profiles/r01d_sweep.md)
 constexpr int kIpt4Min = 20480;    // above: 4 particles per thread in fp32
+constexpr int kIpt4MinBox = 14336; // same in the periodic box (29 instead of 20 instructions per step)
 constexpr int kIpt2Min64 = 12288;  // above: 2 particles per thread in fp64
 constexpr int kIpt8Min = 32768;    // above: 8 per thread in fp32
 constexpr int kIpt4Min64 = 40960;  // above: 4 per thread in fp64
