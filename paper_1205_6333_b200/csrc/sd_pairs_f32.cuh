@@ -33,9 +33,10 @@ namespace sd {
 constexpr int kThreads = 256;
 constexpr int kWarps = kThreads / 32;
 constexpr int kTJ = 128;     // j records per tile (4 KiB)
-// tile of the 2-particle-per-thread variant.  32-record tiles (finer work units at small N) were
-// measured: N = 6000 73.8 -> 57.8 us per product, N = 12000 157.7 -> 148.1, but N = 3000 29.0 -> 38.9
-// (four times the slots to reduce and barriers to cross); kept at 128.
+// tile of the 2-particle-per-thread variant.  32-record tiles (four times the work units) were
+// measured twice.  With the SM-balanced piece map: per product 3-10 % faster for 4500 <= N <= 11000
+// (N = 6000: 61.6 -> 55.4 us), equal at 4000 and 12288, 20 % SLOWER at N <= 3000 (30.8 -> 36.9 us:
+// four times the slots to reduce, a tile hand-over every 32 j); kept at 128.
 constexpr int kTJSmall = 128;
 constexpr int kStages = 4;   // ring depth
 constexpr int kPrefetch = 2; // tiles in flight ahead of the one being consumed
