@@ -616,3 +616,18 @@ def test_small_system_loop_replayed_from_a_cuda_graph(gpu, prec_name, tol, n, in
     w2, _, _ = orc.step(w1, f64, wl.A, wl.ETA, 0.005, steps, oint)
     assert np.abs(dp.cpu().numpy()[:, :3].astype(np.float64) - w2).max() <= tol * wl.cube_side(n, 0.05)
     ctx.close()
+
+
+def test_four_million_particles_sampled_rows(gpu):
+    """Largest size exercised: N = 4,194,304 (1.76e13 pairs, 2048 i-blocks x 32768 j-tiles), fp32-
+    Kahan, 512 seeded rows + the first and last row against the oracle.  Checks the 64-bit unit
+    arithmetic of the schedule and the partial-sum buffers beyond the L2-resident sizes."""
+    torch, sd = gpu
+    n = 4 * 1048576
+    pos = wl.uniform_cube(n, 0.01, wl.SEED_BASE + 990)
+    force = wl.normal_forces(n, wl.SEED_BASE + 991)
+    got, p, f = gpu_apply(torch, sd, pos, force, sd.PREC_F32_KAHAN, sd.TENSOR_RPY)
+    rows = np.unique(np.concatenate([wl.row_subset(n, 512, wl.SEED_BASE + 992), [0, n - 1]]))
+    want = orc.apply_rows(p, f, rows, wl.A, wl.ETA, orc.TENSOR_RPY)
+    assert rel_err(got[rows], want) <= TOL_F32
+    assert np.all(np.isfinite(got))
