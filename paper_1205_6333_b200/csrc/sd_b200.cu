@@ -127,19 +127,18 @@ sd_status fail(sd_ctx* ctx, sd_status code, const std::string& msg) {
                         std::string(#call) + ": " + cudaGetErrorString(e_));               \
     } while (0)
 
-template <int I2, int TENSOR, int ACC, bool PBC>
-const void* f32_kernel() {  // the 2-particle-per-thread variant works on 32-record tiles
-    return reinterpret_cast<const void*>(
-        &sd::pairs_f32_kernel<I2, TENSOR, ACC, PBC, sd::STAGE_BULK, (I2 == 1) ? sd::kTJSmall : sd::kTJ>);
+template <int I2, int TENSOR, int ACC, bool PBC, int TJ = sd::kTJ>
+const void* f32_kernel() {
+    return reinterpret_cast<const void*>(&sd::pairs_f32_kernel<I2, TENSOR, ACC, PBC, sd::STAGE_BULK, TJ>);
 }
 template <int I, int TENSOR, bool PBC>
 const void* f64_kernel() {
     return reinterpret_cast<const void*>(&sd::pairs_f64_kernel<I, TENSOR, PBC>);
 }
-template <int I2, bool PBC>
+template <int I2, bool PBC, int TJ = sd::kTJ>
 const void* f32_pick(bool rpy, bool plain) {
-    return rpy ? (plain ? f32_kernel<I2, 0, 1, PBC>() : f32_kernel<I2, 0, 0, PBC>())
-               : (plain ? f32_kernel<I2, 1, 1, PBC>() : f32_kernel<I2, 1, 0, PBC>());
+    return rpy ? (plain ? f32_kernel<I2, 0, 1, PBC, TJ>() : f32_kernel<I2, 0, 0, PBC, TJ>())
+               : (plain ? f32_kernel<I2, 1, 1, PBC, TJ>() : f32_kernel<I2, 1, 0, PBC, TJ>());
 }
 template <int I, bool PBC>
 const void* f64_pick(bool rpy) {
@@ -202,7 +201,10 @@ sd_status configure(sd_ctx* c) {
         int i2 = (c->N > sd::kIpt8Min) ? 4 : (c->N > (pbc ? sd::kIpt4MinBox : sd::kIpt4Min) ? 2 : 1);
         if (c->ipt_override) i2 = c->ipt_override / 2;
         cfg.ipt = 2 * i2;
-        cfg.TJ = (i2 == 1) ? sd::kTJSmall : sd::kTJ;
+        // 2 particles per thread: 32-record tiles once there are enough of them to pay for the extra
+        // slots and hand-overs (four times the work units: finer balance over 444 CTAs)
+        const bool small_tiles = i2 == 1 && c->N >= sd::kTJSmallMinN && c->N <= sd::kTJSmallMaxN;
+        cfg.TJ = small_tiles ? sd::kTJSmall : sd::kTJ;
         static const char* names[3][2][2][2] = {
             {{{"pairs_f32x2_i2_rpy_kahan", "pairs_f32x2_i2_rpy_kahan_pbc"},
               {"pairs_f32x2_i2_rpy_plain", "pairs_f32x2_i2_rpy_plain_pbc"}},
@@ -221,6 +223,8 @@ sd_status configure(sd_ctx* c) {
             cfg.kernel = pbc ? f32_pick<4, true>(rpy, plain) : f32_pick<4, false>(rpy, plain);
         else if (i2 == 2)
             cfg.kernel = pbc ? f32_pick<2, true>(rpy, plain) : f32_pick<2, false>(rpy, plain);
+        else if (small_tiles)
+            cfg.kernel = pbc ? f32_pick<1, true, sd::kTJSmall>(rpy, plain) : f32_pick<1, false, sd::kTJSmall>(rpy, plain);
         else
             cfg.kernel = pbc ? f32_pick<1, true>(rpy, plain) : f32_pick<1, false>(rpy, plain);
         if (c->staging != sd::STAGE_BULK) {  // ablation variants: RPY, Kahan, free space only
@@ -228,12 +232,14 @@ sd_status configure(sd_ctx* c) {
                 return fail(c, SD_ERR_UNSUPPORTED,
                             "staging ablation exists for RPY, fp32-Kahan, free space only: call sd_set_staging(ctx, 0) first");
             const bool naive = c->staging == sd::STAGE_NAIVE;
-#define SD_STAGED(I2V)                                                                              \
-    (naive ? reinterpret_cast<const void*>(                                                         \
-                 &sd::pairs_f32_kernel<I2V, 0, 0, false, sd::STAGE_NAIVE, (I2V == 1) ? sd::kTJSmall : sd::kTJ>) \
-           : reinterpret_cast<const void*>(                                                         \
-                 &sd::pairs_f32_kernel<I2V, 0, 0, false, sd::STAGE_SYNC, (I2V == 1) ? sd::kTJSmall : sd::kTJ>))
-            cfg.kernel = (i2 == 4) ? SD_STAGED(4) : ((i2 == 2) ? SD_STAGED(2) : SD_STAGED(1));
+#define SD_STAGED_T(I2V, TJV)                                                                       \
+    (naive ? reinterpret_cast<const void*>(&sd::pairs_f32_kernel<I2V, 0, 0, false, sd::STAGE_NAIVE, TJV>) \
+           : reinterpret_cast<const void*>(&sd::pairs_f32_kernel<I2V, 0, 0, false, sd::STAGE_SYNC, TJV>))
+#define SD_STAGED(I2V) SD_STAGED_T(I2V, sd::kTJ)
+            cfg.kernel = (i2 == 4) ? SD_STAGED(4)
+                                   : ((i2 == 2) ? SD_STAGED(2)
+                                                : (small_tiles ? SD_STAGED_T(1, sd::kTJSmall) : SD_STAGED(1)));
+#undef SD_STAGED_T
 #undef SD_STAGED
             static const char* snames[2][3] = {
                 {"pairs_f32x2_i2_rpy_kahan_naive", "pairs_f32x2_i4_rpy_kahan_naive", "pairs_f32x2_i8_rpy_kahan_naive"},

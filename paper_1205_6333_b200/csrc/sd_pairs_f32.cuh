@@ -33,11 +33,14 @@ namespace sd {
 constexpr int kThreads = 256;
 constexpr int kWarps = kThreads / 32;
 constexpr int kTJ = 128;     // j records per tile (4 KiB)
-// tile of the 2-particle-per-thread variant.  32-record tiles (four times the work units) were
-// measured twice.  With the SM-balanced piece map: per product 3-10 % faster for 4500 <= N <= 11000
-// (N = 6000: 61.6 -> 55.4 us), equal at 4000 and 12288, 20 % SLOWER at N <= 3000 (30.8 -> 36.9 us:
-// four times the slots to reduce, a tile hand-over every 32 j); kept at 128.
-constexpr int kTJSmall = 128;
+// Second tile size of the 2-particle-per-thread variant: 32 records, i.e. four times the work
+// units, for a finer balance over the 444 resident CTAs.  Measured per product with the SM-balanced
+// piece map against 128-record tiles: 3-10 % faster for 4500 <= N <= 11000 (N = 6000: 61.6 -> 55.4
+// us), equal at 4000 and 12288, 20 % slower at N <= 3000 (30.8 -> 36.9 us: four times the slots to
+// reduce, a tile hand-over every 32 j), 1.6 % slower at 14000.  Used for kTJSmallMinN <= N <= kTJSmallMaxN.
+constexpr int kTJSmall = 32;
+constexpr int kTJSmallMinN = 4300;
+constexpr int kTJSmallMaxN = 12288;
 constexpr int kStages = 4;   // ring depth
 constexpr int kPrefetch = 2; // tiles in flight ahead of the one being consumed
 constexpr int kChunk = 32;   // j per compensation chunk
