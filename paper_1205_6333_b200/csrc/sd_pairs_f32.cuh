@@ -48,7 +48,7 @@ constexpr int kChunk = 32;   // j per compensation chunk
 #define SD_UNROLL_J 4
 #endif
 constexpr int kUnrollJ = SD_UNROLL_J;  // j per unrolled loop body
-// measured crossovers of the particles-per-thread variants (profiles/r01d_sweep.md)
+// measured crossovers of the particles-per-thread variants (profiles/r01e_sweep.md)
 constexpr int kIpt4Min = 20480;    // above: 4 particles per thread in fp32
 constexpr int kIpt4MinBox = 14336; // same in the periodic box (29 instead of 20 instructions per step)
 constexpr int kIpt2Min64 = 12288;  // above: 2 particles per thread in fp64

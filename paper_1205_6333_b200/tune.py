@@ -6,7 +6,7 @@ For each N it forces, through sd_set_dispatch, the one-launch warp-per-particle 
 and the tiled packed kernels with 2 / 4 / 8 particles per thread (fp64: 1 / 2 / 4), and times
 sd_mobility_apply and one Euler step of sd_step (CUDA events, warm caches, mean of many launches).
 The defaults compiled into the library (kSmallApplyMax, kIpt4Min, kIpt8Min, kIpt4Min64) are the
-crossovers this prints on a B200 (profiles/r01d_sweep.md).  Needs a GPU; argument marshalling and
+crossovers this prints on a B200 (profiles/r01e_sweep.md).  Needs a GPU; argument marshalling and
 timing only.
 """
 from __future__ import annotations
