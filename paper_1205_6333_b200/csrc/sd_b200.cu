@@ -592,6 +592,22 @@ sd_status launch_lubrication(sd_ctx* c, const void* pos, const void* vel, const 
             return fail(c, SD_ERR_UNSUPPORTED, "lubrication in a periodic box needs a box side of at least 9 a");
         grid.nc = std::min(grid.nc, 1024);
     }
+    if (n <= sd::kLubSmallMax) {  // small systems: all pairs in one launch, no cell grid
+        const double gx = g ? g[0] : 0.0, gy = g ? g[1] : 0.0, gz = g ? g[2] : 0.0;
+        const int blocks = (n + 7) / 8;
+        grid.mask = 0;
+        if (c->precision == SD_PREC_F64)
+            sd::lub_small_kernel<double4><<<blocks, 256, 0, st>>>(
+                static_cast<const double4*>(pos), static_cast<const double4*>(vel),
+                static_cast<const double4*>(fext), gx, gy, gz, static_cast<double4*>(force_out), grid, c->a,
+                c->mu0, n);
+        else
+            sd::lub_small_kernel<float4><<<blocks, 256, 0, st>>>(
+                static_cast<const float4*>(pos), static_cast<const float4*>(vel),
+                static_cast<const float4*>(fext), gx, gy, gz, static_cast<float4*>(force_out), grid, c->a,
+                c->mu0, n);
+        return check_launch(c, "lub_small_kernel");
+    }
     {
         sd_status a = ensure_lub_buffers(c);
         if (a != SD_OK) return a;

@@ -249,4 +249,63 @@ lub_force_kernel(const T4* __restrict__ spos, const T4* __restrict__ svel, const
     force_out[i] = Vec4<T4>::make(S(fx - cx), S(fy - cy), S(fz - cz), S(0));
 }
 
+// ---- small systems: all pairs in one launch ---------------------------------------------------
+// Below a few thousand particles the seven launches of the cell grid cost more (~22 us even when
+// replayed from a graph) than testing every pair: one warp per particle i, lane l takes
+// j = l, l + 32, ...; same decision rule, same fp64 pair term, lane sums combined by shuffles in a
+// fixed order.  N <= kLubSmallMax.
+constexpr int kLubSmallMax = 2560;
+
+template <typename T4>
+__global__ void __launch_bounds__(256)
+lub_small_kernel(const T4* __restrict__ pos, const T4* __restrict__ vel, const T4* fext,
+                 const double gx, const double gy, const double gz, T4* force_out,
+                 const LubGrid g, const double a, const double mu0, const int N) {
+    typedef typename Vec4<T4>::S S;
+    const int lane = threadIdx.x & 31;
+    const int i = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (i >= N) return;  // whole warps leave together
+    const T4 pi = pos[i];
+    const T4 vi = vel[i];
+    const double nine_a2 = 9.0 * a * a, inv_a = 1.0 / a, inv_mu0 = 1.0 / mu0;
+    double cx = 0.0, cy = 0.0, cz = 0.0;
+    for (int j = lane; j < N; j += 32) {
+        if (j == i) continue;
+        const T4 pj = pos[j];
+        if (sizeof(S) == 4 && lub_reject_f32(pi, pj, g, static_cast<float>(nine_a2))) continue;
+        const double dx = lub_disp<S>(pi.x, pj.x, g), dy = lub_disp<S>(pi.y, pj.y, g),
+                     dz = lub_disp<S>(pi.z, pj.z, g);
+        if (!lub_inside(S(0), dx, dy, dz, nine_a2)) continue;
+        const double r2 = dx * dx + dy * dy + dz * dz;
+        if (r2 == 0.0) continue;
+        const double r = sqrt(r2);
+        double s = r * inv_a - 2.0;
+        s = s < kLubSmin ? kLubSmin : s;
+        const double ls = log(s);
+        const double par = (0.25 / s - 0.225 * ls) * inv_mu0;
+        const double per = (-ls * (1.0 / 6.0)) * inv_mu0;
+        const T4 vj = vel[j];
+        const double wx = static_cast<double>(vi.x) - static_cast<double>(vj.x);
+        const double wy = static_cast<double>(vi.y) - static_cast<double>(vj.y);
+        const double wz = static_cast<double>(vi.z) - static_cast<double>(vj.z);
+        const double rw = (dx * wx + dy * wy + dz * wz) / r2;
+        cx += per * wx + (par - per) * rw * dx;
+        cy += per * wy + (par - per) * rw * dy;
+        cz += per * wz + (par - per) * rw * dz;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        cx += __shfl_xor_sync(0xffffffffu, cx, o);
+        cy += __shfl_xor_sync(0xffffffffu, cy, o);
+        cz += __shfl_xor_sync(0xffffffffu, cz, o);
+    }
+    if (lane != 0) return;
+    double fx = gx, fy = gy, fz = gz;
+    if (fext) {
+        const T4 f = fext[i];
+        fx = f.x, fy = f.y, fz = f.z;
+    }
+    force_out[i] = Vec4<T4>::make(S(fx - cx), S(fy - cy), S(fz - cz), S(0));
+}
+
 }  // namespace sd
