@@ -78,6 +78,19 @@ sd_status sd_create(sd_ctx** out, long long N, double a, double eta);
 sd_status sd_set_tensor(sd_ctx* ctx, sd_tensor tensor);
 sd_status sd_set_precision(sd_ctx* ctx, sd_precision precision);
 
+/* The static work schedule of the tiled kernels, as a pure host function (no GPU needed; the
+ * library builds its own schedules with the same code).  The (i-block, j-tile) units u = b T + t,
+ * B = ceil(N / particles_per_block) blocks x T = ceil(N / tile_j) tiles, are cut into
+ * G = min(B T, max_ctas) contiguous pieces of equal size +-1: piece g owns units
+ * [cta_u0[g], cta_u0[g+1]).  Block b collects the partial sums of pieces blk_first[b] ...
+ * blk_first[b] + blk_nslots[b] - 1.  CTA x works on piece cta_piece[x]; the CTAs x, x + num_sms,
+ * x + 2 num_sms, ... (which share an SM) own consecutive pieces.  dims receives {B, T, G,
+ * max slots per block}; the arrays (host; sizes G+1, G, B, B) may be NULL, call once with NULL
+ * arrays to learn the sizes. */
+sd_status sd_schedule_plan(long long N, int particles_per_block, int tile_j, long long max_ctas,
+                           int num_sms, long long* cta_u0, int* cta_piece, int* blk_first,
+                           int* blk_nslots, int* dims);
+
 /* Dispatch knobs of the small-N path (below a few thousand particles the device is
  * under-filled), for ablations and tests; the defaults are the measured crossovers.
  *   small_apply_max     : N up to which one product is ONE launch of the warp-per-particle kernel

@@ -176,6 +176,49 @@ void free_buffers(sd_ctx* c) {
     c->d_blk_first = c->d_blk_nslots = nullptr;
 }
 
+// Static schedule of the tiled kernels (pure host code; also exported as sd_schedule_plan so that
+// it can be tested without a GPU).  Units u = b * T + t over B i-blocks x T j-tiles; piece g of G
+// owns units [u0[g], u0[g+1]); block b collects the partial sums of pieces first[b] ...
+// first[b] + nslots[b] - 1; CTA blockIdx.x works on piece piece[blockIdx.x].
+struct HostSchedule {
+    int B = 0, T = 0, G = 0, max_slots = 1;
+    long long U = 0;
+    std::vector<long long> u0;
+    std::vector<int> first, nslots, piece;
+};
+
+HostSchedule build_schedule(long long N, int IB, int TJ, long long max_ctas, int nsm) {
+    HostSchedule h;
+    h.B = static_cast<int>((N + IB - 1) / IB);
+    h.T = static_cast<int>((N + TJ - 1) / TJ);
+    h.U = static_cast<long long>(h.B) * h.T;
+    h.G = static_cast<int>(std::min<long long>(h.U, max_ctas));
+    h.u0.resize(h.G + 1);
+    for (int g = 0; g <= h.G; ++g) h.u0[g] = static_cast<long long>((__int128)g * h.U / h.G);
+    h.first.resize(h.B);
+    h.nslots.resize(h.B);
+    for (int b = 0; b < h.B; ++b) {
+        const long long lo = static_cast<long long>(b) * h.T;
+        const long long hi = lo + h.T - 1;
+        const int cf = static_cast<int>(std::upper_bound(h.u0.begin(), h.u0.end(), lo) - h.u0.begin()) - 1;
+        const int cl = static_cast<int>(std::upper_bound(h.u0.begin(), h.u0.end(), hi) - h.u0.begin()) - 1;
+        h.first[b] = cf;
+        h.nslots[b] = cl - cf + 1;
+        h.max_slots = std::max(h.max_slots, h.nslots[b]);
+    }
+    // Pieces differ by one unit.  The CTAs of the first (and only) wave land on SM blockIdx % #SM,
+    // so CTA k, k + #SM, k + 2 #SM share an SM; when U / G resonates with #SM (N = 6000: U / G =
+    // 1.27, period 3.7 = 148 / 40) the long pieces of a plain blockIdx -> piece map pile up on the
+    // same SMs (6 units on some, 3 on others: 73.8 us instead of 57).  Giving the CTAs of one SM
+    // consecutive pieces balances the SMs to within one unit.
+    h.piece.resize(h.G);
+    std::vector<int> first_of_sm(nsm + 1, 0);
+    for (int sm = 0; sm < nsm; ++sm)
+        first_of_sm[sm + 1] = first_of_sm[sm] + h.G / nsm + (sm < h.G % nsm ? 1 : 0);
+    for (int b = 0; b < h.G; ++b) h.piece[b] = first_of_sm[b % nsm] + b / nsm;
+    return h;
+}
+
 // Pick the kernel variant for (N, precision, tensor), build the static schedule and
 // (re)allocate every scratch buffer.
 sd_status configure(sd_ctx* c) {
@@ -268,27 +311,13 @@ sd_status configure(sd_ctx* c) {
             cfg.kernel = pbc ? f64_pick<1, true>(rpy) : f64_pick<1, false>(rpy);
     }
     cfg.IB = sd::kThreads * cfg.ipt;
-    cfg.B = static_cast<int>((c->N + cfg.IB - 1) / cfg.IB);
-    cfg.T = static_cast<int>((c->N + cfg.TJ - 1) / cfg.TJ);
-    cfg.U = static_cast<long long>(cfg.B) * cfg.T;
     int occ = 0;
     SD_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, cfg.kernel, sd::kThreads, 0));
     if (occ < 1) return fail(c, SD_ERR_CUDA, "pair kernel does not fit on an SM");
-    cfg.G = static_cast<int>(std::min<long long>(cfg.U, static_cast<long long>(c->num_sms) * occ));
-
-    std::vector<long long> u0(cfg.G + 1);
-    for (int g = 0; g <= cfg.G; ++g) u0[g] = static_cast<long long>((__int128)g * cfg.U / cfg.G);
-    std::vector<int> first(cfg.B), nslots(cfg.B);
-    cfg.max_slots = 1;
-    for (int b = 0; b < cfg.B; ++b) {
-        const long long lo = static_cast<long long>(b) * cfg.T;
-        const long long hi = lo + cfg.T - 1;
-        const int cf = static_cast<int>(std::upper_bound(u0.begin(), u0.end(), lo) - u0.begin()) - 1;
-        const int cl = static_cast<int>(std::upper_bound(u0.begin(), u0.end(), hi) - u0.begin()) - 1;
-        first[b] = cf;
-        nslots[b] = cl - cf + 1;
-        cfg.max_slots = std::max(cfg.max_slots, nslots[b]);
-    }
+    const HostSchedule hs = build_schedule(c->N, cfg.IB, cfg.TJ, static_cast<long long>(c->num_sms) * occ, c->num_sms);
+    cfg.B = hs.B, cfg.T = hs.T, cfg.U = hs.U, cfg.G = hs.G, cfg.max_slots = hs.max_slots;
+    const std::vector<long long>& u0 = hs.u0;
+    const std::vector<int>&first = hs.first, &nslots = hs.nslots, &piece = hs.piece;
     c->cfg = cfg;
 
     const size_t es = elem_size(c->precision);
@@ -309,19 +338,6 @@ sd_status configure(sd_ctx* c) {
     SD_CUDA(c, cudaMalloc(&c->d_cta_u0, sizeof(long long) * (cfg.G + 1)));
     SD_CUDA(c, cudaMalloc(&c->d_blk_first, sizeof(int) * cfg.B));
     SD_CUDA(c, cudaMalloc(&c->d_blk_nslots, sizeof(int) * cfg.B));
-    // Pieces differ by one unit.  The CTAs of the first (and only) wave land on SM blockIdx % #SM,
-    // so CTA k, k + #SM, k + 2 #SM share an SM; when U / G resonates with #SM (N = 6000: U / G =
-    // 1.27, period 3.7 = 148 / 40) the long pieces of a plain blockIdx -> piece map pile up on the
-    // same SMs (6 units on some, 3 on others: 73.8 us instead of 57).  Giving the CTAs of one SM
-    // consecutive pieces balances the SMs to within one unit.
-    std::vector<int> piece(cfg.G);
-    {
-        const int nsm = c->num_sms;
-        std::vector<int> first_of_sm(nsm + 1, 0);
-        for (int sm = 0; sm < nsm; ++sm)
-            first_of_sm[sm + 1] = first_of_sm[sm] + cfg.G / nsm + (sm < cfg.G % nsm ? 1 : 0);
-        for (int b = 0; b < cfg.G; ++b) piece[b] = first_of_sm[b % nsm] + b / nsm;
-    }
     SD_CUDA(c, cudaMalloc(&c->d_cta_piece, sizeof(int) * cfg.G));
     SD_CUDA(c, cudaMemcpy(c->d_cta_piece, piece.data(), sizeof(int) * cfg.G, cudaMemcpyHostToDevice));
     SD_CUDA(c, cudaMemcpy(c->d_cta_u0, u0.data(), sizeof(long long) * (cfg.G + 1), cudaMemcpyHostToDevice));
@@ -729,6 +745,19 @@ sd_status sd_set_precision(sd_ctx* ctx, sd_precision precision) {
     cudaDeviceSynchronize();
     ctx->precision = precision;
     return configure(ctx);
+}
+
+sd_status sd_schedule_plan(long long N, int particles_per_block, int tile_j, long long max_ctas, int num_sms,
+                           long long* cta_u0, int* cta_piece, int* blk_first, int* blk_nslots, int* dims) {
+    if (N < 1 || particles_per_block < 1 || tile_j < 1 || max_ctas < 1 || num_sms < 1 || !dims)
+        return fail(nullptr, SD_ERR_INVALID_ARG, "sd_schedule_plan: invalid argument");
+    const HostSchedule h = build_schedule(N, particles_per_block, tile_j, max_ctas, num_sms);
+    dims[0] = h.B, dims[1] = h.T, dims[2] = h.G, dims[3] = h.max_slots;
+    if (cta_u0) std::copy(h.u0.begin(), h.u0.end(), cta_u0);
+    if (cta_piece) std::copy(h.piece.begin(), h.piece.end(), cta_piece);
+    if (blk_first) std::copy(h.first.begin(), h.first.end(), blk_first);
+    if (blk_nslots) std::copy(h.nslots.begin(), h.nslots.end(), blk_nslots);
+    return SD_OK;
 }
 
 sd_status sd_set_dispatch(sd_ctx* ctx, long long small_apply_max, int particles_per_thread) {

@@ -34,6 +34,8 @@ SYMBOLS = {
     "sd_create": (_I, [ctypes.POINTER(_P), _LL, _D, _D]),
     "sd_set_tensor": (_I, [_P, _I]),
     "sd_set_precision": (_I, [_P, _I]),
+    "sd_schedule_plan": (_I, [_LL, _I, _I, _LL, _I, ctypes.POINTER(_LL), ctypes.POINTER(_I),
+                               ctypes.POINTER(_I), ctypes.POINTER(_I), ctypes.POINTER(_I)]),
     "sd_set_dispatch": (_I, [_P, _LL, _I]),
     "sd_set_staging": (_I, [_P, _I]),
     "sd_set_box": (_I, [_P, _D]),
@@ -89,6 +91,27 @@ def _stream_ptr(stream):
     if stream is None:
         stream = torch.cuda.current_stream()
     return ctypes.c_void_p(stream.cuda_stream)
+
+
+def schedule_plan(n: int, particles_per_block: int, tile_j: int, max_ctas: int, num_sms: int):
+    """sd_schedule_plan: the static schedule of the tiled kernels (host only, no GPU).  Returns a
+    dict with B, T, G, max_slots and the arrays cta_u0, cta_piece, blk_first, blk_nslots."""
+    lib = load_library()
+    dims = (ctypes.c_int * 4)()
+    null_ll, null_i = ctypes.POINTER(_LL)(), ctypes.POINTER(_I)()
+    st = lib.sd_schedule_plan(n, particles_per_block, tile_j, max_ctas, num_sms, null_ll, null_i,
+                              null_i, null_i, dims)
+    if st != OK:
+        raise SdError(st, (lib.sd_last_error(None) or b"").decode())
+    B, T, G, ms = (int(x) for x in dims)
+    u0, piece = (ctypes.c_longlong * (G + 1))(), (ctypes.c_int * G)()
+    first, nslots = (ctypes.c_int * B)(), (ctypes.c_int * B)()
+    st = lib.sd_schedule_plan(n, particles_per_block, tile_j, max_ctas, num_sms, u0, piece, first,
+                              nslots, dims)
+    if st != OK:
+        raise SdError(st, (lib.sd_last_error(None) or b"").decode())
+    return {"B": B, "T": T, "G": G, "max_slots": ms, "cta_u0": list(u0), "cta_piece": list(piece),
+            "blk_first": list(first), "blk_nslots": list(nslots)}
 
 
 class Context:
