@@ -206,6 +206,20 @@ const char* sd_kernel_name(const sd_ctx* ctx);
 sd_status sd_fma_peak_probe(sd_ctx* ctx, sd_precision precision, double* tflops_out,
                             void* stream);
 
+/* The paper's Appendix A on this GPU: minimal O(N^2) memory-access kernels,
+ * N threads in blocks of 128, thread j accumulates N array elements (sum of the floats of every
+ * element it visits, starting from its own element in[j]) and stores the sum in out[j] (float).
+ *   elem_floats  1 (float) or 4 (float4)
+ *   pattern      0 linear k -> k, 1 strided k -> 131 k mod N, 2 unordered k -> (131 k + 32 j) mod N
+ *   scheme       0 naive (Alg. 3), 1 small-tiling (first warp stages 32 elements, Alg. 4),
+ *                2 tiling (the block stages 128 elements), 3 bulk asynchronous copies into a
+ *                shared-memory ring (linear pattern only; N % 4 == 0 for float)
+ * Runs one warm-up launch and `reps` timed launches on `stream`, waits for them and returns the
+ * mean time per launch.  in: device array of N elements (16-byte aligned), out: N floats.  No
+ * context is needed; errors are reported through sd_last_error(NULL). */
+sd_status sd_access_bench(int elem_floats, int pattern, int scheme, long long N, int reps,
+                          const void* in, void* out, double* ms_per_launch, void* stream);
+
 const char* sd_last_error(const sd_ctx* ctx);
 void sd_destroy(sd_ctx* ctx);
 

@@ -190,3 +190,47 @@ def num_threads() -> int:
 
 def set_num_threads(n: int) -> None:
     _load().sdo_set_num_threads(int(n))
+
+
+# ---- Appendix A access kernels (Algorithms 3 and 4) ---------------------------
+ACC_LINEAR, ACC_STRIDED, ACC_UNORDERED = 0, 1, 2
+ACC_NAIVE, ACC_SMALL_TILING, ACC_TILING, ACC_BULK = 0, 1, 2, 3
+_ACC_P, _ACC_M, _ACC_BLOCK = 131, 32, 128
+
+
+def _acc_map(k, j, n, pattern):
+    """The three mappings of PAPER.md:295: k -> k, k -> k p mod N, k -> (k p + j M) mod N."""
+    k = np.asarray(k, dtype=np.int64)
+    if pattern == ACC_LINEAR:
+        return k + 0 * np.asarray(j, dtype=np.int64)
+    if pattern == ACC_STRIDED:
+        return (k * _ACC_P) % n + 0 * np.asarray(j, dtype=np.int64)
+    return (k * _ACC_P + np.asarray(j, dtype=np.int64) * _ACC_M) % n
+
+
+def access_sums(data, pattern: int, scheme: int) -> np.ndarray:
+    """What thread j of the Appendix-A kernels stores: its own element plus the N elements it
+    visits, an element counting as the sum of its floats.  data: [N] or [N, 4].  Naive (Alg. 3):
+    the elements map(k, j).  Tiled schemes (Alg. 4; W = 32 small-tiling, 128 tiling; blocks of
+    128 threads): tile m holds, at place n, the element map(m + n, j_n) with j_n the global id of
+    the thread of the SAME block that copied it, and every thread of the block sums the whole
+    tile.  Bulk copies: linear pattern, same sums as naive.  Plain numpy, fp64 sums."""
+    data = np.asarray(data, dtype=np.float64)
+    val = data.sum(axis=1) if data.ndim == 2 else data
+    n = val.shape[0]
+    j = np.arange(n, dtype=np.int64)
+    out = val.copy()
+    if scheme in (ACC_NAIVE, ACC_BULK):
+        if scheme == ACC_BULK and pattern != ACC_LINEAR:
+            raise ValueError("bulk copies exist for the linear pattern only")
+        for k in range(n):
+            out += val[_acc_map(k, j, n, pattern)]
+        return out
+    w = 32 if scheme == ACC_SMALL_TILING else 128
+    for b0 in range(0, n, _ACC_BLOCK):            # one block of 128 threads
+        tile_sum = 0.0
+        for m in range(0, n, w):
+            nn = np.arange(min(w, n - m), dtype=np.int64)
+            tile_sum += val[_acc_map(m + nn, b0 + nn, n, pattern)].sum()
+        out[b0:b0 + _ACC_BLOCK] += tile_sum
+    return out

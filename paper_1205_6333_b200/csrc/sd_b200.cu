@@ -18,6 +18,7 @@
 #include "sd_common.cuh"
 #include "sd_pairs_f32.cuh"
 #include "sd_pairs_f64.cuh"
+#include "sd_access.cuh"
 #include "sd_lub.cuh"
 #include "sd_small.cuh"
 #include "sd_stream.cuh"
@@ -671,6 +672,25 @@ sd_status launch_lubrication(sd_ctx* c, const void* pos, const void* vel, const 
 #undef SD_LUB
 }
 
+template <typename T, int PATTERN>
+void access_launch(int scheme, float* out, const T* in, unsigned N, cudaStream_t st) {
+    const unsigned blocks = (N + sd::kAccThreads - 1) / sd::kAccThreads;
+    if (scheme == sd::ACC_NAIVE)
+        sd::access_naive_kernel<T, PATTERN><<<blocks, sd::kAccThreads, 0, st>>>(out, in, N);
+    else if (scheme == sd::ACC_SMALL_TILING)
+        sd::access_tiled_kernel<T, PATTERN, 32><<<blocks, sd::kAccThreads, 0, st>>>(out, in, N);
+    else if (scheme == sd::ACC_TILING)
+        sd::access_tiled_kernel<T, PATTERN, 128><<<blocks, sd::kAccThreads, 0, st>>>(out, in, N);
+    else
+        sd::access_bulk_kernel<T><<<blocks, sd::kAccThreads, 0, st>>>(out, in, N);
+}
+template <typename T>
+void access_dispatch(int pattern, int scheme, float* out, const void* in, unsigned N, cudaStream_t st) {
+    const T* p = static_cast<const T*>(in);
+    if (pattern == sd::ACC_LINEAR) access_launch<T, sd::ACC_LINEAR>(scheme, out, p, N, st);
+    else if (pattern == sd::ACC_STRIDED) access_launch<T, sd::ACC_STRIDED>(scheme, out, p, N, st);
+    else access_launch<T, sd::ACC_UNORDERED>(scheme, out, p, N, st);
+}
 bool misaligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) & (a - 1)) != 0; }
 
 }  // namespace
@@ -1099,6 +1119,40 @@ sd_status sd_fma_peak_probe(sd_ctx* ctx, sd_precision precision, double* tflops_
     SD_CUDA(ctx, cudaGetLastError());
     const double fmas = static_cast<double>(iters) * 64.0 * threads * blocks;
     *tflops_out = 2.0 * fmas / (best * 1e-3) / 1e12;
+    return SD_OK;
+}
+
+sd_status sd_access_bench(int elem_floats, int pattern, int scheme, long long N, int reps, const void* in,
+                          void* out, double* ms_per_launch, void* stream) {
+    if ((elem_floats != 1 && elem_floats != 4) || pattern < 0 || pattern > 2 || scheme < 0 || scheme > 3 ||
+        N < 1 || N > (1LL << 24) || reps < 1 || !in || !out)
+        return fail(nullptr, SD_ERR_INVALID_ARG, "sd_access_bench: invalid argument");
+    if (scheme == sd::ACC_BULK && (pattern != sd::ACC_LINEAR || (elem_floats == 1 && N % 4 != 0)))
+        return fail(nullptr, SD_ERR_UNSUPPORTED,
+                    "sd_access_bench: bulk copies need the linear pattern (and N % 4 == 0 for float)");
+    if (misaligned(in, 16)) return fail(nullptr, SD_ERR_INVALID_ARG, "sd_access_bench: in must be 16-byte aligned");
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const unsigned n = static_cast<unsigned>(N);
+    float* o = static_cast<float*>(out);
+    auto launch = [&]() {
+        if (elem_floats == 1) access_dispatch<float>(pattern, scheme, o, in, n, st);
+        else access_dispatch<float4>(pattern, scheme, o, in, n, st);
+    };
+    launch();  // warm-up (and the result the caller checks)
+    cudaEvent_t e0, e1;
+    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess)
+        return fail(nullptr, SD_ERR_CUDA, "sd_access_bench: cannot create events");
+    cudaEventRecord(e0, st);
+    for (int r = 0; r < reps; ++r) launch();
+    cudaEventRecord(e1, st);
+    cudaError_t e = cudaEventSynchronize(e1);
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0, e1);
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    if (e != cudaSuccess || (e = cudaGetLastError()) != cudaSuccess)
+        return fail(nullptr, SD_ERR_CUDA, std::string("sd_access_bench: ") + cudaGetErrorString(e));
+    if (ms_per_launch) *ms_per_launch = static_cast<double>(ms) / reps;
     return SD_OK;
 }
 

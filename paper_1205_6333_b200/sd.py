@@ -56,6 +56,7 @@ SYMBOLS = {
     "sd_profile_enable": (_I, [_P, _I]),
     "sd_profile_read": (_I, [_P, ctypes.POINTER(_D), ctypes.POINTER(_LL)]),
     "sd_fma_peak_probe": (_I, [_P, _I, ctypes.POINTER(_D), _P]),
+    "sd_access_bench": (_I, [_I, _I, _I, _LL, _I, _P, _P, ctypes.POINTER(_D), _P]),
     "sd_last_error": (ctypes.c_char_p, [_P]),
     "sd_destroy": (None, [_P]),
 }
@@ -112,6 +113,20 @@ def schedule_plan(n: int, particles_per_block: int, tile_j: int, max_ctas: int, 
         raise SdError(st, (lib.sd_last_error(None) or b"").decode())
     return {"B": B, "T": T, "G": G, "max_slots": ms, "cta_u0": list(u0), "cta_piece": list(piece),
             "blk_first": list(first), "blk_nslots": list(nslots)}
+
+
+def access_bench(data, out, pattern: int, scheme: int, reps: int = 10, stream=None) -> float:
+    """sd_access_bench (Appendix A).  data: CUDA float32 tensor [N] or [N, 4]; out: CUDA
+    float32 tensor [N].  Returns the mean milliseconds per launch."""
+    lib = load_library()
+    elem = 4 if data.dim() == 2 else 1
+    ms = ctypes.c_double(0.0)
+    st = lib.sd_access_bench(elem, int(pattern), int(scheme), int(data.shape[0]), int(reps),
+                             ctypes.c_void_p(data.data_ptr()), ctypes.c_void_p(out.data_ptr()),
+                             ctypes.byref(ms), _stream_ptr(stream))
+    if st != OK:
+        raise SdError(st, (lib.sd_last_error(None) or b"").decode())
+    return ms.value
 
 
 class Context:
