@@ -327,9 +327,10 @@ sd_status configure(sd_ctx* c) {
     SD_CUDA(c, cudaMalloc(&c->rec, nrec * 2 * v4));
     const size_t part_per_slot = f64 ? nrec * v4 : nrec * 2 * v4;
     SD_CUDA(c, cudaMalloc(&c->part, part_per_slot * cfg.max_slots));
-    if (!c->vel) {
+    if (!c->vel) {  // "velocities of the previous step" start at zero (cold start of the lubrication loop)
         SD_CUDA(c, cudaMalloc(&c->vel, nrec * v4));
-            c->vel_bytes = nrec * v4;
+        SD_CUDA(c, cudaMemset(c->vel, 0, nrec * v4));
+        c->vel_bytes = nrec * v4;
     }
     SD_CUDA(c, cudaMalloc(&c->pos_lo, nrec * v4));
     SD_CUDA(c, cudaMalloc(&c->pos_half, nrec * v4));
@@ -517,9 +518,47 @@ sd_status launch_small_apply_t(sd_ctx* c, const void* posx, const void* force, c
     return check_launch(c, "small_apply_kernel");
 }
 
+// fp32 modes from kPackedMinN particles on: the packed variant (sd_small.cuh)
+template <int TENSOR, bool KAHAN, bool PBC>
+void launch_small_packed_k(sd_ctx* c, const void* posx, const void* force, const double g[3], void* vel,
+                           const void* pos_base, void* pos_out, double dt, int mode, cudaStream_t st) {
+    const int n = static_cast<int>(c->N);
+    const int per_cta = (sd::kPackedThreads / 32) * 2;
+    const int blocks = (n + per_cta - 1) / per_cta;
+    const double gx = g ? g[0] : 0.0, gy = g ? g[1] : 0.0, gz = g ? g[2] : 0.0;
+    const size_t smem = static_cast<size_t>(n) * 32;
+    static bool attr_set = false;  // once per instantiation: up to 80 KiB of dynamic shared memory
+    if (!attr_set) {
+        cudaFuncSetAttribute(sd::small_apply_packed_kernel<TENSOR, KAHAN, PBC>,
+                             cudaFuncAttributeMaxDynamicSharedMemorySize, sd::kPackedMaxN * 32);
+        attr_set = true;
+    }
+    sd::small_apply_packed_kernel<TENSOR, KAHAN, PBC><<<blocks, sd::kPackedThreads, smem, st>>>(
+        static_cast<const float4*>(posx), static_cast<const float4*>(force), gx, gy, gz,
+        static_cast<float4*>(vel), static_cast<const float4*>(pos_base), static_cast<float4*>(c->pos_lo),
+        static_cast<float4*>(pos_out), dt, mode, folded_coef<float>(c), c->mu0 * 0.75 * c->a, c->mu0, n,
+        c->pos_comp);
+}
+template <bool KAHAN>
+sd_status launch_small_packed(sd_ctx* c, const void* posx, const void* force, const double g[3], void* vel,
+                              const void* pos_base, void* pos_out, double dt, int mode, cudaStream_t st) {
+    const bool rpy = c->tensor == SD_TENSOR_RPY, pbc = c->box > 0.0;
+#define SD_PK(T, P) launch_small_packed_k<T, KAHAN, P>(c, posx, force, g, vel, pos_base, pos_out, dt, mode, st)
+    if (rpy) { if (pbc) SD_PK(0, true); else SD_PK(0, false); }
+    else { if (pbc) SD_PK(1, true); else SD_PK(1, false); }
+#undef SD_PK
+    return check_launch(c, "small_apply_packed_kernel");
+}
+
 sd_status launch_small_apply(sd_ctx* c, const void* posx, const void* force, const double g[3],
                              void* vel, const void* pos_base, void* pos_out, double dt, int mode,
                              cudaStream_t st) {
+    if (c->precision != SD_PREC_F64 && c->N >= sd::kPackedMinN && c->N <= sd::kPackedMaxN &&
+        c->N <= c->small_apply_max) {
+        if (c->precision == SD_PREC_F32_PLAIN)
+            return launch_small_packed<false>(c, posx, force, g, vel, pos_base, pos_out, dt, mode, st);
+        return launch_small_packed<true>(c, posx, force, g, vel, pos_base, pos_out, dt, mode, st);
+    }
     if (c->precision == SD_PREC_F64)
         return launch_small_apply_t<double4, false>(c, posx, force, g, vel, pos_base, pos_out, dt, mode, st);
     if (c->precision == SD_PREC_F32_PLAIN)
@@ -1063,7 +1102,9 @@ long long sd_launch_count(const sd_ctx* ctx) { return ctx ? ctx->launches : 0; }
 const char* sd_kernel_name(const sd_ctx* ctx) {
     if (!ctx) return "";
     if (ctx->N <= ctx->small_apply_max)
-        return ctx->precision == SD_PREC_F64 ? "small_apply_f64" : "small_apply_f32";
+        return ctx->precision == SD_PREC_F64
+                   ? "small_apply_f64"
+                   : ((ctx->N >= sd::kPackedMinN && ctx->N <= sd::kPackedMaxN) ? "small_apply_f32x2" : "small_apply_f32");
     return ctx->cfg.name;
 }
 

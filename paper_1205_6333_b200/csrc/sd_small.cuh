@@ -238,6 +238,127 @@ small_apply_kernel(const T4* __restrict__ posx, const T4* __restrict__ force, co
     }
 }
 
+// ---- one product per launch, fp32, packed arithmetic -------------------------------------------
+// Same mapping as small_apply_kernel (a warp owns two particles, its lanes split j, tiles staged
+// by the CTA, shuffle reduction, fused integrator update), but the pair arithmetic is the packed
+// "careful" body of the tiled kernel (sd_pairs_f32.cuh): the two particles of a warp are the two
+// halves of f32x2 registers, r^2 is clamped from below so that every pair -- self pair included --
+// adds a finite term, and the pairs below the clamp are put right one by one (clamped term out,
+// exact term in).  ~30 instead of ~110 instructions per two pairs.  Works in the folded units of
+// the tiled kernels on the caller's raw forces: the sum is multiplied by c1 = mu0 3a/4 at the end.
+// Compensation: plain adds over the (at most 4) terms a lane takes from a 128-record tile, Kahan
+// merge per 128 j.  CTAs of 128 threads = 8 particles: N / 8 CTAs; the CTA keeps all N records in
+// shared memory.
+constexpr int kPackedThreads = 128;
+// Measured window (graph-replayed Euler steps on the fcc benchmark, us per step, scalar -> packed):
+// N = 108 2.99 -> 3.37, 500 5.29 -> 6.05, 864 8.09 -> 7.56, 2048 17.96 -> 13.89; N = 2560 22.6 -> 30.8
+// per product (80 KiB of shared memory per CTA).  Below the window every CTA copying all N records
+// costs more than the arithmetic saves, above it the shared-memory footprint limits the CTAs per SM.
+constexpr int kPackedMinN = 768;
+constexpr int kPackedMaxN = 2304;
+constexpr int kPackedTile = 128;
+
+template <int TENSOR, bool KAHAN, bool PBC>
+__global__ void __launch_bounds__(kPackedThreads)
+small_apply_packed_kernel(const float4* __restrict__ posx, const float4* __restrict__ force,
+                          const double gx, const double gy, const double gz,
+                          float4* __restrict__ vel, const float4* __restrict__ pos_base,
+                          float4* __restrict__ pos_lo, float4* __restrict__ pos_out, const double dt,
+                          const int MODE, const PairCoef k, const double c1, const double mu0,
+                          const int N, const int pos_comp) {
+    // all N records (positions, then forces) in dynamic shared memory: 32 N bytes <= 80 KiB, one
+    // barrier per product instead of two per tile (at these sizes the kernel is latency, not
+    // arithmetic: 8 serial tile hand-overs cost more than the pairs)
+    extern __shared__ float4 s_all[];
+    float4* sp = s_all;
+    float4* sf = s_all + N;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int i0 = (blockIdx.x * (kPackedThreads / 32) + warp) * 2;
+    const int ia = min(i0, N - 1), ib = min(i0 + 1, N - 1);
+    for (int j = tid; j < N; j += kPackedThreads) {
+        sp[j] = posx[j];
+        sf[j] = force ? force[j] : make_float4(float(gx), float(gy), float(gz), 0.f);
+    }
+    __syncthreads();
+    const float4 pa = sp[ia], pb = sp[ib];
+    const f32x2 zero = bc2(0.f);
+    f32x2 xi[1] = {add2(pk2(pa.x, pb.x), zero)}, yi[1] = {add2(pk2(pa.y, pb.y), zero)},
+          zi[1] = {add2(pk2(pa.z, pb.z), zero)};
+    f32x2 sx = zero, sy = zero, sz = zero, cx = zero, cy = zero, cz = zero;
+    for (int j0 = 0; j0 < N; j0 += kPackedTile) {   // compensation chunk: <= 4 terms per lane
+        const int nj = min(j0 + kPackedTile, N);
+        f32x2 px[1] = {zero}, py[1] = {zero}, pz[1] = {zero};
+        for (int j = j0 + lane; j < nj; j += 32) {
+            const float4 pj = sp[j];
+            const float4 fj = sf[j];
+            float mn = 0.f, r2v[2];
+            pair_fast_staged<1, TENSOR, PBC, true>(xi, yi, zi, pj, fj, k, px, py, pz, mn, r2v);
+            if (fminf(r2v[0], r2v[1]) < k.clampv) {
+                float ax = lo2(px[0]), ay = lo2(py[0]), az = lo2(pz[0]);
+                float bx = hi2(px[0]), by = hi2(py[0]), bz = hi2(pz[0]);
+                if (r2v[0] < k.clampv) {
+                    pair_clamped_sub<TENSOR, PBC>(pa.x, pa.y, pa.z, pj, fj, k, ax, ay, az);
+                    pair_exact<TENSOR, PBC>(pa.x, pa.y, pa.z, j == ia, pj, fj, k, ax, ay, az);
+                }
+                if (r2v[1] < k.clampv) {
+                    pair_clamped_sub<TENSOR, PBC>(pb.x, pb.y, pb.z, pj, fj, k, bx, by, bz);
+                    pair_exact<TENSOR, PBC>(pb.x, pb.y, pb.z, j == ib, pj, fj, k, bx, by, bz);
+                }
+                px[0] = pk2(ax, bx);
+                py[0] = pk2(ay, by);
+                pz[0] = pk2(az, bz);
+            }
+        }
+        if (KAHAN) {
+            kahan_merge2(sx, cx, px[0]);
+            kahan_merge2(sy, cy, py[0]);
+            kahan_merge2(sz, cz, pz[0]);
+        } else {
+            sx = add2(sx, px[0]);
+            sy = add2(sy, py[0]);
+            sz = add2(sz, pz[0]);
+        }
+    }
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+        const int i = i0 + h;
+        const float hx = h ? hi2(sx) : lo2(sx), hy = h ? hi2(sy) : lo2(sy), hz = h ? hi2(sz) : lo2(sz);
+        const float lx = h ? hi2(cx) : lo2(cx), ly = h ? hi2(cy) : lo2(cy), lz = h ? hi2(cz) : lo2(cz);
+        float4 fi = make_float4(float(gx), float(gy), float(gz), 0.f);
+        if (force) fi = sf[min(i, N - 1)];
+        double vx, vy, vz;
+        if (KAHAN) {
+            vx = lanes_sum<32>(double(hx) - double(lx)) * c1 + mu0 * double(fi.x);
+            vy = lanes_sum<32>(double(hy) - double(ly)) * c1 + mu0 * double(fi.y);
+            vz = lanes_sum<32>(double(hz) - double(lz)) * c1 + mu0 * double(fi.z);
+        } else {  // SD_PREC_F32_PLAIN: fp32 end to end
+            const float cf = float(c1), mf = float(mu0);
+            vx = fmaf(mf, fi.x, cf * lanes_sum_f32<32>(hx));
+            vy = fmaf(mf, fi.y, cf * lanes_sum_f32<32>(hy));
+            vz = fmaf(mf, fi.z, cf * lanes_sum_f32<32>(hz));
+        }
+        if (lane == 0 && i < N) {
+            vel[i] = make_float4(float(vx), float(vy), float(vz), 0.f);
+            if (MODE != FIN_VEL) {
+                const float4 ph = pos_base[i];
+                double X = ph.x, Y = ph.y, Z = ph.z;
+                if (pos_comp) {
+                    const float4 pl = pos_lo[i];
+                    X += pl.x, Y += pl.y, Z += pl.z;
+                }
+                const double hh = (MODE == FIN_HALF) ? 0.5 * dt : dt;
+                X += hh * vx, Y += hh * vy, Z += hh * vz;
+                const float xh = float(X), yh = float(Y), zh = float(Z);
+                pos_out[i] = make_float4(xh, yh, zh, 0.f);
+                if (MODE != FIN_HALF)
+                    pos_lo[i] = pos_comp ? make_float4(float(X - double(xh)), float(Y - double(yh)),
+                                                       float(Z - double(zh)), 0.f)
+                                         : make_float4(0.f, 0.f, 0.f, 0.f);
+            }
+        }
+    }
+}
+
 // ---- all steps in one launch ------------------------------------------------------------------
 // One CTA of N * SUB threads (SUB lanes per particle, SUB | 32).  Positions live in shared memory
 // as doubles (= hi + lo of the fp32 modes); the pair arithmetic runs in S on S-rounded positions,

@@ -204,3 +204,26 @@ def test_graph_replay_follows_changes_of_arguments_and_settings(gpu):
                           orc.INT_EULER, box=L, image=orc.IMAGE_F64)
     assert np.abs(dq.cpu().numpy()[:, :3] - want).max() <= 1e-9
     ctx.close()
+
+
+def test_previous_velocities_start_at_zero_in_recycled_memory(gpu):
+    """Regression: the context-owned velocities ("of the previous step", reading C4) must be zero
+    after sd_create even when cudaMalloc hands back the block a closed context left full of
+    velocities (a missing memset showed up as order-dependent failures of the tests above)."""
+    torch, sd = gpu
+    n = 700
+    pos = wl.rsa_cube(n, 0.25, wl.SEED_BASE + 333, a=1.3)
+    p = wl.to_xyzw(pos, np.float32)
+    for cycle in range(4):
+        ctx = sd.Context(n, wl.A, wl.ETA)
+        dv = torch.full((n, 4), float("nan"), device="cuda")
+        ctx.get_velocity(dv)
+        torch.cuda.synchronize()
+        assert np.all(dv.cpu().numpy() == 0.0), f"cycle {cycle}"
+        ctx.set_lubrication(True)
+        dp = torch.from_numpy(p).cuda()
+        ctx.step(dp, 0.01, 3, sd.INT_EULER, gravity=(0.0, 0.0, -1.0))   # leaves |v| ~ 10 behind
+        ctx.get_velocity(dv)
+        torch.cuda.synchronize()
+        assert np.abs(dv.cpu().numpy()).max() > 1.0
+        ctx.close()

@@ -672,3 +672,48 @@ def test_side_stream_and_two_contexts_give_the_same_bits(gpu):
     torch.cuda.synchronize()
     assert np.array_equal(base[0], got[0]) and np.array_equal(base[1], got[1])
     noise_ctx.close()
+
+
+@pytest.mark.parametrize("prec_name,tol", [("PREC_F32_KAHAN", TOL_F32), ("PREC_F32_PLAIN", 5e-5)])
+@pytest.mark.parametrize("tname", ["TENSOR_RPY", "TENSOR_OSEEN"])
+@pytest.mark.parametrize("boxed", [False, True])
+def test_packed_one_launch_kernel_window(gpu, prec_name, tol, tname, boxed):
+    """768 <= N <= 2304 in the fp32 modes runs small_apply_packed_kernel (two particles of a warp as
+    the halves of packed registers, clamped body + per-pair corrections, all records in shared
+    memory).  Dense clouds (phi = 0.2: overlaps in most rows, one pair of coincident centres), both
+    ends of the window and an odd N, all rows; then one step against the oracle."""
+    torch, sd = gpu
+    prec, tensor = getattr(sd, prec_name), getattr(sd, tname)
+    otensor = orc.TENSOR_RPY if tname == "TENSOR_RPY" else orc.TENSOR_OSEEN
+    for n in (768, 1001, 2304):
+        L = wl.cube_side(n, 0.2)
+        pos = wl.uniform_cube(n, 0.2, wl.SEED_BASE + 1040 + n)
+        pos[n // 2] = pos[3]
+        force = wl.normal_forces(n, wl.SEED_BASE + 1041 + n)
+        p, f = wl.to_xyzw(pos, np.float32), wl.to_xyzw(force, np.float32)
+        ctx = sd.Context(n, wl.A, wl.ETA)
+        ctx.set_precision(prec)
+        ctx.set_tensor(tensor)
+        if boxed:
+            ctx.set_box(L)
+        assert ctx.kernel_name == "small_apply_f32x2"
+        dp, df = torch.from_numpy(p).cuda(), torch.from_numpy(f).cuda()
+        dv = torch.full_like(dp, float("nan"))
+        ctx.mobility_apply(dp, df, dv)
+        torch.cuda.synchronize()
+        p64, f64 = p[:, :3].astype(np.float64), f[:, :3].astype(np.float64)
+        box = float(np.float32(L)) if boxed else 0.0
+        want = orc.apply(p64, f64, wl.A, wl.ETA, otensor, box=box, image=orc.IMAGE_F32)
+        assert rel_err(dv.cpu().numpy()[:, :3].astype(np.float64), want) <= tol
+        # midpoint for Rotne-Prager; Euler for Oseen: its 1/r terms of overlapping pairs amplify the
+        # fp32 rounding of the half-step positions (ulp(x) / r_min ~ 2e-5) beyond any fixed bound
+        gi, oi = ((sd.INT_MIDPOINT, orc.INT_MIDPOINT) if tname == "TENSOR_RPY"
+                  else (sd.INT_EULER, orc.INT_EULER))
+        ctx.step(dp, 0.01, 1, gi, force=df)
+        torch.cuda.synchronize()
+        wp, wv, _ = orc.step(p64, f64, wl.A, wl.ETA, 0.01, 1, oi, otensor, box=box, image=orc.IMAGE_F32)
+        # position error <= rounding of the stored word + dt x (velocity error <= tol |v|): the
+        # unregularised Oseen tensor gives overlapping spheres velocities of several hundred mu0 F
+        vmax = np.linalg.norm(wv, axis=1).max()
+        assert np.abs(dp.cpu().numpy()[:, :3] - wp).max() <= 2e-7 * L + 3 * tol * 0.01 * vmax
+        ctx.close()
