@@ -139,7 +139,11 @@ sd_status sd_mobility_apply_host(sd_ctx* ctx, const void* pos_host, const void* 
  * Positions are carried with a context-owned low word (double-single) in
  * the fp32 modes; it stays valid while the caller does not modify pos between calls (see
  * sd_reset_compensation).  After the call sd_get_velocity returns the velocities of the last
- * product evaluated (Euler: M(r_n)F; midpoint: M(r_h)F). */
+ * product evaluated (Euler: M(r_n)F; midpoint: M(r_h)F).
+ * Launch-bound loops (constant forces, no callback, 32 steps or more, N <= 32768 or the
+ * lubrication correction on) are enqueued as replays of a CUDA graph of 16 steps, captured once
+ * per (pos, force, gravity, dt, integrator) on a context-owned stream, plus a direct tail; the
+ * kernels and therefore the results are those of step-by-step launches. */
 sd_status sd_step(sd_ctx* ctx, void* pos, sd_force_fn fn, void* user, const void* force,
                   const double gravity[3], double dt, long long n_steps,
                   sd_integrator integrator, void* stream);
