@@ -95,6 +95,17 @@ def time_oracle(pos64, force64, wl, tensor, target_seconds, box=0.0, image=0):
     return len(sample) * n / t, cores, len(sample), t
 
 
+def cpu_model():
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.startswith("model name"):
+                    return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
 def run_reference(args, rank):
     """--impl reference: the oracle as it stands, on the host cores."""
     if rank != 0:
@@ -497,9 +508,16 @@ def main():
         f64 = h_force.numpy()[:, :3].astype(np.float64)
         rate, cores, rows, secs = time_oracle(p64, f64, wl, args.tensor, 15.0,
                                               box=float(np.float32(box_side(args, wl))))
+        from oracle import sd_oracle as _orc
+        _orc.set_num_threads(1)   # also the one-thread figure, on a 3 s sample
+        rate1, _, rows1, secs1 = time_oracle(p64, f64, wl, args.tensor, 3.0,
+                                             box=float(np.float32(box_side(args, wl))))
+        _orc.set_num_threads(cores)
         line["cpu_baseline"] = {"value": rate, "unit": "pairs/s", "cores": cores, "kind": "oracle",
                                 "sample": f"{rows} seeded rows x all {n} columns of the same "
-                                          f"workload, {secs:.1f} s"}
+                                          f"workload, {secs:.1f} s",
+                                "cpu_model": cpu_model(), "one_thread_value": rate1,
+                                "one_thread_sample": f"{rows1} rows, {secs1:.1f} s"}
     ctx.close()
     if rank == 0:
         print(json.dumps(line), flush=True)
