@@ -2,6 +2,7 @@
 
     python -m paper_1205_6333_b200.tune [f64] [box]
     python -m paper_1205_6333_b200.tune cfg5        (the reporting sweep)
+    python -m paper_1205_6333_b200.tune one N IPT   (4 products at one size, for ncu)
 
 For each N it forces, through sd_set_dispatch, the one-launch warp-per-particle kernel ("small")
 and the tiled packed kernels with 2 / 4 / 8 particles per thread (fp64: 1 / 2 / 4), and times
@@ -102,6 +103,17 @@ def main(argv):
     torch.cuda.set_device(0)
     if "cfg5" in argv:
         return cfg5(torch, sd, wl)
+    if argv and argv[0] == "one":
+        n, ipt = int(argv[1]), int(argv[2])
+        pos, force = wl.sweep(n)
+        dp = torch.from_numpy(wl.to_xyzw(pos, np.float32)).cuda()
+        df = torch.from_numpy(wl.to_xyzw(force, np.float32)).cuda()
+        dv = torch.empty_like(dp)
+        ctx = sd.Context(n, wl.A, wl.ETA)
+        ctx.set_dispatch(-1 if ipt == 0 else 0, ipt)
+        print(n, ctx.kernel_name, _time(torch, lambda: ctx.mobility_apply(dp, df, dv), 1) * 1e6, "us")
+        ctx.close()
+        return None
     f64, box = "f64" in argv, "box" in argv
     prec, npdt = (sd.PREC_F64, np.float64) if f64 else (sd.PREC_F32_KAHAN, np.float32)
     print(f"| N | apply us: small | i2 | i4 | i8 | auto | step us: small | i2 | i4 | i8 | auto | auto kernel "
