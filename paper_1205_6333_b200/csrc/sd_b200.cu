@@ -242,7 +242,7 @@ sd_status configure(sd_ctx* c) {
         // particles per thread: 8 once there is enough work to balance 2048-particle i-blocks
         // over the SMs (more operand reuse per j record), 4 and 2 below that (measured
         // crossovers, profiles/r01e_sweep.md).  N <= small_apply_max never reaches this kernel.
-        int i2 = (c->N > sd::kIpt8Min) ? 4 : (c->N > (pbc ? sd::kIpt4MinBox : sd::kIpt4Min) ? 2 : 1);
+        int i2 = (c->N > (pbc ? sd::kIpt8MinBox : sd::kIpt8Min)) ? 4 : (c->N > (pbc ? sd::kIpt4MinBox : sd::kIpt4Min) ? 2 : 1);
         if (c->ipt_override) i2 = c->ipt_override / 2;
         cfg.ipt = 2 * i2;
         // 2 particles per thread: 32-record tiles once there are enough of them to pay for the extra

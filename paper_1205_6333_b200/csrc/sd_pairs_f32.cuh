@@ -52,7 +52,8 @@ constexpr int kUnrollJ = SD_UNROLL_J;  // j per unrolled loop body
 constexpr int kIpt4Min = 20480;    // above: 4 particles per thread in fp32
 constexpr int kIpt4MinBox = 14336; // same in the periodic box (29 instead of 20 instructions per step)
 constexpr int kIpt2Min64 = 12288;  // above: 2 particles per thread in fp64
-constexpr int kIpt8Min = 32768;    // above: 8 per thread in fp32
+constexpr int kIpt8Min = 29000;    // above: 8 per thread in fp32 (r01f: 30000: 717 against 730 us, 28000: 654 against 647)
+constexpr int kIpt8MinBox = 43000; // same in the periodic box (36000: 1404 against 1370 us, 49152: 2433 against 2455)
 constexpr int kIpt4Min64 = 40960;  // above: 4 per thread in fp64
 
 enum { TENSOR_RPY = 0, TENSOR_OSEEN = 1 };
