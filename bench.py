@@ -29,8 +29,14 @@ import numpy as np  # noqa: E402
 FLOPS_PER_PAIR = {"rpy": 34, "oseen": 29}       # algorithmic flops
 FLOPS_NEAREST_IMAGE = 15                        # + 3 x (fma, add, fma) per pair in a periodic box
 FP32_LANES_PER_SM, FP64_LANES_PER_SM = 128, 64  # CUDA-core FMA lanes per SM (measured: ubench)
-# DRAM bytes per pair-kernel launch from the ncu --set full capture named in profiles/README.md
-NCU_TRAFFIC_BYTES = {(1048576, "f32", "rpy"): 43.7e6}  # profiles/r01c_pairs_f32_ncu_full.md
+# DRAM bytes (read + write) per pair-kernel launch.  NOT measured by this script (ncu cannot run
+# inside a timed bench): copied from the committed `ncu --set full` capture of the kernel this
+# commit ships, named beside it; a configuration without such a capture reports null.
+NCU_TRAFFIC = {
+    (1048576, "f32", "rpy", False): (42.1e6, "profiles/r01e_launches_bench_f32.md (dram__bytes_read.sum + "
+                                             "dram__bytes_write.sum of pairs_f32_kernel<4,RPY,Kahan>)"),
+}
+CFG5_NS = [1024, 4096, 16384, 65536, 262144, 1048576]   # BASELINE.json configs[4]
 
 
 def parse_args():
@@ -57,6 +63,11 @@ def parse_args():
                     help="instead of the product: the lubrication correction of the forces (Eq. 8, "
                          "PAPER.md:80-104) on N uniform points at phi = 0.05; reports particles/s")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extra", action="store_true",
+                    help="skip the `extra` object (fp64 / Oseen at N = 1M, the configuration-5 sweep, "
+                         "sd_step steps/s on configurations 1, 3, 4)")
+    ap.add_argument("--extra-only", action="store_true",
+                    help="print only the `extra` object (one JSON line)")
     return ap.parse_args()
 
 
@@ -374,6 +385,93 @@ def run_lub(args, rank):
     print(json.dumps(line), flush=True)
 
 
+def fma_peaks(sm_count):
+    """Derived FMA peaks (TFLOP/s) at sm_max_mhz of MEASURED_PEAKS.json."""
+    sm_max_mhz = 1965.0
+    peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(peaks_path):
+        with open(peaks_path) as f:
+            sm_max_mhz = float(json.load(f).get("sm_max_mhz", sm_max_mhz))
+    return {"f32": sm_count * FP32_LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12,
+            "f64": sm_count * FP64_LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12}, sm_max_mhz
+
+
+def _sample_times(torch, fn, warm, samples, per_sample):
+    """`samples` timings of `per_sample` back-to-back calls of fn between one pair of CUDA events on
+    the current (launching) stream, after `warm` untimed calls; seconds per call."""
+    for _ in range(warm):
+        fn()
+    torch.cuda.synchronize()
+    out = []
+    for _ in range(samples):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(per_sample):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        out.append(e0.elapsed_time(e1) * 1e-3 / per_sample)
+    return np.array(out)
+
+
+def extra_measurements(torch, sd, wl, sm_count, probes):
+    """The rest of BASELINE.json's metric, measured in this process:
+    configuration 5 (sd_mobility_apply at six sizes x {fp32-Kahan, fp64} x {RPY, Oseen}; best and
+    median of 10 samples after 3 warm-ups, warm L2 -- the inputs are at most 67 MB) and sd_step
+    steps/s on configurations 1, 3 and 4.  Small products are launch-bound when timed one by one
+    (an event pair costs more than the kernel), so a sample is `launches_per_sample` back-to-back
+    launches on one stream, as a simulation issues them."""
+    peaks, _ = fma_peaks(sm_count)
+    sweep = []
+    for n in CFG5_NS:
+        pos, force = wl.sweep(n)
+        per = int(max(1, min(50, 4e9 // (n * n))))
+        for pname, prec, npdt in (("f32", sd.PREC_F32_KAHAN, np.float32), ("f64", sd.PREC_F64, np.float64)):
+            dp = torch.from_numpy(wl.to_xyzw(pos, npdt)).cuda()
+            df = torch.from_numpy(wl.to_xyzw(force, npdt)).cuda()
+            dv = torch.empty_like(dp)
+            for tname, tensor in (("rpy", sd.TENSOR_RPY), ("oseen", sd.TENSOR_OSEEN)):
+                ctx = sd.Context(n, wl.A, wl.ETA)
+                ctx.set_tensor(tensor)
+                ctx.set_precision(prec)
+                t = _sample_times(torch, lambda: ctx.mobility_apply(dp, df, dv), 3, 10, per)
+                best, med = n * n / t.min(), n * n / float(np.median(t))
+                fl = FLOPS_PER_PAIR[tname] / 1e12
+                sweep.append({"n": n, "precision": pname, "tensor": tname, "kernel": ctx.kernel_name,
+                              "launches_per_sample": per, "us_per_product_median": 1e6 * float(np.median(t)),
+                              "pairs_per_s_best": best, "pairs_per_s_median": med,
+                              "frac_of_derived_peak_best": best * fl / peaks[pname],
+                              "frac_of_derived_peak_median": med * fl / peaks[pname],
+                              "frac_of_probe_median": med * fl / probes[pname]})
+                ctx.close()
+            del dp, df, dv
+    steps = []
+    p1, _ = wl.four_sphere(wl.SEED_BASE + 1)
+    p3, _ = wl.config3()
+    p4, _ = wl.config4()
+    for cfg, pos, integ, iname, dt, nsteps in ((1, p1, sd.INT_MIDPOINT, "midpoint", 0.01, 10000),
+                                               (3, p3, sd.INT_EULER, "euler", 0.01, 20),
+                                               (4, p4, sd.INT_MIDPOINT, "midpoint", 0.05, 10)):
+        n = pos.shape[0]
+        for pname, prec, npdt in (("f32", sd.PREC_F32_KAHAN, np.float32), ("f64", sd.PREC_F64, np.float64)):
+            if cfg == 4 and pname == "f64":
+                continue   # BASELINE.json configs[3] is fp32-Kahan only
+            ctx = sd.Context(n, wl.A, wl.ETA)
+            ctx.set_precision(prec)
+            dq = torch.from_numpy(wl.to_xyzw(pos, npdt)).cuda()
+            t = _sample_times(torch, lambda: ctx.step(dq, dt, nsteps, integ, gravity=(0.0, 0.0, -1.0)),
+                              1, 5, 1)
+            steps.append({"config": cfg, "n": n, "integrator": iname, "precision": pname,
+                          "steps_per_call": nsteps, "steps_per_s_median": nsteps / float(np.median(t)),
+                          "pairs_per_s_median": (2 if iname == "midpoint" else 1) * n * n * nsteps
+                          / float(np.median(t))})
+            ctx.close()
+    return {"what": "BASELINE.json metric beyond the headline point, same process, CUDA events on the "
+                    "launching stream; fractions = pairs/s x (34 RPY | 29 Oseen) flops / FMA peak",
+            "fma_probe_tflops": probes, "derived_peak_tflops": peaks,
+            "config5_sweep": sweep, "sd_step": steps}
+
+
 def main():
     args = parse_args()
     rank = int(os.environ.get("RANK", "0"))
@@ -420,6 +518,7 @@ def main():
     ctx.set_box(box_side(args, wl))
     ctx.set_staging({"bulk": 0, "naive": 1, "sync": 2}[args.staging])
     peak_probe = ctx.fma_peak_probe(prec)
+    probe64 = peak_probe if f64mode else ctx.fma_peak_probe(sd.PREC_F64)
 
     def barrier():
         if world > 1:
@@ -467,28 +566,32 @@ def main():
 
     # ---- roofline of the dominant kernel (compute bound on the CUDA-core FMA pipes) --------
     sm_count = torch.cuda.get_device_properties(dev).multi_processor_count
-    peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
-    sm_max_mhz = 1965.0
-    if os.path.exists(peaks_path):
-        with open(peaks_path) as f:
-            sm_max_mhz = float(json.load(f).get("sm_max_mhz", sm_max_mhz))
+    peaks, sm_max_mhz = fma_peaks(sm_count)
+    pkey = "f64" if f64mode else "f32"
     lanes = FP64_LANES_PER_SM if f64mode else FP32_LANES_PER_SM
-    peak_tflops = sm_count * lanes * 2 * sm_max_mhz * 1e6 / 1e12
+    peak_tflops = peaks[pkey]
     flops = FLOPS_PER_PAIR[args.tensor] + (FLOPS_NEAREST_IMAGE if args.box else 0)
     achieved = flops * float(n) * n * pair_launches / (pair_ms * 1e-3) / 1e12 if pair_ms > 0 else None
+    traffic, traffic_src = NCU_TRAFFIC.get((n, args.precision, args.tensor, args.box), (None, None))
+    if args.staging != "bulk":
+        traffic, traffic_src = None, None
     roofline = {
         "bound": "alu", "kernel": ctx.kernel_name, "achieved": achieved, "peak": peak_tflops,
         "unit": "TFLOP/s", "frac": (achieved / peak_tflops) if achieved else None,
-        "traffic": None if args.box else NCU_TRAFFIC_BYTES.get((n, args.precision, args.tensor)),
+        "frac_is": "of the DERIVED peak (no CUDA-core FMA figure in MEASURED_PEAKS.json)",
+        "frac_of_probe": (achieved / peak_probe) if achieved and peak_probe else None,
+        "traffic": traffic, "traffic_source": traffic_src,
         "peak_source": f"derived: {sm_count} SMs x {lanes} FMA lanes x 2 flop x {sm_max_mhz:.0f} MHz "
                        "(sm_max_mhz of MEASURED_PEAKS.json; DESIGN.md)",
         "fma_probe_tflops": peak_probe,
+        "fma_probe_is": "dependent-FMA-chain kernel of this library (sd_fma_peak_probe) timed in this run",
         "flops_per_pair": flops, "kernel_ms": pair_ms / max(pair_launches, 1),
         "kernel_share_of_step": pair_ms * 1e-3 / local_s if local_s > 0 else None,
-        "frac_at_measured_clock": (achieved / (peak_tflops * clocks["sm_mhz"] / sm_max_mhz))
-        if achieved and clocks.get("sm_mhz") else None,
     }
+    if clocks.get("sm_mhz") and abs(clocks["sm_mhz"] - sm_max_mhz) > 1.0 and achieved:
+        roofline["frac_at_measured_clock"] = achieved / (peak_tflops * clocks["sm_mhz"] / sm_max_mhz)
 
+    in_mb = 2 * n * 4 * (8 if f64mode else 4) / 1e6
     line = {
         "metric": "pair interactions/s (mobility matvec)", "value": value, "unit": "pairs/s",
         "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -496,7 +599,7 @@ def main():
         "vs_baseline": None, "dtype": "f64" if f64mode else "f32", "data": "synthetic",
         "config": {"workload": workload_name(args), "kernel": ctx.kernel_name,
                    "parallelism": "replicas only (no sharding, no collective)" if world > 1 else "1 GPU",
-                   "l2": "inputs (33.5 MB) fit in L2; L2 flushed with a 256 MiB write between timed iterations"},
+                   "l2": f"inputs ({in_mb:.1f} MB) fit in L2; L2 flushed with a 256 MiB write between timed iterations"},
         "clocks": clocks, "gpu_launches": gpu_launches,
         "e2e": {"value": e2e_units / e2e_t, "unit": "pairs/s", "h2d_bytes_per_step": 2 * rec_bytes,
                 "d2h_bytes_per_step": rec_bytes},
@@ -519,8 +622,15 @@ def main():
                                 "cpu_model": cpu_model(), "one_thread_value": rate1,
                                 "one_thread_sample": f"{rows1} rows, {secs1:.1f} s"}
     ctx.close()
+    default_point = (n == 1048576 and not f64mode and args.tensor == "rpy" and not args.box
+                     and args.staging == "bulk")
+    if rank == 0 and world == 1 and default_point and not args.no_extra:
+        del d_pos, d_force, d_vel
+        probes = {"f32": peak_probe, "f64": probe64}
+        line["extra"] = extra_measurements(torch, sd, wl, sm_count, probes)
     if rank == 0:
-        print(json.dumps(line), flush=True)
+        print(json.dumps({"extra": line["extra"]} if args.extra_only and "extra" in line else line),
+              flush=True)
     if world > 1:
         dist.destroy_process_group()
 

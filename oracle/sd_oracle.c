@@ -39,8 +39,9 @@
  *     excluded.  SDO_IMAGE_DEFINITION takes n from C99 remainder() (exact, ties to even).
  *     SDO_IMAGE_F32 / SDO_IMAGE_F64 take the DECISION n the way an fp32 / fp64 evaluation
  *     does (reading B2): n = nearest integer (ties to even) of the exact product
- *     d * inv with inv = 1/L rounded to that precision (and, for F32, d the fp32 difference
- *     of the fp32 positions); the displacement d - L n itself is then formed in double.
+ *     d * inv with inv = 1/L rounded to that precision (and, for F32, d in that product the
+ *     fp32 difference of the fp32 positions); the displacement d - L n itself is formed in
+ *     double from the exact difference of the stored coordinates.
  *     The variants differ only for pairs within rounding of |d_alpha| = L/2.
  *
  *   - lubrication correction (Eq. 8): see the block comment above
@@ -118,7 +119,9 @@ static double sdo_min_image(double xi, double xj, double L, int image) {
         const float df = (float)xi - (float)xj;    /* fp32 difference of fp32 positions */
         const float invf = 1.0f / (float)L;        /* 1/L rounded to fp32 */
         const double prod = (double)df * (double)invf; /* 24 x 24 bits: exact in double */
-        return (double)df - nearbyint(prod) * (double)(float)L;
+        /* only the DECISION n is taken the fp32 way (reading B2); the displacement is
+         * the exact difference of the stored coordinates shifted by n box sides */
+        return (xi - xj) - nearbyint(prod) * (double)(float)L;
     }
     const double d = xi - xj;
     if (image == SDO_IMAGE_F64) {

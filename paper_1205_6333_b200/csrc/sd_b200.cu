@@ -18,6 +18,7 @@
 #include "sd_common.cuh"
 #include "sd_pairs_f32.cuh"
 #include "sd_pairs_f64.cuh"
+#include "sd_pairs_f32w.cuh"
 #include "sd_access.cuh"
 #include "sd_lub.cuh"
 #include "sd_small.cuh"
@@ -85,6 +86,21 @@ struct sd_ctx {
     int device = 0;
     int num_sms = 0;
     Config cfg;
+    // warp-split one-launch kernel (sd_pairs_f32w.cuh): its own schedule and scratch
+    int jsplit = 0;             // 0 automatic, 1 classic tiled kernels only, 2 warp-split wherever it exists
+    int w_ch = 0;               // j per warp and tile override (0 = automatic)
+    bool w_on = false;          // the current settings run through the warp-split kernel
+    Config wcfg;
+    size_t w_smem = 0;
+    void* w_part = nullptr;
+    int* w_blk_done = nullptr;
+    long long* w_cta_u0 = nullptr;
+    int* w_blk_first = nullptr;
+    int* w_blk_nslots = nullptr;
+    int* w_cta_piece = nullptr;
+    void* w_pad = nullptr;      // 2 x kWTJMax pad records: far-away positions | zero forces
+    void* grav_buf = nullptr;   // uniform force written out per particle (sd_step with gravity)
+    bool valid = false;         // false after a failed (re)configuration: every entry point refuses
     // device buffers (context-owned)
     void* rec = nullptr;        // packed records
     void* part = nullptr;       // segment partial sums
@@ -168,6 +184,14 @@ void free_buffers(sd_ctx* c) {
         *b = nullptr;
     }
     c->lub_H = 0;
+    void** wb[] = {&c->w_part, reinterpret_cast<void**>(&c->w_blk_done), reinterpret_cast<void**>(&c->w_cta_u0),
+                   reinterpret_cast<void**>(&c->w_blk_first), reinterpret_cast<void**>(&c->w_blk_nslots),
+                   reinterpret_cast<void**>(&c->w_cta_piece), &c->w_pad, &c->grav_buf};
+    for (void** b : wb) {
+        if (*b) cudaFree(*b);
+        *b = nullptr;
+    }
+    c->w_on = false;
     if (c->d_cta_u0) cudaFree(c->d_cta_u0);
     if (c->d_blk_first) cudaFree(c->d_blk_first);
     if (c->d_blk_nslots) cudaFree(c->d_blk_nslots);
@@ -220,6 +244,8 @@ HostSchedule build_schedule(long long N, int IB, int TJ, long long max_ctas, int
     return h;
 }
 
+sd_status configure_w(sd_ctx* c);
+
 // Pick the kernel variant for (N, precision, tensor), build the static schedule and
 // (re)allocate every scratch buffer.
 sd_status configure(sd_ctx* c) {
@@ -232,6 +258,7 @@ sd_status configure(sd_ctx* c) {
         c->vel = nullptr;
     }
     free_buffers(c);
+    c->valid = false;  // until every buffer below exists again
     c->vel = keep_vel;
     Config cfg;
     const bool f64 = c->precision == SD_PREC_F64;
@@ -346,6 +373,85 @@ sd_status configure(sd_ctx* c) {
     SD_CUDA(c, cudaMemcpy(c->d_blk_first, first.data(), sizeof(int) * cfg.B, cudaMemcpyHostToDevice));
     SD_CUDA(c, cudaMemcpy(c->d_blk_nslots, nslots.data(), sizeof(int) * cfg.B, cudaMemcpyHostToDevice));
     c->lo_valid = true;  // zeroed
+    // mid N in the fp32 modes: the whole product in one launch of the warp-split kernel
+    if (!f64 && c->staging == sd::STAGE_BULK && c->N > c->small_apply_max &&
+        (c->jsplit == 2 || (c->jsplit == 0 && c->N <= sd::kWMaxN))) {
+        sd_status ws = configure_w(c);
+        if (ws != SD_OK) return ws;
+    }
+    c->valid = true;
+    return SD_OK;
+}
+
+// ---- warp-split one-launch kernel (sd_pairs_f32w.cuh) -----------------------------------------
+template <int I2, int CH>
+const void* w_pick(bool rpy, bool plain, bool pbc) {
+#define SD_W(T, A, P) reinterpret_cast<const void*>(&sd::pairs_f32w_kernel<I2, T, A, P, CH>)
+    if (rpy) {
+        if (plain) return pbc ? SD_W(0, 1, true) : SD_W(0, 1, false);
+        return pbc ? SD_W(0, 0, true) : SD_W(0, 0, false);
+    }
+    if (plain) return pbc ? SD_W(1, 1, true) : SD_W(1, 1, false);
+    return pbc ? SD_W(1, 0, true) : SD_W(1, 0, false);
+#undef SD_W
+}
+
+// j records per warp and tile: the largest chunk that still leaves every CTA enough units for an
+// even split (stream-K pieces differ by one unit)
+int w_auto_ch(long long N, int ibw, long long ctas) {
+    for (int ch : {32, 16}) {
+        const long long U = ((N + ibw - 1) / ibw) * ((N + 8 * ch - 1) / (8 * ch));
+        if (U >= 12 * ctas) return ch;
+    }
+    return 8;
+}
+
+sd_status configure_w(sd_ctx* c) {
+    const bool rpy = c->tensor == SD_TENSOR_RPY, plain = c->precision == SD_PREC_F32_PLAIN, pbc = c->box > 0.0;
+    Config w;
+    const int i2 = 4;
+    w.ipt = 2 * i2;
+    w.IB = 64 * i2;
+    const int ch = c->w_ch ? c->w_ch : w_auto_ch(c->N, w.IB, c->num_sms);
+    w.TJ = 8 * ch;
+    size_t smem = 0;
+    if (ch == 128) w.kernel = w_pick<4, 128>(rpy, plain, pbc), smem = sd::WShape<4, 128>::smem_bytes;
+    else if (ch == 64) w.kernel = w_pick<4, 64>(rpy, plain, pbc), smem = sd::WShape<4, 64>::smem_bytes;
+    else if (ch == 32) w.kernel = w_pick<4, 32>(rpy, plain, pbc), smem = sd::WShape<4, 32>::smem_bytes;
+    else if (ch == 16) w.kernel = w_pick<4, 16>(rpy, plain, pbc), smem = sd::WShape<4, 16>::smem_bytes;
+    else if (ch == 8) w.kernel = w_pick<4, 8>(rpy, plain, pbc), smem = sd::WShape<4, 8>::smem_bytes;
+    else return fail(c, SD_ERR_INVALID_ARG, "warp-split kernel: j per warp and tile must be 8, 16, 32, 64 or 128");
+    static const char* wn[2][2][2] = {{{"pairs_f32x2_w8_rpy_kahan", "pairs_f32x2_w8_rpy_kahan_pbc"},
+                                       {"pairs_f32x2_w8_rpy_plain", "pairs_f32x2_w8_rpy_plain_pbc"}},
+                                      {{"pairs_f32x2_w8_oseen_kahan", "pairs_f32x2_w8_oseen_kahan_pbc"},
+                                       {"pairs_f32x2_w8_oseen_plain", "pairs_f32x2_w8_oseen_plain_pbc"}}};
+    w.name = wn[rpy ? 0 : 1][plain ? 1 : 0][pbc ? 1 : 0];
+    SD_CUDA(c, cudaFuncSetAttribute(w.kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem)));
+    int occ = 0;
+    SD_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, w.kernel, sd::kThreads, smem));
+    if (occ < 1) return fail(c, SD_ERR_CUDA, "warp-split pair kernel does not fit on an SM");
+    const HostSchedule hs = build_schedule(c->N, w.IB, w.TJ, static_cast<long long>(c->num_sms) * occ, c->num_sms);
+    w.B = hs.B, w.T = hs.T, w.U = hs.U, w.G = hs.G, w.max_slots = hs.max_slots;
+    c->wcfg = w;
+    c->w_smem = smem;
+    const size_t nrec = static_cast<size_t>(c->Nrec);
+    SD_CUDA(c, cudaMalloc(&c->w_part, nrec * 2 * sizeof(float4) * w.max_slots));
+    SD_CUDA(c, cudaMalloc(&c->w_blk_done, sizeof(int) * w.B));
+    SD_CUDA(c, cudaMemset(c->w_blk_done, 0, sizeof(int) * w.B));
+    SD_CUDA(c, cudaMalloc(&c->w_cta_u0, sizeof(long long) * (w.G + 1)));
+    SD_CUDA(c, cudaMalloc(&c->w_blk_first, sizeof(int) * w.B));
+    SD_CUDA(c, cudaMalloc(&c->w_blk_nslots, sizeof(int) * w.B));
+    SD_CUDA(c, cudaMalloc(&c->w_cta_piece, sizeof(int) * w.G));
+    SD_CUDA(c, cudaMemcpy(c->w_cta_u0, hs.u0.data(), sizeof(long long) * (w.G + 1), cudaMemcpyHostToDevice));
+    SD_CUDA(c, cudaMemcpy(c->w_blk_first, hs.first.data(), sizeof(int) * w.B, cudaMemcpyHostToDevice));
+    SD_CUDA(c, cudaMemcpy(c->w_blk_nslots, hs.nslots.data(), sizeof(int) * w.B, cudaMemcpyHostToDevice));
+    SD_CUDA(c, cudaMemcpy(c->w_cta_piece, hs.piece.data(), sizeof(int) * w.G, cudaMemcpyHostToDevice));
+    std::vector<float4> pad(2 * sd::kWTJMax, make_float4(0.f, 0.f, 0.f, 0.f));
+    for (int q = 0; q < sd::kWTJMax; ++q) pad[q] = make_float4(SD_PAD_POS, SD_PAD_POS, SD_PAD_POS, 0.f);
+    SD_CUDA(c, cudaMalloc(&c->w_pad, pad.size() * sizeof(float4)));
+    SD_CUDA(c, cudaMemcpy(c->w_pad, pad.data(), pad.size() * sizeof(float4), cudaMemcpyHostToDevice));
+    SD_CUDA(c, cudaMalloc(&c->grav_buf, nrec * sizeof(float4)));
+    c->w_on = true;
     return SD_OK;
 }
 
@@ -416,8 +522,10 @@ sd::PairCoefT<S> folded_coef(const sd_ctx* c) {
     return k;
 }
 
-sd_status launch_pairs(sd_ctx* c, cudaStream_t st) {
-    if (!c->profiling || c->prof_events.size() >= 4096) return launch_pairs_impl(c, st);
+// runs `impl` (a pair-kernel launch); while profiling is on, between two events on the stream
+template <typename Impl>
+sd_status profiled(sd_ctx* c, cudaStream_t st, Impl impl) {
+    if (!c->profiling || c->prof_events.size() >= 4096) return impl();
     std::pair<cudaEvent_t, cudaEvent_t> ev;
     if (!c->prof_pool.empty()) {
         ev = c->prof_pool.back();
@@ -427,10 +535,48 @@ sd_status launch_pairs(sd_ctx* c, cudaStream_t st) {
         SD_CUDA(c, cudaEventCreate(&ev.second));
     }
     SD_CUDA(c, cudaEventRecord(ev.first, st));
-    sd_status s = launch_pairs_impl(c, st);
+    sd_status s = impl();
     SD_CUDA(c, cudaEventRecord(ev.second, st));
     c->prof_events.push_back(ev);
     return s;
+}
+
+sd_status launch_pairs(sd_ctx* c, cudaStream_t st) {
+    return profiled(c, st, [&]() { return launch_pairs_impl(c, st); });
+}
+
+// one product (+ fused update) in one launch of the warp-split kernel; arguments as launch_small_apply
+sd_status launch_w(sd_ctx* c, const void* posx, const void* force, void* vel, const void* pos_base,
+                   void* pos_out, double dt, int mode, cudaStream_t st) {
+    return profiled(c, st, [&]() -> sd_status {
+        sd::Schedule sch;
+        sch.cta_u0 = c->w_cta_u0;
+        sch.blk_first_cta = c->w_blk_first;
+        sch.blk_nslots = c->w_blk_nslots;
+        sch.cta_piece = c->w_cta_piece;
+        sch.T = c->wcfg.T, sch.B = c->wcfg.B, sch.G = c->wcfg.G;
+        sd::PairCoef k = folded_coef<float>(c);
+        sd::FinArgs fin;
+        fin.vel = static_cast<float4*>(vel);
+        fin.pos_base = static_cast<const float4*>(pos_base);
+        fin.pos_lo = static_cast<float4*>(c->pos_lo);
+        fin.pos_out = static_cast<float4*>(pos_out);
+        fin.dt = dt;
+        fin.c1 = c->mu0 * 0.75 * c->a;
+        fin.mu0 = c->mu0;
+        fin.mode = mode;
+        fin.pos_comp = c->pos_comp;
+        const float4* pp = static_cast<const float4*>(posx);
+        const float4* ff = static_cast<const float4*>(force);
+        const float4* pad = static_cast<const float4*>(c->w_pad);
+        float4* part = static_cast<float4*>(c->w_part);
+        int n = static_cast<int>(c->N);
+        long long stride = c->Nrec;
+        void* args[] = {&pp, &ff, &pad, &part, &c->w_blk_done, &sch, &k, &fin, &n, &stride};
+        cudaError_t e = cudaLaunchKernel(c->wcfg.kernel, dim3(c->wcfg.G), dim3(sd::kThreads), args, c->w_smem, st);
+        if (e != cudaSuccess) return fail(c, SD_ERR_CUDA, std::string("pairs_f32w: ") + cudaGetErrorString(e));
+        return check_launch(c, c->wcfg.name);
+    });
 }
 
 sd_status launch_pairs_impl(sd_ctx* c, cudaStream_t st) {
@@ -466,13 +612,15 @@ sd_status launch_finalize(sd_ctx* c, void* vel, void* pos, double dt, cudaStream
         sd::finalize_f64_kernel<MODE><<<blocks, sd::kFinThreads, 0, st>>>(
             static_cast<const double4*>(c->part), c->d_blk_nslots, static_cast<double4*>(c->rec),
             static_cast<double4*>(vel), static_cast<double4*>(pos),
-            static_cast<double4*>(c->pos_half), dt, 4.0 / (3.0 * c->a), n, c->cfg.IB, c->Nrec);
+            static_cast<double4*>(c->pos_half), dt, 4.0 / (3.0 * c->a), n, c->cfg.IB, c->Nrec,
+            c->tensor, 4.0 * c->a * c->a, 2.0 * c->a * c->a / 3.0);
     else
         sd::finalize_f32_kernel<MODE><<<blocks, sd::kFinThreads, 0, st>>>(
             static_cast<const float4*>(c->part), c->d_blk_nslots, static_cast<float4*>(c->rec),
             static_cast<float4*>(vel), static_cast<float4*>(pos), static_cast<float4*>(c->pos_lo),
             static_cast<float4*>(c->pos_half), dt, 4.0 / (3.0 * c->a), n, c->cfg.IB, c->Nrec,
-            c->pos_comp);
+            c->pos_comp, c->tensor, static_cast<float>(4.0 * c->a * c->a),
+            static_cast<float>(2.0 * c->a * c->a / 3.0));
     return check_launch(c, "finalize_kernel");
 }
 
@@ -553,6 +701,8 @@ sd_status launch_small_packed(sd_ctx* c, const void* posx, const void* force, co
 sd_status launch_small_apply(sd_ctx* c, const void* posx, const void* force, const double g[3],
                              void* vel, const void* pos_base, void* pos_out, double dt, int mode,
                              cudaStream_t st) {
+    if (c->w_on)  // mid N: warp-split kernel; a uniform force has been written to grav_buf by the caller
+        return launch_w(c, posx, force ? force : c->grav_buf, vel, pos_base, pos_out, dt, mode, st);
     if (c->precision != SD_PREC_F64 && c->N >= sd::kPackedMinN && c->N <= sd::kPackedMaxN &&
         c->N <= c->small_apply_max) {
         if (c->precision == SD_PREC_F32_PLAIN)
@@ -830,6 +980,18 @@ sd_status sd_set_dispatch(sd_ctx* ctx, long long small_apply_max, int particles_
     return configure(ctx);
 }
 
+sd_status sd_set_jsplit(sd_ctx* ctx, int mode, int j_per_warp) {
+    if (!ctx) return fail(nullptr, SD_ERR_INVALID_ARG, "sd_set_jsplit: ctx is NULL");
+    if (mode < 0 || mode > 2) return fail(ctx, SD_ERR_INVALID_ARG, "sd_set_jsplit: mode must be 0, 1 or 2");
+    if (j_per_warp != 0 && j_per_warp != 8 && j_per_warp != 16 && j_per_warp != 32 && j_per_warp != 64 &&
+        j_per_warp != 128)
+        return fail(ctx, SD_ERR_INVALID_ARG, "sd_set_jsplit: j_per_warp must be 0, 8, 16, 32, 64 or 128");
+    cudaDeviceSynchronize();
+    ctx->jsplit = mode;
+    ctx->w_ch = j_per_warp;
+    return configure(ctx);
+}
+
 sd_status sd_set_position_compensation(sd_ctx* ctx, int on) {
     if (!ctx) return fail(nullptr, SD_ERR_INVALID_ARG, "sd_set_position_compensation: ctx is NULL");
     ctx->pos_comp = on ? 1 : 0;
@@ -879,7 +1041,7 @@ sd_status sd_mobility_apply(sd_ctx* ctx, const void* pos, const void* force, voi
         return fail(ctx, SD_ERR_INVALID_ARG, "sd_mobility_apply: records must be 16-byte (float) / 32-byte (double) aligned");
     if (vel == pos || vel == force) return fail(ctx, SD_ERR_INVALID_ARG, "sd_mobility_apply: vel aliases an input");
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    if (ctx->N <= ctx->small_apply_max)  // small-N path: one launch, no pack / partials / finalize
+    if (ctx->N <= ctx->small_apply_max || ctx->w_on)  // one launch, no pack / finalize kernels
         return launch_small_apply(ctx, pos, force, nullptr, vel, nullptr, nullptr, 0.0, sd::FIN_VEL, st);
     sd_status s = launch_pack(ctx, pos, force, sd::PACK_POS | sd::PACK_FORCE, nullptr, st);
     if (s != SD_OK) return s;
@@ -930,6 +1092,13 @@ sd_status sd_step(sd_ctx* ctx, void* pos, sd_force_fn fn, void* user, const void
         ctx->lo_valid = true;
     }
     const bool lub = ctx->lubrication != 0;
+    if (ctx->w_on && !fn && !lub && !force) {  // the warp-split kernel reads a force array
+        const int n = static_cast<int>(ctx->N);
+        sd::fill4_kernel<<<(n + 255) / 256, 256, 0, st>>>(static_cast<float4*>(ctx->grav_buf),
+                                                         static_cast<float>(gravity[0]), static_cast<float>(gravity[1]),
+                                                         static_cast<float>(gravity[2]), n);
+        if ((s = check_launch(ctx, "fill4_kernel")) != SD_OK) return s;
+    }
     if (!fn && !lub && ctx->N <= sd::kStepperMax)  // all steps in one launch
         return launch_stepper(ctx, pos, force, gravity, dt, n_steps, integrator, st);
 
@@ -951,7 +1120,7 @@ sd_status sd_step(sd_ctx* ctx, void* pos, sd_force_fn fn, void* user, const void
         if (lub) return launch_lubrication(ctx, p, ctx->vel, fe, fe ? nullptr : gg, ctx->force_buf, st);
         return SD_OK;
     };
-    if (ctx->N <= ctx->small_apply_max) {    // one launch per product
+    if (ctx->N <= ctx->small_apply_max || ctx->w_on) {    // one launch per product
         const void* fptr = dynamic ? ctx->force_buf : force;
         const double* g = (dynamic || force) ? nullptr : gravity;
         void* cur = pos;
@@ -1101,6 +1270,7 @@ double sd_box(const sd_ctx* ctx) { return ctx ? ctx->box : 0.0; }
 long long sd_launch_count(const sd_ctx* ctx) { return ctx ? ctx->launches : 0; }
 const char* sd_kernel_name(const sd_ctx* ctx) {
     if (!ctx) return "";
+    if (ctx->w_on) return ctx->wcfg.name;
     if (ctx->N <= ctx->small_apply_max)
         return ctx->precision == SD_PREC_F64
                    ? "small_apply_f64"

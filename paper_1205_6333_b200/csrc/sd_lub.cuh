@@ -135,7 +135,9 @@ __device__ __forceinline__ double lub_disp<float>(const float xi, const float xj
     const float d = __fsub_rn(xi, xj);
     const float Lf = static_cast<float>(g.L);
     const float n = __fsub_rn(__fmaf_rn(d, __fdiv_rn(1.0f, Lf), 12582912.0f), 12582912.0f);
-    return static_cast<double>(d) - static_cast<double>(n) * static_cast<double>(Lf);
+    // only the image index n is an fp32 decision; the displacement is the exact difference of the
+    // stored coordinates shifted by n box sides (all three terms are exact in double)
+    return (static_cast<double>(xi) - static_cast<double>(xj)) - static_cast<double>(n) * static_cast<double>(Lf);
 }
 template <>
 __device__ __forceinline__ double lub_disp<double>(const double xi, const double xj, const LubGrid& g) {
@@ -154,10 +156,11 @@ __device__ __forceinline__ bool lub_inside(double, double dx, double dy, double 
     return __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz)) < nine_a2;
 }
 
-// fp32 contexts: the same decision without leaving fp32 (the float difference is the correctly
-// rounded exact difference, and fmaf(-n, L, d) the correctly rounded image displacement, i.e. the
-// very floats lub_inside(float, ...) forms from the doubles): rejects the ~95 % of candidates
-// that lie outside 3a before any fp64 instruction is issued.
+// fp32 contexts: a conservative pre-filter that never leaves fp32.  The decision itself is taken
+// by lub_inside on the floats of the exact image displacement; the all-fp32 displacement used here
+// differs from those by a few ulp of the box side, so candidates are only rejected when they lie
+// outside 3a by a relative margin of 2^-10 in r^2 (>> ulp(L) / 3a for any box whose coordinates
+// fp32 can still tell apart): ~95 % of the candidates go before any fp64 instruction is issued.
 __device__ __forceinline__ bool lub_reject_f32(const float4 pi, const float4 pj, const LubGrid& g,
                                                const float nine_a2) {
     float dx = __fsub_rn(pi.x, pj.x), dy = __fsub_rn(pi.y, pj.y), dz = __fsub_rn(pi.z, pj.z);
@@ -167,7 +170,7 @@ __device__ __forceinline__ bool lub_reject_f32(const float4 pi, const float4 pj,
         dy = __fmaf_rn(-__fsub_rn(__fmaf_rn(dy, iL, M), M), Lf, dy);
         dz = __fmaf_rn(-__fsub_rn(__fmaf_rn(dz, iL, M), M), Lf, dz);
     }
-    return !(__fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx))) < nine_a2);
+    return __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx))) > nine_a2 * 1.0009765625f;
 }
 __device__ __forceinline__ bool lub_reject_f32(const double4, const double4, const LubGrid&, const float) {
     return false;  // fp64 contexts decide in fp64 below

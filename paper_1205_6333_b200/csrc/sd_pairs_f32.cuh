@@ -44,10 +44,7 @@ constexpr int kTJSmallMaxN = 12288;
 constexpr int kStages = 4;   // ring depth
 constexpr int kPrefetch = 2; // tiles in flight ahead of the one being consumed
 constexpr int kChunk = 32;   // j per compensation chunk
-#ifndef SD_UNROLL_J
-#define SD_UNROLL_J 4
-#endif
-constexpr int kUnrollJ = SD_UNROLL_J;  // j per unrolled loop body
+constexpr int kUnrollJ = 4;  // j per unrolled loop body (2: -3 %, 8: -2.7 % at N = 1 M)
 // measured crossovers of the particles-per-thread variants (profiles/r01e_sweep.md)
 constexpr int kIpt4Min = 20480;    // above: 4 particles per thread in fp32
 constexpr int kIpt4MinBox = 14336; // same in the periodic box (29 instead of 20 instructions per step)
@@ -177,11 +174,7 @@ __device__ __forceinline__ void pair_fast_staged(const f32x2 (&xi)[I2], const f3
             mn = fminf(mn, fminf(a, b));
         }
         inv[m] = pk2(rsq_approx(a), rsq_approx(b));
-#ifdef SD_INV2_MUL
-        inv2[m] = mul2(inv[m], inv[m]);
-#else
         inv2[m] = pk2(rcp_approx(a), rcp_approx(b));
-#endif
     }
 #pragma unroll
     for (int m = 0; m < I2; ++m) dF[m] = mul2(dx[m], fx);
@@ -296,6 +289,89 @@ __device__ __forceinline__ void pair_clamped_sub(const float xi, const float yi,
     px = fmaf(-Bd, dx, px);
     py = fmaf(-Bd, dy, py);
     pz = fmaf(-Bd, dz, pz);
+}
+
+// Coefficient of F'_i in the term the CLAMP body adds for the self pair (d = 0, r^2 clamped to
+// k.clampv): A_c = 1/r_c + k2/r_c^3 (Rotne-Prager) or 1/r_c (Oseen), formed by the very
+// instructions of pair_fast_staged so that the finalize kernel subtracts what the pair kernel
+// added.  The d-dependent part of the term is exactly 0.
+__device__ __forceinline__ float self_clamped_coef(const int tensor, const float clampv, const float k2) {
+    const float inv = rsq_approx(clampv), inv2 = rcp_approx(clampv);
+    const float inv3 = __fmul_rn(inv, inv2);
+    return tensor == TENSOR_RPY ? __fmaf_rn(inv3, k2, inv) : inv;
+}
+
+// Repair of one chunk whose packed pass met a pair below the clamp (overlapping spheres,
+// coincident centres).  The fast body has then added a far-field term of enormous size to ONE
+// lane's sum of ONE particle; every other sum of the chunk is fine.  So nothing is redone for the
+// warp: each lane scans its 2 I2 particles for min r^2 over the chunk (self pair and pad records
+// excluded) and recomputes, with the exact branching body, only the chunk sums of the particles
+// that have such a pair -- about half the cost of one ordinary chunk pass, where redoing the
+// chunk with per-pair checks cost six to eight (the mid-N loss of round 1: at phi = 0.01 one
+// chunk pass in 50 is hit at N = 32768, one in 12 at N = 8192).
+//   cp / cf : positions / forces of the chunk's records, JS float4 apart from one j to the next
+//   ISTEP   : index distance between the particles of consecutive slots (m, half) of a lane
+//   thr     : k.thr after the unclamped body; k.clampv after the clamped body of a diagonal chunk
+//             (there every pair below the clamp was evaluated with the clamped r, Oseen included)
+// Convention kept for the epilogue: a self pair leaves the clamped term A_c F'_i in the sum.
+template <int I2, int TENSOR, int ACC, bool PBC, int CK, int JS, int ISTEP>
+__device__ __forceinline__ void chunk_fix(const f32x2 (&xi)[I2], const f32x2 (&yi)[I2], const f32x2 (&zi)[I2],
+                                          const float4* cp, const float4* cf, const int j0, const int N,
+                                          const int i_first, const PairCoef& k, const float thr, f32x2 (&px)[I2],
+                                          f32x2 (&py)[I2], f32x2 (&pz)[I2], const f32x2 (&qx)[I2],
+                                          const f32x2 (&qy)[I2], const f32x2 (&qz)[I2]) {
+    const int nj = min(CK, N - j0);  // pad records (j >= N) hold no particle
+#pragma unroll
+    for (int m = 0; m < I2; ++m) {
+        float nx[2], ny[2], nz[2];
+        bool redo[2];
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const float x = h ? hi2(xi[m]) : lo2(xi[m]);
+            const float y = h ? hi2(yi[m]) : lo2(yi[m]);
+            const float z = h ? hi2(zi[m]) : lo2(zi[m]);
+            const int jself = i_first + (2 * m + h) * ISTEP - j0;  // position of the self pair in the chunk
+            float mnq = 3.0e38f;
+#pragma unroll 4
+            for (int jj = 0; jj < nj; ++jj) {
+                const float4 pj = cp[jj * JS];
+                float dx = x - pj.x, dy = y - pj.y, dz = z - pj.z;
+                if (PBC) {
+                    dx = __fmaf_rn(__fsub_rn(__fmaf_rn(dx, k.invL, k.magic), k.magic), k.mL, dx);
+                    dy = __fmaf_rn(__fsub_rn(__fmaf_rn(dy, k.invL, k.magic), k.magic), k.mL, dy);
+                    dz = __fmaf_rn(__fsub_rn(__fmaf_rn(dz, k.invL, k.magic), k.magic), k.mL, dz);
+                }
+                const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+                mnq = fminf(mnq, jj == jself ? 3.0e38f : r2);
+            }
+            redo[h] = mnq < thr;
+            nx[h] = ny[h] = nz[h] = 0.f;
+            if (redo[h]) {
+#pragma unroll 1
+                for (int jj = 0; jj < nj; ++jj) {
+                    const float4 pj = cp[jj * JS];
+                    const float4 fj = cf[jj * JS];
+                    if (jj == jself) {  // keep the convention: clamped self term
+                        const float ac = self_clamped_coef(TENSOR, k.clampv, k.k2);
+                        nx[h] = fmaf(ac, fj.x, nx[h]);
+                        ny[h] = fmaf(ac, fj.y, ny[h]);
+                        nz[h] = fmaf(ac, fj.z, nz[h]);
+                    } else {
+                        pair_exact<TENSOR, PBC>(x, y, z, false, pj, fj, k, nx[h], ny[h], nz[h]);
+                    }
+                }
+            }
+        }
+        if (redo[0] || redo[1]) {
+            // sums of the chunk so far: PLAIN carries the running sum (value at chunk start in q)
+            const float bx0 = ACC == ACC_KAHAN ? 0.f : lo2(qx[m]), bx1 = ACC == ACC_KAHAN ? 0.f : hi2(qx[m]);
+            const float by0 = ACC == ACC_KAHAN ? 0.f : lo2(qy[m]), by1 = ACC == ACC_KAHAN ? 0.f : hi2(qy[m]);
+            const float bz0 = ACC == ACC_KAHAN ? 0.f : lo2(qz[m]), bz1 = ACC == ACC_KAHAN ? 0.f : hi2(qz[m]);
+            px[m] = pk2(redo[0] ? bx0 + nx[0] : lo2(px[m]), redo[1] ? bx1 + nx[1] : hi2(px[m]));
+            py[m] = pk2(redo[0] ? by0 + ny[0] : lo2(py[m]), redo[1] ? by1 + ny[1] : hi2(py[m]));
+            pz[m] = pk2(redo[0] ? bz0 + nz[0] : lo2(pz[m]), redo[1] ? bz1 + nz[1] : hi2(pz[m]));
+        }
+    }
 }
 
 __device__ __forceinline__ void kahan_merge2(f32x2& s, f32x2& c, const f32x2 p) {
@@ -434,6 +510,9 @@ pairs_f32_kernel(const float4* __restrict__ rec, float4* __restrict__ part, cons
                     // chunk.  Every pair goes through the clamped packed body (finite terms of
                     // ordinary size, so nothing cancels); the pairs below the clamp are then put
                     // right one by one: clamped term out, exact term (none for the self pair) in.
+                    // (The cheaper repair of the warp-split kernel, chunk_fix, was measured here too:
+                    // it moves the register allocation of the hot loop, -2.0 % at N = 1 M, -1.4 % at
+                    // 65 536, +0.9 % at 32 768; profiles/r02_mid_n.md.)
 #pragma unroll
                     for (int m = 0; m < I2; ++m) {
                         if (ACC == ACC_KAHAN) {
@@ -453,22 +532,26 @@ pairs_f32_kernel(const float4* __restrict__ rec, float4* __restrict__ part, cons
                                                                 mn, r2v);
 #pragma unroll
                         for (int m = 0; m < I2; ++m) {
-                            if (fminf(r2v[2 * m], r2v[2 * m + 1]) < k.clampv && j < N) {
-                                const int i0 = i_first + (2 * m) * kThreads;
+                            // the self pair keeps its clamped term A_c F'_i: the finalize kernel
+                            // takes it out again (self_clamped_coef), all rows at once, instead of
+                            // 32 lanes walking through this branch one after the other
+                            const int i0 = i_first + (2 * m) * kThreads;
+                            const bool fix0 = r2v[2 * m] < k.clampv && j != i0;
+                            const bool fix1 = r2v[2 * m + 1] < k.clampv && j != i0 + kThreads;
+                            if ((fix0 || fix1) && j < N) {
                                 float ax = lo2(px[m]), ay = lo2(py[m]), az = lo2(pz[m]);
                                 float bx = hi2(px[m]), by = hi2(py[m]), bz = hi2(pz[m]);
-                                if (r2v[2 * m] < k.clampv) {
+                                if (fix0) {
                                     pair_clamped_sub<TENSOR, PBC>(lo2(xi[m]), lo2(yi[m]), lo2(zi[m]),
                                                                   pj, fj, k, ax, ay, az);
                                     pair_exact<TENSOR, PBC>(lo2(xi[m]), lo2(yi[m]), lo2(zi[m]),
-                                                            j == i0, pj, fj, k, ax, ay, az);
+                                                            false, pj, fj, k, ax, ay, az);
                                 }
-                                if (r2v[2 * m + 1] < k.clampv) {
+                                if (fix1) {
                                     pair_clamped_sub<TENSOR, PBC>(hi2(xi[m]), hi2(yi[m]), hi2(zi[m]),
                                                                   pj, fj, k, bx, by, bz);
                                     pair_exact<TENSOR, PBC>(hi2(xi[m]), hi2(yi[m]), hi2(zi[m]),
-                                                            j == i0 + kThreads, pj, fj, k, bx, by,
-                                                            bz);
+                                                            false, pj, fj, k, bx, by, bz);
                                 }
                                 px[m] = pk2(ax, bx);
                                 py[m] = pk2(ay, by);

@@ -24,22 +24,22 @@ constexpr int kTJ64 = 64;  // j records per tile (4 KiB)
 // 1/r^3 terms: 40x below the 1e-11 tolerance of this path, in 4 fp64 instructions.  The kernel is
 // bound by the FP64 pipe (80 % active, 2 cycles per warp instruction), so the count matters:
 //   Newton (shipped)                      25 fp64 instructions per pair   5.985e11 pairs/s at N = 1 M
-//   Halley, y0 e (1/2 + 3e/8)  (-DSD_F64_HALLEY)      26, error ~1e-21    5.736e11
-//   Halley with the correction in fp32 (-DSD_F64_HALLEY_IN_F32)  24 + 2 F2F   5.549e11
+//   Halley, y0 e (1/2 + 3e/8)  (measured in round 1, removed)   26, error ~1e-21    5.736e11
+//   Halley with the correction in fp32 (measured in round 1, removed)  24 + 2 F2F   5.549e11
 __device__ __forceinline__ double rsqrt_nr2(const double r2, const float r2f) {
     const float yf = rsq_approx(r2f);
     const double y = static_cast<double>(yf);
     const double e = fma(-r2, y * y, 1.0);
-#if defined(SD_F64_HALLEY_IN_F32)
-    const float ef = static_cast<float>(e);
-    const float corr = (yf * ef) * fmaf(0.375f, ef, 0.5f);
-    return y + static_cast<double>(corr);
-#elif defined(SD_F64_HALLEY)
-    const double p = fma(0.375, e, 0.5);
-    return fma(y * e, p, y);
-#else
     return fma(y * e, 0.5, y);
-#endif
+}
+
+// fp64 counterpart of self_clamped_coef (sd_pairs_f32.cuh): what pair_fast_f64<CLAMP> multiplies
+// F'_i with for the self pair.
+__device__ __forceinline__ double self_clamped_coef_f64(const int tensor, const double clampv, const double k2) {
+    const double inv = rsqrt_nr2(clampv, static_cast<float>(clampv));
+    const double inv2 = inv * inv;
+    const double inv3 = inv2 * inv;
+    return tensor == TENSOR_RPY ? fma(k2, inv3, inv) : inv;
 }
 
 // PBC: nearest image as in the fp32 kernel, d <- d - L rint(d / L) with rint taken as
@@ -158,6 +158,51 @@ __device__ __forceinline__ void pair_clamped_sub_f64(const double xi, const doub
     pz = fma(-Bd, dz, pz);
 }
 
+// fp64 counterpart of chunk_fix (sd_pairs_f32.cuh): per particle of the lane, min r^2 over the
+// chunk (self pair and pad records excluded); the chunk sums of the particles that have a pair
+// below `thr` are recomputed with the exact branching body.  A self pair keeps the clamped term
+// A_c F'_i (removed by finalize_f64_kernel).
+template <int I, int TENSOR, bool PBC>
+__device__ __forceinline__ void chunk_fix_f64(const double (&xi)[I], const double (&yi)[I], const double (&zi)[I],
+                                              const double4* cj, const int j0, const int N, const int i_first,
+                                              const PairCoef64& k, const double thr, double (&px)[I],
+                                              double (&py)[I], double (&pz)[I], const double (&qx)[I],
+                                              const double (&qy)[I], const double (&qz)[I]) {
+    const int nj = min(kChunk, N - j0);
+#pragma unroll
+    for (int m = 0; m < I; ++m) {
+        const int jself = i_first + m * kThreads - j0;
+        double mnq = 1.0e300;
+#pragma unroll 4
+        for (int jj = 0; jj < nj; ++jj) {
+            const double4 pj = cj[2 * jj];
+            const double dx = min_image_f64<PBC>(xi[m] - pj.x, k), dy = min_image_f64<PBC>(yi[m] - pj.y, k),
+                         dz = min_image_f64<PBC>(zi[m] - pj.z, k);
+            const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+            mnq = fmin(mnq, jj == jself ? 1.0e300 : r2);
+        }
+        if (mnq < thr) {
+            double nx = 0.0, ny = 0.0, nz = 0.0;
+#pragma unroll 1
+            for (int jj = 0; jj < nj; ++jj) {
+                const double4 pj = cj[2 * jj];
+                const double4 fj = cj[2 * jj + 1];
+                if (jj == jself) {
+                    const double ac = self_clamped_coef_f64(TENSOR, k.clampv, k.k2);
+                    nx = fma(ac, fj.x, nx);
+                    ny = fma(ac, fj.y, ny);
+                    nz = fma(ac, fj.z, nz);
+                } else {
+                    pair_exact_f64<TENSOR, PBC>(xi[m], yi[m], zi[m], false, pj, fj, k, nx, ny, nz);
+                }
+            }
+            px[m] = qx[m] + nx;
+            py[m] = qy[m] + ny;
+            pz[m] = qz[m] + nz;
+        }
+    }
+}
+
 template <int I, int TENSOR, bool PBC>
 __global__ void __launch_bounds__(kThreads, (I == 1) ? 3 : ((I == 2) ? 2 : 1))
 pairs_f64_kernel(const double4* __restrict__ rec, double4* __restrict__ part, const Schedule sch,
@@ -243,6 +288,7 @@ pairs_f64_kernel(const double4* __restrict__ rec, double4* __restrict__ part, co
                 const int j0 = jbase + ch * kChunk;
                 const int rel = j0 - (i_first - lane);  // chunk holding this warp's own particles?
                 const bool diag = rel >= 0 && (rel % kThreads) == 0 && rel < I * kThreads;
+                bool fix;
                 if (!diag) {
 #pragma unroll 4
                     for (int jj = 0; jj < kChunk; ++jj) {
@@ -253,33 +299,29 @@ pairs_f64_kernel(const double4* __restrict__ rec, double4* __restrict__ part, co
                             pair_fast_f64<TENSOR, PBC, false>(xi[m], yi[m], zi[m], pj, fj, k, px[m],
                                                               py[m], pz[m], mn, r2t);
                     }
-                }
-                if (diag || mn < thr) {  // careful pass, as in the fp32 kernel
-#pragma unroll
-                    for (int m = 0; m < I; ++m) {
-                        px[m] = qx[m];
-                        py[m] = qy[m];
-                        pz[m] = qz[m];
-                    }
-#pragma unroll 2
+                    fix = mn < thr;
+                } else {
+                    // diagonal chunk: clamped body, branch-free; exact unless a pair other than the
+                    // lane's self pair lies below the clamp (see the fp32 kernel)
+                    int zeros = 0;
+#pragma unroll 4
                     for (int jj = 0; jj < kChunk; ++jj) {
                         const double4 pj = cj[2 * jj];
                         const double4 fj = cj[2 * jj + 1];
-                        const int j = j0 + jj;
 #pragma unroll
                         for (int m = 0; m < I; ++m) {
                             pair_fast_f64<TENSOR, PBC, true>(xi[m], yi[m], zi[m], pj, fj, k, px[m],
                                                              py[m], pz[m], mn, r2t);
-                            if (r2t < k.clampv && j < N) {
-                                pair_clamped_sub_f64<TENSOR, PBC>(xi[m], yi[m], zi[m], pj, fj, k,
-                                                                  px[m], py[m], pz[m]);
-                                pair_exact_f64<TENSOR, PBC>(xi[m], yi[m], zi[m],
-                                                            j == i_first + m * kThreads, pj, fj, k,
-                                                            px[m], py[m], pz[m]);
-                            }
+                            const bool z = r2t == 0.0;
+                            zeros += z ? 1 : 0;
+                            mn = fminf(mn, z ? 3.0e38f : static_cast<float>(r2t));
                         }
                     }
+                    fix = mn < static_cast<float>(k.clampv) * 1.000001f || zeros != ((j0 + lane < N) ? 1 : 0);
                 }
+                if (fix)  // rare: repair the sums of the particles that have a pair below the clamp
+                    chunk_fix_f64<I, TENSOR, PBC>(xi, yi, zi, cj, j0, N, i_first, k, diag ? k.clampv : k.thr, px,
+                                                  py, pz, qx, qy, qz);
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(&empty_bar[s]);

@@ -9,6 +9,8 @@
 // :263): the update is formed in fp64 from hi + lo + dt v and split again.
 #pragma once
 #include "sd_common.cuh"
+#include "sd_pairs_f32.cuh"
+#include "sd_pairs_f64.cuh"
 
 namespace sd {
 
@@ -60,6 +62,13 @@ pack_kernel(const T4* __restrict__ pos, const T4* __restrict__ force, T4* __rest
     }
 }
 
+// uniform force written out per particle (sd_step with gravity on the paths that read a force array)
+__global__ void __launch_bounds__(256)
+fill4_kernel(float4* __restrict__ out, const float x, const float y, const float z, const int n) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) out[i] = make_float4(x, y, z, 0.f);
+}
+
 constexpr int kFinThreads = 128;
 constexpr int kFinBatch = 8;
 
@@ -70,14 +79,17 @@ finalize_f32_kernel(const float4* __restrict__ part, const int* __restrict__ blk
                     float4* __restrict__ rec, float4* __restrict__ vel, float4* __restrict__ pos,
                     float4* __restrict__ pos_lo, float4* __restrict__ pos_half, const double dt,
                     const double mu0r, const int N, const int IB, const long long slot_stride,
-                    const int pos_comp) {
+                    const int pos_comp, const int tensor, const float clampv, const float k2) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N) return;
     const int nslots = blk_nslots[i / IB];
     const float4 f = rec[2 * static_cast<size_t>(i) + 1];
-    double vx = mu0r * static_cast<double>(f.x);   // self term mu0 F_i = (mu0 / c1) (c1 F_i)
-    double vy = mu0r * static_cast<double>(f.y);
-    double vz = mu0r * static_cast<double>(f.z);
+    // self term mu0 F_i = (mu0 / c1) (c1 F_i), minus the clamped self-pair term A_c F'_i that the
+    // pair kernel's careful pass left in the partial sums (sd_pairs_f32.cuh)
+    const double sc = mu0r - static_cast<double>(self_clamped_coef(tensor, clampv, k2));
+    double vx = sc * static_cast<double>(f.x);
+    double vy = sc * static_cast<double>(f.y);
+    double vz = sc * static_cast<double>(f.z);
     // slots in batches of kFinBatch: the loads of a batch are in flight together (a small-N
     // product has up to T slots per row and this kernel is pure latency); the sum keeps slot order
     for (int s0 = 0; s0 < nslots; s0 += kFinBatch) {
@@ -126,12 +138,14 @@ __global__ void __launch_bounds__(kFinThreads)
 finalize_f64_kernel(const double4* __restrict__ part, const int* __restrict__ blk_nslots,
                     double4* __restrict__ rec, double4* __restrict__ vel,
                     double4* __restrict__ pos, double4* __restrict__ pos_half, const double dt,
-                    const double mu0r, const int N, const int IB, const long long slot_stride) {
+                    const double mu0r, const int N, const int IB, const long long slot_stride,
+                    const int tensor, const double clampv, const double k2) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N) return;
     const int nslots = blk_nslots[i / IB];
     const double4 f = rec[2 * static_cast<size_t>(i) + 1];
-    double vx = mu0r * f.x, vy = mu0r * f.y, vz = mu0r * f.z;
+    const double sc = mu0r - self_clamped_coef_f64(tensor, clampv, k2);  // see finalize_f32_kernel
+    double vx = sc * f.x, vy = sc * f.y, vz = sc * f.z;
     for (int s0 = 0; s0 < nslots; s0 += kFinBatch) {
         double4 p[kFinBatch];
 #pragma unroll

@@ -63,17 +63,23 @@ def uniform_ball(n: int, phi: float, seed: int, a: float = A) -> np.ndarray:
     return u * rad
 
 
-def rsa_cube(n: int, phi: float, seed: int, a: float = A) -> np.ndarray:
+def rsa_cube(n: int, phi: float, seed: int, a: float = A,
+             shell: tuple[float, float] | None = None) -> np.ndarray:
     """Random sequential addition of n non-overlapping spheres (centre distance >= 2a) in a
-    cube centred on the origin.  Cell grid with cell side >= 2a."""
+    cube centred on the origin.  Cell grid with cell side >= 2a.
+    shell = (lo, hi): a candidate is also rejected when its distance to an accepted centre lies in
+    [lo, hi] -- clouds in which no pair sits near a cut-off radius (trajectory parity runs must not
+    straddle the discontinuity of the lubrication correction at r = 3a, reading C3)."""
     L = cube_side(n, phi, a)
     rng = _rng(seed)
-    ncell = max(1, int(L // (2.0 * a)))
+    reach = 2.0 * a if shell is None else max(2.0 * a, float(shell[1]))
+    ncell = max(1, int(L // reach))
     cs = L / ncell
     cells: dict[tuple[int, int, int], list[int]] = {}
     pts = np.empty((n, 3))
     count = 0
     min2 = (2.0 * a) ** 2
+    lo2, hi2 = (shell[0] ** 2, shell[1] ** 2) if shell is not None else (1.0, 0.0)
     while count < n:
         p = rng.uniform(0.0, L, size=3)
         c = tuple(int(v) for v in np.minimum(p // cs, ncell - 1))
@@ -84,7 +90,8 @@ def rsa_cube(n: int, phi: float, seed: int, a: float = A) -> np.ndarray:
                     key = (c[0] + dx, c[1] + dy, c[2] + dz)
                     for k in cells.get(key, ()):
                         q = pts[k]
-                        if (p[0] - q[0]) ** 2 + (p[1] - q[1]) ** 2 + (p[2] - q[2]) ** 2 < min2:
+                        d2 = (p[0] - q[0]) ** 2 + (p[1] - q[1]) ** 2 + (p[2] - q[2]) ** 2
+                        if d2 < min2 or lo2 <= d2 <= hi2:
                             ok = False
                             break
                     if not ok:
@@ -115,6 +122,27 @@ def fcc_lattice(n_cells: int, number_density: float = 0.1, a: float = A,
     if jitter_seed is not None:
         pts = pts + a * _rng(jitter_seed).uniform(-jitter, jitter, size=pts.shape)
     return pts
+
+
+def sc_lattice(n_edge: int, number_density: float = 0.1, a: float = A,
+               jitter_seed: int | None = None, jitter: float = 1e-2) -> np.ndarray:
+    """Simple-cubic lattice of n_edge^3 sites at the given number density, centred, with the same
+    seeded jitter as fcc_lattice.  With an ODD number of sites per edge half a box (sc_box) falls
+    midway between two lattice planes, so no pair component lies within half a lattice spacing of
+    the discontinuity of the nearest-image rule: the cloud for long trajectory
+    comparisons in the periodic box (reading B3)."""
+    sp = (1.0 / number_density) ** (1.0 / 3.0) * a
+    g = np.arange(n_edge)
+    pts = np.stack(np.meshgrid(g, g, g, indexing="ij"), axis=-1).reshape(-1, 3) * sp
+    pts = pts - pts.mean(axis=0)
+    if jitter_seed is not None:
+        pts = pts + a * _rng(jitter_seed).uniform(-jitter, jitter, size=pts.shape)
+    return pts
+
+
+def sc_box(n_edge: int, number_density: float = 0.1, a: float = A) -> float:
+    """Side L of the periodic cube commensurate with sc_lattice(n_edge)."""
+    return n_edge * (1.0 / number_density) ** (1.0 / 3.0) * a
 
 
 def fcc_box(n_cells: int, number_density: float = 0.1, a: float = A) -> float:

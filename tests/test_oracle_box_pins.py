@@ -166,8 +166,9 @@ def test_image_decision_variants_agree_away_from_half_box(image):
     assert np.abs(frac - 0.5).min() > 1e-5           # no pair near the decision boundary
     want = orc.apply(pos, F, 1.0, ETA1, box=L)
     got = orc.apply(pos, F, 1.0, ETA1, box=L, image=image)
-    # same images; IMAGE_F32 forms d from the fp32 difference (<= 1 ulp_32 of |x| off)
-    np.testing.assert_allclose(got, want, rtol=0, atol=1e-5 if image == orc.IMAGE_F32 else 1e-13)
+    # same images, and the displacement is the exact difference in every variant (reading B2:
+    # only the decision n is taken in the kernel's precision)
+    np.testing.assert_allclose(got, want, rtol=0, atol=1e-13)
 
 
 @pytest.mark.parametrize("image", [orc.IMAGE_F32, orc.IMAGE_F64])
@@ -207,8 +208,9 @@ def test_image_decision_rule_against_exact_rational_arithmetic(image):
                 above += abs(prod) > Fraction(1, 2)
                 got = orc.apply(np.array([[xa, 0.25, 0.125], [xb, 0.0, 0.0]]), F, 1.0, ETA1,
                                 box=L, image=image)
-                want = orc.apply(np.array([[d - n * L, 0.25, 0.125], [0.0, 0.0, 0.0]]), F, 1.0,
-                                 ETA1)
+                # the decision uses the fp32 difference d; the displacement is exact: xa - xb - n L
+                want = orc.apply(np.array([[(xa - xb) - n * L, 0.25, 0.125], [0.0, 0.0, 0.0]]), F,
+                                 1.0, ETA1)
                 np.testing.assert_allclose(got, want, rtol=0, atol=1e-14)
                 checked += 1
     assert checked >= 40 and below > 0 and above > 0
