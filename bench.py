@@ -62,6 +62,12 @@ def parse_args():
     ap.add_argument("--lub", action="store_true",
                     help="instead of the product: the lubrication correction of the forces (Eq. 8, "
                          "PAPER.md:80-104) on N uniform points at phi = 0.05; reports particles/s")
+    ap.add_argument("--jsplit", choices=["auto", "classic", "warp"], default="auto",
+                    help="fp32 mapping of the j sum (sd_set_jsplit): classic tiled kernels (pack + pairs + "
+                         "finalize) or the warp-split one-launch kernel; auto = by N")
+    ap.add_argument("--launches-per-step", type=int, default=1,
+                    help="products enqueued back to back inside one timed step (small N: one launch is "
+                         "shorter than the event pair around it); value and ms_per_step are per product")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extra", action="store_true",
                     help="skip the `extra` object (fp64 / Oseen at N = 1M, the configuration-5 sweep, "
@@ -517,6 +523,8 @@ def main():
     ctx.set_tensor(tensor)
     ctx.set_box(box_side(args, wl))
     ctx.set_staging({"bulk": 0, "naive": 1, "sync": 2}[args.staging])
+    ctx.set_jsplit({"auto": 0, "classic": 1, "warp": 2}[args.jsplit])
+    lps = max(1, args.launches_per_step)
     peak_probe = ctx.fma_peak_probe(prec)
     probe64 = peak_probe if f64mode else ctx.fma_peak_probe(sd.PREC_F64)
 
@@ -540,7 +548,8 @@ def main():
         flush.zero_()  # L2 flush between timed iterations (outside the event pair)
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record()
-        ctx.mobility_apply(d_pos, d_force, d_vel)
+        for _ in range(lps):
+            ctx.mobility_apply(d_pos, d_force, d_vel)
         e1.record()
         evs.append((e0, e1))
     barrier()
@@ -549,7 +558,7 @@ def main():
     gpu_launches = ctx.launch_count - launches0
     pair_ms, pair_launches = ctx.profile_read()
     ctx.profile_enable(False)
-    units, t_max = benchutil.aggregate_over_ranks(local_s, float(args.steps) * n * n)
+    units, t_max = benchutil.aggregate_over_ranks(local_s, float(args.steps) * lps * n * n)
     value = units / t_max
 
     # ---- end to end through the host-buffer entry point ------------------------------------
@@ -595,9 +604,10 @@ def main():
     line = {
         "metric": "pair interactions/s (mobility matvec)", "value": value, "unit": "pairs/s",
         "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": 1e3 * t_max / args.steps, "higher_is_better": True, "scaling": "weak",
+        "ms_per_step": 1e3 * t_max / (args.steps * lps), "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64" if f64mode else "f32", "data": "synthetic",
         "config": {"workload": workload_name(args), "kernel": ctx.kernel_name,
+                   "jsplit": args.jsplit, "launches_per_step": lps,
                    "parallelism": "replicas only (no sharding, no collective)" if world > 1 else "1 GPU",
                    "l2": f"inputs ({in_mb:.1f} MB) fit in L2; L2 flushed with a 256 MiB write between timed iterations"},
         "clocks": clocks, "gpu_launches": gpu_launches,

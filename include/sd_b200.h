@@ -102,14 +102,14 @@ sd_status sd_set_dispatch(sd_ctx* ctx, long long small_apply_max, int particles_
 
 /* How the j sum of one particle is split (north_star: "splits j across warps"), fp32 modes, above
  * the small-N path:
- *   mode 0  automatic: the warp-split one-launch kernel up to N ~ 2e5, the classic tiled kernels above
+ *   mode 0  automatic: the warp-split one-launch kernel up to a measured N, the classic kernels above
  *   mode 1  classic only: the 8 warps of a CTA own different particles and share every j tile; j is
  *           split across CTAs; pack / pair / finalize kernels
  *   mode 2  warp-split wherever it exists: the 8 warps of a CTA own the same 256 particles and take
- *           j_per_warp records of every j tile each; sums combined through shared memory; one launch
- *   j_per_warp: 8, 16 or 32 records per warp and tile (tile = 8 x that); 0 = automatic (by N).
+ *           an eighth of the CTA's j range each (their own bulk-copy pipelines), sums combined
+ *           through shared memory, the last CTA of an i-block finishes its rows: one launch
  * Reallocates the scratch buffers; synchronises the device. */
-sd_status sd_set_jsplit(sd_ctx* ctx, int mode, int j_per_warp);
+sd_status sd_set_jsplit(sd_ctx* ctx, int mode);
 
 /* Ablation of the memory-access schemes the paper compares (PAPER.md:111-241 and Appendix A): how
  * the j records reach the threads of the tiled kernel.

@@ -88,7 +88,6 @@ struct sd_ctx {
     Config cfg;
     // warp-split one-launch kernel (sd_pairs_f32w.cuh): its own schedule and scratch
     int jsplit = 0;             // 0 automatic, 1 classic tiled kernels only, 2 warp-split wherever it exists
-    int w_ch = 0;               // j per warp and tile override (0 = automatic)
     bool w_on = false;          // the current settings run through the warp-split kernel
     Config wcfg;
     size_t w_smem = 0;
@@ -98,7 +97,7 @@ struct sd_ctx {
     int* w_blk_first = nullptr;
     int* w_blk_nslots = nullptr;
     int* w_cta_piece = nullptr;
-    void* w_pad = nullptr;      // 2 x kWTJMax pad records: far-away positions | zero forces
+    void* w_pad = nullptr;      // 2 x kWSJ pad records: far-away positions | zero forces
     void* grav_buf = nullptr;   // uniform force written out per particle (sd_step with gravity)
     bool valid = false;         // false after a failed (re)configuration: every entry point refuses
     // device buffers (context-owned)
@@ -375,7 +374,7 @@ sd_status configure(sd_ctx* c) {
     c->lo_valid = true;  // zeroed
     // mid N in the fp32 modes: the whole product in one launch of the warp-split kernel
     if (!f64 && c->staging == sd::STAGE_BULK && c->N > c->small_apply_max &&
-        (c->jsplit == 2 || (c->jsplit == 0 && c->N <= sd::kWMaxN))) {
+        (c->jsplit == 2 || (c->jsplit == 0 && c->N <= (pbc ? sd::kWMaxNBox : sd::kWMaxN)))) {
         sd_status ws = configure_w(c);
         if (ws != SD_OK) return ws;
     }
@@ -384,9 +383,9 @@ sd_status configure(sd_ctx* c) {
 }
 
 // ---- warp-split one-launch kernel (sd_pairs_f32w.cuh) -----------------------------------------
-template <int I2, int CH>
+template <int I2>
 const void* w_pick(bool rpy, bool plain, bool pbc) {
-#define SD_W(T, A, P) reinterpret_cast<const void*>(&sd::pairs_f32w_kernel<I2, T, A, P, CH>)
+#define SD_W(T, A, P) reinterpret_cast<const void*>(&sd::pairs_f32w_kernel<I2, T, A, P>)
     if (rpy) {
         if (plain) return pbc ? SD_W(0, 1, true) : SD_W(0, 1, false);
         return pbc ? SD_W(0, 0, true) : SD_W(0, 0, false);
@@ -396,31 +395,15 @@ const void* w_pick(bool rpy, bool plain, bool pbc) {
 #undef SD_W
 }
 
-// j records per warp and tile: the largest chunk that still leaves every CTA enough units for an
-// even split (stream-K pieces differ by one unit)
-int w_auto_ch(long long N, int ibw, long long ctas) {
-    for (int ch : {32, 16}) {
-        const long long U = ((N + ibw - 1) / ibw) * ((N + 8 * ch - 1) / (8 * ch));
-        if (U >= 12 * ctas) return ch;
-    }
-    return 8;
-}
-
 sd_status configure_w(sd_ctx* c) {
     const bool rpy = c->tensor == SD_TENSOR_RPY, plain = c->precision == SD_PREC_F32_PLAIN, pbc = c->box > 0.0;
     Config w;
     const int i2 = 4;
     w.ipt = 2 * i2;
     w.IB = 64 * i2;
-    const int ch = c->w_ch ? c->w_ch : w_auto_ch(c->N, w.IB, c->num_sms);
-    w.TJ = 8 * ch;
-    size_t smem = 0;
-    if (ch == 128) w.kernel = w_pick<4, 128>(rpy, plain, pbc), smem = sd::WShape<4, 128>::smem_bytes;
-    else if (ch == 64) w.kernel = w_pick<4, 64>(rpy, plain, pbc), smem = sd::WShape<4, 64>::smem_bytes;
-    else if (ch == 32) w.kernel = w_pick<4, 32>(rpy, plain, pbc), smem = sd::WShape<4, 32>::smem_bytes;
-    else if (ch == 16) w.kernel = w_pick<4, 16>(rpy, plain, pbc), smem = sd::WShape<4, 16>::smem_bytes;
-    else if (ch == 8) w.kernel = w_pick<4, 8>(rpy, plain, pbc), smem = sd::WShape<4, 8>::smem_bytes;
-    else return fail(c, SD_ERR_INVALID_ARG, "warp-split kernel: j per warp and tile must be 8, 16, 32, 64 or 128");
+    w.TJ = sd::kWQ;  // the schedule is cut at 4-record granularity; tiles are private to the warps
+    w.kernel = w_pick<4>(rpy, plain, pbc);
+    const size_t smem = sd::WShape<4>::smem_bytes;
     static const char* wn[2][2][2] = {{{"pairs_f32x2_w8_rpy_kahan", "pairs_f32x2_w8_rpy_kahan_pbc"},
                                        {"pairs_f32x2_w8_rpy_plain", "pairs_f32x2_w8_rpy_plain_pbc"}},
                                       {{"pairs_f32x2_w8_oseen_kahan", "pairs_f32x2_w8_oseen_kahan_pbc"},
@@ -430,7 +413,8 @@ sd_status configure_w(sd_ctx* c) {
     int occ = 0;
     SD_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, w.kernel, sd::kThreads, smem));
     if (occ < 1) return fail(c, SD_ERR_CUDA, "warp-split pair kernel does not fit on an SM");
-    const HostSchedule hs = build_schedule(c->N, w.IB, w.TJ, static_cast<long long>(c->num_sms) * occ, c->num_sms);
+    // one CTA per SM (the kernel takes piece = blockIdx.x and recomputes the cut points g U / G)
+    const HostSchedule hs = build_schedule(c->N, w.IB, w.TJ, c->num_sms, c->num_sms);
     w.B = hs.B, w.T = hs.T, w.U = hs.U, w.G = hs.G, w.max_slots = hs.max_slots;
     c->wcfg = w;
     c->w_smem = smem;
@@ -446,8 +430,8 @@ sd_status configure_w(sd_ctx* c) {
     SD_CUDA(c, cudaMemcpy(c->w_blk_first, hs.first.data(), sizeof(int) * w.B, cudaMemcpyHostToDevice));
     SD_CUDA(c, cudaMemcpy(c->w_blk_nslots, hs.nslots.data(), sizeof(int) * w.B, cudaMemcpyHostToDevice));
     SD_CUDA(c, cudaMemcpy(c->w_cta_piece, hs.piece.data(), sizeof(int) * w.G, cudaMemcpyHostToDevice));
-    std::vector<float4> pad(2 * sd::kWTJMax, make_float4(0.f, 0.f, 0.f, 0.f));
-    for (int q = 0; q < sd::kWTJMax; ++q) pad[q] = make_float4(SD_PAD_POS, SD_PAD_POS, SD_PAD_POS, 0.f);
+    std::vector<float4> pad(2 * sd::kWSJ, make_float4(0.f, 0.f, 0.f, 0.f));
+    for (int q = 0; q < sd::kWSJ; ++q) pad[q] = make_float4(SD_PAD_POS, SD_PAD_POS, SD_PAD_POS, 0.f);
     SD_CUDA(c, cudaMalloc(&c->w_pad, pad.size() * sizeof(float4)));
     SD_CUDA(c, cudaMemcpy(c->w_pad, pad.data(), pad.size() * sizeof(float4), cudaMemcpyHostToDevice));
     SD_CUDA(c, cudaMalloc(&c->grav_buf, nrec * sizeof(float4)));
@@ -980,15 +964,11 @@ sd_status sd_set_dispatch(sd_ctx* ctx, long long small_apply_max, int particles_
     return configure(ctx);
 }
 
-sd_status sd_set_jsplit(sd_ctx* ctx, int mode, int j_per_warp) {
+sd_status sd_set_jsplit(sd_ctx* ctx, int mode) {
     if (!ctx) return fail(nullptr, SD_ERR_INVALID_ARG, "sd_set_jsplit: ctx is NULL");
     if (mode < 0 || mode > 2) return fail(ctx, SD_ERR_INVALID_ARG, "sd_set_jsplit: mode must be 0, 1 or 2");
-    if (j_per_warp != 0 && j_per_warp != 8 && j_per_warp != 16 && j_per_warp != 32 && j_per_warp != 64 &&
-        j_per_warp != 128)
-        return fail(ctx, SD_ERR_INVALID_ARG, "sd_set_jsplit: j_per_warp must be 0, 8, 16, 32, 64 or 128");
     cudaDeviceSynchronize();
     ctx->jsplit = mode;
-    ctx->w_ch = j_per_warp;
     return configure(ctx);
 }
 

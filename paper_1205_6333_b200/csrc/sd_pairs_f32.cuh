@@ -129,12 +129,14 @@ __device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b) {
 // before the MUFUs, so that every pair -- the self pair and overlapping pairs included -- adds a
 // finite term of ordinary magnitude; the unclamped r^2 of every pair is returned in r2out and
 // the caller corrects the few pairs below the clamp.  Branch-free, 2 FMNMX per two pairs more.
-template <int I2, int TENSOR, bool PBC, bool CLAMP>
+// MNG: min r^2 is tracked per packed group in mng[m] instead of in the single mn (same number of
+// instructions; the warp-split kernel repairs only the groups that met a close pair).
+template <int I2, int TENSOR, bool PBC, bool CLAMP, bool MNG = false>
 __device__ __forceinline__ void pair_fast_staged(const f32x2 (&xi)[I2], const f32x2 (&yi)[I2],
                                                  const f32x2 (&zi)[I2], const float4 pj,
                                                  const float4 fj, const PairCoef& k,
                                                  f32x2 (&px)[I2], f32x2 (&py)[I2], f32x2 (&pz)[I2],
-                                                 float& mn, float (&r2out)[2 * I2]) {
+                                                 float& mn, float (&r2out)[2 * I2], float* mng = nullptr) {
     f32x2 dx[I2], dy[I2], dz[I2], r2[I2], inv[I2], inv2[I2], dF[I2], A[I2], Bd[I2];
     const f32x2 xj = bc2(pj.x), yj = bc2(pj.y), zj = bc2(pj.z);
     const f32x2 fx = bc2(fj.x), fy = bc2(fj.y), fz = bc2(fj.z);
@@ -171,7 +173,8 @@ __device__ __forceinline__ void pair_fast_staged(const f32x2 (&xi)[I2], const f3
             a = fmaxf(a, k.clampv);
             b = fmaxf(b, k.clampv);
         } else {
-            mn = fminf(mn, fminf(a, b));
+            if (MNG) mng[m] = fminf(mng[m], fminf(a, b));
+            else mn = fminf(mn, fminf(a, b));
         }
         inv[m] = pk2(rsq_approx(a), rsq_approx(b));
         inv2[m] = pk2(rcp_approx(a), rcp_approx(b));
@@ -302,75 +305,63 @@ __device__ __forceinline__ float self_clamped_coef(const int tensor, const float
 }
 
 // Repair of one chunk whose packed pass met a pair below the clamp (overlapping spheres,
-// coincident centres).  The fast body has then added a far-field term of enormous size to ONE
-// lane's sum of ONE particle; every other sum of the chunk is fine.  So nothing is redone for the
-// warp: each lane scans its 2 I2 particles for min r^2 over the chunk (self pair and pad records
-// excluded) and recomputes, with the exact branching body, only the chunk sums of the particles
-// that have such a pair -- about half the cost of one ordinary chunk pass, where redoing the
-// chunk with per-pair checks cost six to eight (the mid-N loss of round 1: at phi = 0.01 one
-// chunk pass in 50 is hit at N = 32768, one in 12 at N = 8192).
+// coincident centres).  The unclamped body has then added a far-field term of enormous size to the
+// sum of ONE particle; the other packed groups of the lane are fine.  Only the groups flagged in
+// `groups` (bit m) are redone: their chunk sum restarts from its base, every pair goes through the
+// clamped packed body for that one group (finite terms of ordinary size), and the pairs below the
+// clamp are put right one by one -- clamped term out, exact term in.  About a quarter of an
+// ordinary chunk pass per flagged group, where redoing the chunk for all groups with per-pair
+// checks cost six to eight passes (at phi = 0.01 one chunk pass in 6 is hit at N = 4096, one in 50
+// at N = 32768: the mid-N loss of round 1).
 //   cp / cf : positions / forces of the chunk's records, JS float4 apart from one j to the next
 //   ISTEP   : index distance between the particles of consecutive slots (m, half) of a lane
-//   thr     : k.thr after the unclamped body; k.clampv after the clamped body of a diagonal chunk
-//             (there every pair below the clamp was evaluated with the clamped r, Oseen included)
 // Convention kept for the epilogue: a self pair leaves the clamped term A_c F'_i in the sum.
-template <int I2, int TENSOR, int ACC, bool PBC, int CK, int JS, int ISTEP>
+template <int I2, int TENSOR, int ACC, bool PBC, int JS, int ISTEP>
 __device__ __forceinline__ void chunk_fix(const f32x2 (&xi)[I2], const f32x2 (&yi)[I2], const f32x2 (&zi)[I2],
-                                          const float4* cp, const float4* cf, const int j0, const int N,
-                                          const int i_first, const PairCoef& k, const float thr, f32x2 (&px)[I2],
-                                          f32x2 (&py)[I2], f32x2 (&pz)[I2], const f32x2 (&qx)[I2],
-                                          const f32x2 (&qy)[I2], const f32x2 (&qz)[I2]) {
-    const int nj = min(CK, N - j0);  // pad records (j >= N) hold no particle
+                                          const float4* cp, const float4* cf, const int j0, const int len,
+                                          const int N, const int i_first, const PairCoef& k,
+                                          const unsigned groups, f32x2 (&px)[I2], f32x2 (&py)[I2],
+                                          f32x2 (&pz)[I2], const f32x2 (&qx)[I2], const f32x2 (&qy)[I2],
+                                          const f32x2 (&qz)[I2]) {
 #pragma unroll
     for (int m = 0; m < I2; ++m) {
-        float nx[2], ny[2], nz[2];
-        bool redo[2];
-#pragma unroll
-        for (int h = 0; h < 2; ++h) {
-            const float x = h ? hi2(xi[m]) : lo2(xi[m]);
-            const float y = h ? hi2(yi[m]) : lo2(yi[m]);
-            const float z = h ? hi2(zi[m]) : lo2(zi[m]);
-            const int jself = i_first + (2 * m + h) * ISTEP - j0;  // position of the self pair in the chunk
-            float mnq = 3.0e38f;
-#pragma unroll 4
-            for (int jj = 0; jj < nj; ++jj) {
-                const float4 pj = cp[jj * JS];
-                float dx = x - pj.x, dy = y - pj.y, dz = z - pj.z;
-                if (PBC) {
-                    dx = __fmaf_rn(__fsub_rn(__fmaf_rn(dx, k.invL, k.magic), k.magic), k.mL, dx);
-                    dy = __fmaf_rn(__fsub_rn(__fmaf_rn(dy, k.invL, k.magic), k.magic), k.mL, dy);
-                    dz = __fmaf_rn(__fsub_rn(__fmaf_rn(dz, k.invL, k.magic), k.magic), k.mL, dz);
+        if (!((groups >> m) & 1u)) continue;
+        f32x2 x1[1] = {xi[m]}, y1[1] = {yi[m]}, z1[1] = {zi[m]};
+        f32x2 p1x[1], p1y[1], p1z[1];
+        p1x[0] = ACC == ACC_KAHAN ? bc2(0.f) : qx[m];
+        p1y[0] = ACC == ACC_KAHAN ? bc2(0.f) : qy[m];
+        p1z[0] = ACC == ACC_KAHAN ? bc2(0.f) : qz[m];
+        const int i0 = i_first + (2 * m) * ISTEP;
+        const float xa = lo2(xi[m]), ya = lo2(yi[m]), za = lo2(zi[m]);
+        const float xb = hi2(xi[m]), yb = hi2(yi[m]), zb = hi2(zi[m]);
+        float mnd = 0.f, r2p[2];
+#pragma unroll 2
+        for (int jj = 0; jj < len; ++jj) {
+            const float4 pj = cp[jj * JS];
+            const float4 fj = cf[jj * JS];
+            const int j = j0 + jj;
+            pair_fast_staged<1, TENSOR, PBC, true>(x1, y1, z1, pj, fj, k, p1x, p1y, p1z, mnd, r2p);
+            const bool fix0 = r2p[0] < k.clampv && j != i0;
+            const bool fix1 = r2p[1] < k.clampv && j != i0 + ISTEP;
+            if ((fix0 || fix1) && j < N) {
+                float ax = lo2(p1x[0]), ay = lo2(p1y[0]), az = lo2(p1z[0]);
+                float bx = hi2(p1x[0]), by = hi2(p1y[0]), bz = hi2(p1z[0]);
+                if (fix0) {
+                    pair_clamped_sub<TENSOR, PBC>(xa, ya, za, pj, fj, k, ax, ay, az);
+                    pair_exact<TENSOR, PBC>(xa, ya, za, false, pj, fj, k, ax, ay, az);
                 }
-                const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-                mnq = fminf(mnq, jj == jself ? 3.0e38f : r2);
-            }
-            redo[h] = mnq < thr;
-            nx[h] = ny[h] = nz[h] = 0.f;
-            if (redo[h]) {
-#pragma unroll 1
-                for (int jj = 0; jj < nj; ++jj) {
-                    const float4 pj = cp[jj * JS];
-                    const float4 fj = cf[jj * JS];
-                    if (jj == jself) {  // keep the convention: clamped self term
-                        const float ac = self_clamped_coef(TENSOR, k.clampv, k.k2);
-                        nx[h] = fmaf(ac, fj.x, nx[h]);
-                        ny[h] = fmaf(ac, fj.y, ny[h]);
-                        nz[h] = fmaf(ac, fj.z, nz[h]);
-                    } else {
-                        pair_exact<TENSOR, PBC>(x, y, z, false, pj, fj, k, nx[h], ny[h], nz[h]);
-                    }
+                if (fix1) {
+                    pair_clamped_sub<TENSOR, PBC>(xb, yb, zb, pj, fj, k, bx, by, bz);
+                    pair_exact<TENSOR, PBC>(xb, yb, zb, false, pj, fj, k, bx, by, bz);
                 }
+                p1x[0] = pk2(ax, bx);
+                p1y[0] = pk2(ay, by);
+                p1z[0] = pk2(az, bz);
             }
         }
-        if (redo[0] || redo[1]) {
-            // sums of the chunk so far: PLAIN carries the running sum (value at chunk start in q)
-            const float bx0 = ACC == ACC_KAHAN ? 0.f : lo2(qx[m]), bx1 = ACC == ACC_KAHAN ? 0.f : hi2(qx[m]);
-            const float by0 = ACC == ACC_KAHAN ? 0.f : lo2(qy[m]), by1 = ACC == ACC_KAHAN ? 0.f : hi2(qy[m]);
-            const float bz0 = ACC == ACC_KAHAN ? 0.f : lo2(qz[m]), bz1 = ACC == ACC_KAHAN ? 0.f : hi2(qz[m]);
-            px[m] = pk2(redo[0] ? bx0 + nx[0] : lo2(px[m]), redo[1] ? bx1 + nx[1] : hi2(px[m]));
-            py[m] = pk2(redo[0] ? by0 + ny[0] : lo2(py[m]), redo[1] ? by1 + ny[1] : hi2(py[m]));
-            pz[m] = pk2(redo[0] ? bz0 + nz[0] : lo2(pz[m]), redo[1] ? bz1 + nz[1] : hi2(pz[m]));
-        }
+        px[m] = p1x[0];
+        py[m] = p1y[0];
+        pz[m] = p1z[0];
     }
 }
 

@@ -6,15 +6,22 @@
 // (PAPER.md:239, :273), where the classic kernel needs 2048-particle i-blocks to run its best
 // inner loop and then has too few, too coarse work units for 148 SMs:
 //  * all 8 warps of a CTA own the SAME 32 * 2 I2 particles i (8 per lane with I2 = 4, the inner
-//    loop of the large-N kernel) and split every j tile between them: warp w takes the CH records
-//    [w CH, (w + 1) CH) of each tile of TJ = 8 CH.  An i-block is 256 particles instead of 2048,
-//    so N = 4096 already gives 16 x 32 units, and the per-unit tail (careful pass, diagonal tile)
-//    shrinks by the same factor;
+//    loop of the large-N kernel) and split the CTA's j range between them: the flattened
+//    (i-block, j) space is cut at a granularity of 4 j into one equal piece per SM ("stream-K"),
+//    and every warp takes an eighth of its CTA's piece -- the split is exact to 4 j per warp at
+//    any N.  An i-block is 256 particles instead of 2048, so the per-block tail (diagonal chunks,
+//    repairs) shrinks by the same factor;
+//  * every warp runs its own pipeline of bulk copies (cp.async.bulk + one mbarrier per stage,
+//    three 64-record sub-tiles in flight / in use per warp): no barrier is shared between warps
+//    inside a segment, a warp that repairs a chunk delays nobody;
+//  * the Kahan pairs (s, c) live in shared memory (touched once per 32 j), 48 registers less;
+//  * diagonal chunks run the clamped body branch-free and count exact zeros; a chunk that met a
+//    pair below the clamp repairs only the packed groups concerned (chunk_fix);
 //  * the warps' compensated sums are combined through shared memory in fp64 in warp order, and
 //    the CTA writes ONE (hi, lo) partial per particle and segment;
-//  * the kernel reads the caller's pos / force arrays directly (two bulk copies per tile into a
-//    tile laid out {TJ positions | TJ forces}; the ragged tail of the last tile comes from a
-//    context-owned block of pad records), works in the folded units of sd_common.cuh on the RAW
+//  * the kernel reads the caller's pos / force arrays directly (two bulk copies per sub-tile, laid
+//    out {64 positions | 64 forces}; the ragged tail of the system comes from a context-owned
+//    block of pad records), works in the folded units of sd_common.cuh on the RAW
 //    forces and multiplies by c1 = mu0 3a/4 at the very end;
 //  * the last CTA to deliver a partial of an i-block (a ticket counter per block; the sum itself
 //    runs over the slots in fixed order, so the result does not depend on who is last) adds the
@@ -28,8 +35,12 @@
 
 namespace sd {
 
-constexpr int kWTJMax = 1024;  // largest tile of this kernel: size of the pad block halves
-constexpr int kWMaxN = 6000;   // up to here the warp-split kernel runs by default (measured crossover)
+// Up to here the warp-split kernel runs by default (measured against the classic kernels, both
+// tensors, profiles/r02_mid_n.md: free space 17 % faster at N = 3000 and 4096, 7 % at 8192, 1-2 % up
+// to 20480, equal at 24576, 4 % slower at 32768; periodic box 17 % at 4096, 4 % at 8192, equal from
+// 12288 to 16384, 2-4 % slower above).
+constexpr int kWMaxN = 20480;
+constexpr int kWMaxNBox = 12288;
 
 // everything the fused epilogue needs
 struct FinArgs {
@@ -44,76 +55,70 @@ struct FinArgs {
     int pos_comp;
 };
 
-template <int I2, int CH>
+constexpr int kWQ = 4;        // schedule granule: j records per "quad" (= the unrolled loop body)
+constexpr int kWSJ = 64;      // j records per warp-private sub-tile (two compensation chunks)
+constexpr int kWStages = 3;   // sub-tiles per warp in flight / in use
+
+template <int I2>
 struct WShape {
-    static constexpr int TJ = kWarps * CH;
     static constexpr int IBW = 64 * I2;  // particles per i-block: 32 lanes x 2 I2
-    static constexpr size_t tile_bytes = static_cast<size_t>(kStages) * TJ * 2 * sizeof(float4);
+    static constexpr size_t tile_bytes = static_cast<size_t>(kWarps) * kWStages * kWSJ * 2 * sizeof(float4);
     static constexpr size_t red_bytes = static_cast<size_t>(kWarps) * 6 * IBW * sizeof(float);
     static constexpr size_t smem_bytes = tile_bytes + red_bytes;
 };
 
-template <int I2, int TENSOR, int ACC, bool PBC, int CH>
+#ifdef SD_W_TRACE  // per-CTA timeline for tuning; not part of the product build
+__device__ unsigned long long g_wtrace[1024 * 8];
+__device__ __forceinline__ void wtrace(const int slot) {
+    if (threadIdx.x == 0 && blockIdx.x < 1024) {
+        unsigned long long t;
+        asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+        g_wtrace[blockIdx.x * 8 + slot] = t;
+    }
+}
+#define SD_WTRACE(slot) wtrace(slot)
+#else
+#define SD_WTRACE(slot)
+#endif
+
+__device__ __forceinline__ void fence_proxy_async() {
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+
+template <int I2, int TENSOR, int ACC, bool PBC>
 __global__ void __launch_bounds__(kThreads, (I2 == 4) ? 1 : 2)
 pairs_f32w_kernel(const float4* __restrict__ pos, const float4* __restrict__ frc,
                   const float4* __restrict__ padblk, float4* __restrict__ part,
                   int* __restrict__ blk_done, const Schedule sch, const PairCoef k, const FinArgs fin,
                   const int N, const long long slot_stride) {
-    typedef WShape<I2, CH> W;
-    constexpr int TJ = W::TJ;
+    typedef WShape<I2> W;
     constexpr int IBW = W::IBW;
-    constexpr int CK = CH < kChunk ? CH : kChunk;  // j per compensation chunk
-    constexpr int NCH = CH / CK;                   // chunks per warp and tile
-    static_assert(CK % kUnrollJ == 0 && CH % CK == 0 && TJ <= kWTJMax, "tile shape");
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    float4* tiles = reinterpret_cast<float4*>(smem_raw);                  // [kStages][2 TJ]
     float* red = reinterpret_cast<float*>(smem_raw + W::tile_bytes);      // [kWarps][6][IBW]
-    __shared__ __align__(8) uint64_t full_bar[kStages];
-    __shared__ __align__(8) uint64_t empty_bar[kStages];
+    __shared__ __align__(8) uint64_t full_bar[kWarps][kWStages];
     __shared__ int s_last;
 
+    SD_WTRACE(0);
     const int tid = threadIdx.x;
     const int lane = tid & 31;
     const int warp = tid >> 5;
-    const int c = sch.cta_piece[blockIdx.x];
-    const long long u_begin = sch.cta_u0[c];
-    const long long u_end = sch.cta_u0[c + 1];
-    const int n_units = static_cast<int>(u_end - u_begin);
-    const int T = sch.T;
+    // this warp's private ring of sub-tiles, each laid out {kWSJ positions | kWSJ forces}
+    float4* wtiles = reinterpret_cast<float4*>(smem_raw) + static_cast<size_t>(warp) * (kWStages * 2 * kWSJ);
+    // one CTA per SM, piece = blockIdx.x; the cut points g U / G of build_schedule (sd_b200.cu) are
+    // recomputed here instead of loaded: two dependent global loads less before the first copy
+    const int c = blockIdx.x;
+    const int T = sch.T;  // quads per row of the (i-block, quad) grid
+    const long long U = static_cast<long long>(sch.B) * T;
+    const long long u_begin = static_cast<long long>(c) * U / sch.G;
+    const long long u_end = static_cast<long long>(c + 1) * U / sch.G;
 
-    if (tid == 0) {
-        for (int s = 0; s < kStages; ++s) {
-            mbar_init(&full_bar[s], 1);
-            mbar_init(&empty_bar[s], kWarps);
-        }
+    if (lane == 0) {
+        for (int s = 0; s < kWStages; ++s) mbar_init(&full_bar[warp][s], 1);
         mbar_fence_init();
     }
-    __syncthreads();
+    __syncwarp();
 
-    int pf_n = 0;
-    int pf_t = static_cast<int>(u_begin % T);
-    auto produce = [&]() {
-        const int s = pf_n % kStages;
-        const int q = pf_n / kStages;
-        if (q > 0) mbar_wait(&empty_bar[s], (q - 1) & 1);
-        float4* dst = tiles + static_cast<size_t>(s) * (2 * TJ);
-        const int j0 = pf_t * TJ;
-        const int valid = min(TJ, N - j0);
-        mbar_arrive_expect_tx(&full_bar[s], TJ * 32);
-        bulk_load(dst, pos + j0, valid * 16, &full_bar[s]);
-        bulk_load(dst + TJ, frc + j0, valid * 16, &full_bar[s]);
-        if (valid < TJ) {  // ragged tail: pad records (far away, zero force) complete the tile
-            bulk_load(dst + valid, padblk, (TJ - valid) * 16, &full_bar[s]);
-            bulk_load(dst + TJ + valid, padblk + kWTJMax, (TJ - valid) * 16, &full_bar[s]);
-        }
-        ++pf_n;
-        if (++pf_t == T) pf_t = 0;
-    };
-    if (tid == 0) {
-        for (int q = 0; q < kPrefetch && pf_n < n_units; ++q) produce();
-    }
-
-    int n = 0;
+    int wn = 0;  // sub-tiles this warp has consumed so far (ring position and barrier phase)
     long long u = u_begin;
     while (u < u_end) {
         const int b = static_cast<int>(u / T);
@@ -122,6 +127,33 @@ pairs_f32w_kernel(const float4* __restrict__ pos, const float4* __restrict__ frc
         const int nt = (left < static_cast<long long>(T - t0)) ? static_cast<int>(left) : (T - t0);
         const int i_blk = b * IBW;
         const int i_first = i_blk + lane;  // particle of (m = 0, half 0); the others follow in steps of 32
+        // this warp's share of the segment: a contiguous run of quads, the same number (+-1) for
+        // every warp: the split of the work is exact to 4 j per warp whatever N
+        const int per = (nt + kWarps - 1) / kWarps;
+        const int q_lo = min(t0 + warp * per, t0 + nt), q_hi = min(q_lo + per, t0 + nt);
+        const int j_lo = q_lo * kWQ, j_hi = q_hi * kWQ;      // records [j_lo, j_hi); those >= N are pads
+        const int nsub = (j_hi - j_lo + kWSJ - 1) / kWSJ;
+
+        auto produce = [&](const int ks) {  // lane 0: fetch sub-tile ks of this warp's run
+            const int s = (wn + ks) % kWStages;
+            float4* dst = wtiles + s * (2 * kWSJ);
+            const int j0 = j_lo + ks * kWSJ;
+            const int cnt = min(kWSJ, j_hi - j0);
+            const int valid = max(0, min(cnt, N - j0));
+            fence_proxy_async();  // the generic-proxy reads of the stage's previous tenant are done
+            mbar_arrive_expect_tx(&full_bar[warp][s], cnt * 32);
+            if (valid > 0) {
+                bulk_load(dst, pos + j0, valid * 16, &full_bar[warp][s]);
+                bulk_load(dst + kWSJ, frc + j0, valid * 16, &full_bar[warp][s]);
+            }
+            if (valid < cnt) {  // ragged tail of the system: pad records (far away, zero force)
+                bulk_load(dst + valid, padblk, (cnt - valid) * 16, &full_bar[warp][s]);
+                bulk_load(dst + kWSJ + valid, padblk + kWSJ, (cnt - valid) * 16, &full_bar[warp][s]);
+            }
+        };
+        if (lane == 0) {
+            for (int ks = 0; ks < kWStages - 1 && ks < nsub; ++ks) produce(ks);
+        }
 
         f32x2 xi[I2], yi[I2], zi[I2];
 #pragma unroll
@@ -136,25 +168,35 @@ pairs_f32w_kernel(const float4* __restrict__ pos, const float4* __restrict__ frc
             yi[m] = add2(pk2(p0.y, p1.y), zero);
             zi[m] = add2(pk2(p0.z, p1.z), zero);
         }
-        f32x2 sx[I2], sy[I2], sz[I2], cx[I2], cy[I2], cz[I2];
+        // The Kahan pairs (s, c) of the lane's particles live in shared memory, in the very array
+        // the cross-warp combine reads afterwards: they are touched once per chunk of 32 j, and 48
+        // registers less in the hot loop is what keeps it free of spills and copies.  Element
+        // (warp, component, m, lane) is one f32x2 = the two particles of packed group m.
+        f32x2* kst = reinterpret_cast<f32x2*>(red) + (warp * 6) * (IBW / 2) + lane;
         f32x2 px[I2], py[I2], pz[I2];
 #pragma unroll
         for (int m = 0; m < I2; ++m) {
-            sx[m] = sy[m] = sz[m] = cx[m] = cy[m] = cz[m] = bc2(0.f);
+#pragma unroll
+            for (int comp = 0; comp < 6; ++comp) kst[comp * (IBW / 2) + 32 * m] = bc2(0.f);
             px[m] = py[m] = pz[m] = bc2(0.f);
         }
 
 #pragma unroll 1
-        for (int tt = 0; tt < nt; ++tt, ++n) {
-            const int s = n % kStages;
-            if (tid == 0 && pf_n < n_units) produce();
-            mbar_wait(&full_bar[s], (n / kStages) & 1);
+        for (int ks = 0; ks < nsub; ++ks) {
+            const int s = (wn + ks) % kWStages;
+            __syncwarp();
+            if (lane == 0 && ks + kWStages - 1 < nsub) produce(ks + kWStages - 1);
+            mbar_wait(&full_bar[warp][s], ((wn + ks) / kWStages) & 1);
+            if (ks == 0 && u == u_begin) SD_WTRACE(1);
+            const float4* tp = wtiles + s * (2 * kWSJ);
+            const int jt = j_lo + ks * kWSJ;
+            const int cnt = min(kWSJ, j_hi - jt);
 #pragma unroll 1
-            for (int ch = 0; ch < NCH; ++ch) {
-            // this warp's share of the tile: CH consecutive records = NCH compensation chunks
-            const float4* cp = tiles + static_cast<size_t>(s) * (2 * TJ) + warp * CH + ch * CK;  // positions
-            const float4* cf = cp + TJ;                                                          // forces
-            const int j0 = (t0 + tt) * TJ + warp * CH + ch * CK;
+            for (int c0 = 0; c0 < cnt; c0 += kChunk) {
+            const int len = min(kChunk, cnt - c0);      // records of this compensation chunk (multiple of 4)
+            const float4* cp = tp + c0;                 // positions
+            const float4* cf = cp + kWSJ;               // forces
+            const int j0 = jt + c0;
             f32x2 qx[I2], qy[I2], qz[I2];
 #pragma unroll
             for (int m = 0; m < I2; ++m) {
@@ -166,78 +208,100 @@ pairs_f32w_kernel(const float4* __restrict__ pos, const float4* __restrict__ frc
                     qz[m] = pz[m];
                 }
             }
-            float mn = 3.0e38f;
+            float mn = 3.0e38f;  // unused: min r^2 is tracked per packed group
+            float mng[I2];
+#pragma unroll
+            for (int m = 0; m < I2; ++m) mng[m] = 3.0e38f;
             float r2v[2 * I2];
             // does this chunk hold self pairs (j = i) of the warp's particles?
-            const bool diag = (j0 + CK > i_blk) && (j0 < i_blk + IBW);
-            bool fix;
+            const bool diag = (j0 + len > i_blk) && (j0 < i_blk + IBW);
+            unsigned groups = 0u;  // packed groups whose chunk sum has to be repaired
             if (!diag) {
+                if (len == kChunk) {  // the common case, with a compile-time trip count
 #pragma unroll kUnrollJ
-                for (int jj = 0; jj < CK; ++jj) {
-                    const float4 pj = cp[jj];
-                    const float4 fj = cf[jj];
-                    pair_fast_staged<I2, TENSOR, PBC, false>(xi, yi, zi, pj, fj, k, px, py, pz, mn, r2v);
+                    for (int jj = 0; jj < kChunk; ++jj) {
+                        const float4 pj = cp[jj];
+                        const float4 fj = cf[jj];
+                        pair_fast_staged<I2, TENSOR, PBC, false, true>(xi, yi, zi, pj, fj, k, px, py, pz, mn,
+                                                                       r2v, mng);
+                    }
+                } else {
+#pragma unroll 1
+                    for (int jq = 0; jq < len; jq += kWQ) {
+#pragma unroll
+                        for (int jj = 0; jj < kWQ; ++jj) {
+                            const float4 pj = cp[jq + jj];
+                            const float4 fj = cf[jq + jj];
+                            pair_fast_staged<I2, TENSOR, PBC, false, true>(xi, yi, zi, pj, fj, k, px, py, pz,
+                                                                           mn, r2v, mng);
+                        }
+                    }
                 }
-                fix = mn < k.thr;
+#pragma unroll
+                for (int m = 0; m < I2; ++m) groups |= (mng[m] < k.thr ? 1u : 0u) << m;
             } else {
                 // diagonal chunk: the clamped body, branch-free (a self pair adds the finite term
                 // A_c F'_i that the epilogue removes).  It is exact unless a pair other than the
-                // self pairs lies below the clamp: min r^2 over the pairs with r^2 > 0, and the
-                // number of exact zeros against the number of self pairs this lane meets here.
+                // self pairs lies below the clamp: min r^2 per group over the pairs with r^2 > 0,
+                // and the number of exact zeros against the number of self pairs this lane meets.
                 int zeros = 0;
-#pragma unroll kUnrollJ
-                for (int jj = 0; jj < CK; ++jj) {
-                    const float4 pj = cp[jj];
-                    const float4 fj = cf[jj];
-                    pair_fast_staged<I2, TENSOR, PBC, true>(xi, yi, zi, pj, fj, k, px, py, pz, mn, r2v);
+#pragma unroll 1
+                for (int jq = 0; jq < len; jq += kWQ) {
 #pragma unroll
-                    for (int q = 0; q < 2 * I2; ++q) {
-                        const bool z = r2v[q] == 0.f;
-                        zeros += z ? 1 : 0;
-                        mn = fminf(mn, z ? 3.0e38f : r2v[q]);
+                    for (int jj = 0; jj < kWQ; ++jj) {
+                        const float4 pj = cp[jq + jj];
+                        const float4 fj = cf[jq + jj];
+                        pair_fast_staged<I2, TENSOR, PBC, true>(xi, yi, zi, pj, fj, k, px, py, pz, mn, r2v);
+#pragma unroll
+                        for (int q = 0; q < 2 * I2; ++q) {
+                            const bool z = r2v[q] == 0.f;
+                            zeros += z ? 1 : 0;
+                            mng[q / 2] = fminf(mng[q / 2], z ? 3.0e38f : r2v[q]);
+                        }
                     }
                 }
-                const int rel = j0 - i_blk;  // >= 0 here; this chunk holds the particles rel ... rel + CK - 1 of the block
-                const int off = rel & 31;
-                const bool mine = rel >= 0 && lane >= off && lane < off + CK && (i_first + (rel - off)) < N;
-                fix = mn < k.clampv || zeros != (mine ? 1 : 0);
+                // the lane's particles are i_first + 32 q: at most one of them lies in [j0, j0 + len)
+                const int first = j0 > i_first ? i_first + ((j0 - i_first + 31) & ~31) : i_first;
+                const bool mine = first < j0 + len && first < i_blk + IBW && first < N;
+#pragma unroll
+                for (int m = 0; m < I2; ++m) groups |= (mng[m] < k.clampv ? 1u : 0u) << m;
+                if (zeros != (mine ? 1 : 0)) groups = (1u << I2) - 1u;  // coincident centres: all groups
             }
-            if (fix)  // rare: repair the sums of the particles that have a pair below the clamp here
-                chunk_fix<I2, TENSOR, ACC, PBC, CK, 1, 32>(xi, yi, zi, cp, cf, j0, N, i_first, k,
-                                                           diag ? k.clampv : k.thr, px, py, pz, qx, qy, qz);
+            if (groups)  // rare: repair the chunk sums of the groups that met a pair below the clamp
+                chunk_fix<I2, TENSOR, ACC, PBC, 1, 32>(xi, yi, zi, cp, cf, j0, len, N, i_first, k, groups, px,
+                                                       py, pz, qx, qy, qz);
             if (ACC == ACC_KAHAN) {
 #pragma unroll
                 for (int m = 0; m < I2; ++m) {
-                    kahan_merge2(sx[m], cx[m], px[m]);
-                    kahan_merge2(sy[m], cy[m], py[m]);
-                    kahan_merge2(sz[m], cz[m], pz[m]);
+                    f32x2* e = kst + 32 * m;
+                    f32x2 s0 = e[0 * (IBW / 2)], s1 = e[1 * (IBW / 2)], s2 = e[2 * (IBW / 2)];
+                    f32x2 c0k = e[3 * (IBW / 2)], c1k = e[4 * (IBW / 2)], c2k = e[5 * (IBW / 2)];
+                    kahan_merge2(s0, c0k, px[m]);
+                    kahan_merge2(s1, c1k, py[m]);
+                    kahan_merge2(s2, c2k, pz[m]);
+                    e[0 * (IBW / 2)] = s0, e[1 * (IBW / 2)] = s1, e[2 * (IBW / 2)] = s2;
+                    e[3 * (IBW / 2)] = c0k, e[4 * (IBW / 2)] = c1k, e[5 * (IBW / 2)] = c2k;
                 }
             }
             }  // chunks
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&empty_bar[s]);
         }
+        wn += nsub;
+        if (u == u_begin) SD_WTRACE(2);
 
         // ---- combine the warps' sums (fp64, warp order): one (hi, lo) partial per particle ----
+        if (ACC == ACC_PLAIN) {  // the running sums are the result; compensation words stay 0
 #pragma unroll
-        for (int m = 0; m < I2; ++m) {
-            if (ACC == ACC_PLAIN) {
-                sx[m] = px[m];
-                sy[m] = py[m];
-                sz[m] = pz[m];
+            for (int m = 0; m < I2; ++m) {
+                kst[0 * (IBW / 2) + 32 * m] = px[m];
+                kst[1 * (IBW / 2) + 32 * m] = py[m];
+                kst[2 * (IBW / 2) + 32 * m] = pz[m];
             }
-            float* r0 = red + (warp * 6) * IBW + 64 * m + lane;  // [warp][component][particle]
-            r0[0 * IBW] = lo2(sx[m]), r0[0 * IBW + 32] = hi2(sx[m]);
-            r0[1 * IBW] = lo2(sy[m]), r0[1 * IBW + 32] = hi2(sy[m]);
-            r0[2 * IBW] = lo2(sz[m]), r0[2 * IBW + 32] = hi2(sz[m]);
-            r0[3 * IBW] = lo2(cx[m]), r0[3 * IBW + 32] = hi2(cx[m]);
-            r0[4 * IBW] = lo2(cy[m]), r0[4 * IBW + 32] = hi2(cy[m]);
-            r0[5 * IBW] = lo2(cz[m]), r0[5 * IBW + 32] = hi2(cz[m]);
         }
         __syncthreads();
         const int slot = c - sch.blk_first_cta[b];
         const int nslots = sch.blk_nslots[b];
-        const int i_mine = i_blk + tid;  // the particle this thread reduces (tid < IBW)
+        // float t of a component row belongs to packed group t / 64, lane (t % 64) / 2, half t % 2
+        const int i_mine = i_blk + 64 * (tid >> 6) + 32 * (tid & 1) + ((tid & 63) >> 1);  // tid < IBW
         double vx = 0.0, vy = 0.0, vz = 0.0;
         if (tid < IBW) {
 #pragma unroll
@@ -248,6 +312,7 @@ pairs_f32w_kernel(const float4* __restrict__ pos, const float4* __restrict__ frc
                 vz += static_cast<double>(r0[2 * IBW]) - static_cast<double>(r0[5 * IBW]);
             }
         }
+        if (u == u_begin) SD_WTRACE(3);
         bool last = true;
         if (nslots > 1) {
             if (tid < IBW && i_mine < N) {
@@ -264,6 +329,7 @@ pairs_f32w_kernel(const float4* __restrict__ pos, const float4* __restrict__ frc
             __syncthreads();
             last = s_last != 0;
         }
+        if (u == u_begin) SD_WTRACE(4);
         // ---- the CTA that delivered the last partial of this i-block finishes its rows ----------
         if (last) {
             if (nslots > 1) {
@@ -322,8 +388,10 @@ pairs_f32w_kernel(const float4* __restrict__ pos, const float4* __restrict__ frc
             }
         }
         __syncthreads();  // `red` and `s_last` are reused by the next segment
+        if (u == u_begin) SD_WTRACE(5);
         u += nt;
     }
+    SD_WTRACE(6);
 }
 
 }  // namespace sd

@@ -38,7 +38,7 @@ SYMBOLS = {
                                ctypes.POINTER(_I), ctypes.POINTER(_I), ctypes.POINTER(_I)]),
     "sd_set_dispatch": (_I, [_P, _LL, _I]),
     "sd_set_staging": (_I, [_P, _I]),
-    "sd_set_jsplit": (_I, [_P, _I, _I]),
+    "sd_set_jsplit": (_I, [_P, _I]),
     "sd_set_box": (_I, [_P, _D]),
     "sd_box": (_D, [_P]),
     "sd_mobility_apply": (_I, [_P, _P, _P, _P, _P]),
@@ -174,9 +174,9 @@ class Context:
         self._check(self._lib.sd_set_dispatch(self._h, int(small_apply_max),
                                               int(particles_per_thread)))
 
-    def set_jsplit(self, mode: int = 0, j_per_warp: int = 0):
+    def set_jsplit(self, mode: int = 0):
         """0 automatic, 1 classic tiled kernels only, 2 warp-split one-launch kernel wherever it exists."""
-        self._check(self._lib.sd_set_jsplit(self._h, int(mode), int(j_per_warp)))
+        self._check(self._lib.sd_set_jsplit(self._h, int(mode)))
 
     def set_staging(self, mode: int):
         """Memory-access ablation (Appendix A): 0 bulk copies, 1 naive, 2 tiled + barriers."""

@@ -1,6 +1,6 @@
 """GPU parity of the warp-split one-launch kernel (sd_pairs_f32w.cuh; north_star: "splits j across
-warps"; SURVEY 8(a) a1-a6 in one launch) against the CPU oracle, through the C ABI.  `sd_set_jsplit(2, ch)`
-forces it at any N with `ch` records per warp and tile; by default it runs for N up to a few
+warps"; SURVEY 8(a) a1-a6 in one launch) against the CPU oracle, through the C ABI.  `sd_set_jsplit(2)`
+forces it at any N; by default it runs for N up to a few
 thousand.  Tolerances: north_star's 1e-5 on max_i |v_gpu,i - v_ref,i| / |v_ref,i| (fp32-Kahan)."""
 import numpy as np
 import pytest
@@ -46,16 +46,15 @@ def dense_cloud(n, seed):
     return pos
 
 
-@pytest.mark.parametrize("ch", [8, 16, 32, 64, 128])
 @pytest.mark.parametrize("prec_name", ["PREC_F32_KAHAN", "PREC_F32_PLAIN"])
 @pytest.mark.parametrize("tname", ["rpy", "oseen"])
 @pytest.mark.parametrize("boxed", [False, True])
-def test_dense_clouds_all_rows(gpu, ch, prec_name, tname, boxed):
-    """Every tile shape x tensor x accumulation x boundary condition on dense clouds, all rows:
-    N = 257 (two i-blocks, one of them a single particle), 3000 and 5003 (ragged last tile, pad
-    records, several CTAs per i-block: the last-arriver epilogue)."""
+def test_dense_clouds_all_rows(gpu, prec_name, tname, boxed):
+    """Tensor x accumulation x boundary condition on dense clouds, all rows: N = 257 (two i-blocks,
+    one of them a single particle; most warps without work), 3000, 5003 and 9999 (ragged tails, pad
+    records, several CTAs per i-block: the last-arriver epilogue; warp shares of every length)."""
     torch, sd = gpu
-    for n in (257, 3000, 5003):
+    for n in (257, 3000, 5003, 9999):
         pos = dense_cloud(n, wl.SEED_BASE + 40 + n)
         force = wl.normal_forces(n, wl.SEED_BASE + 41 + n)
         L = 1.01 * wl.cube_side(n, 0.2) if boxed else 0.0
@@ -65,7 +64,7 @@ def test_dense_clouds_all_rows(gpu, ch, prec_name, tname, boxed):
         ctx.set_tensor(TENSOR[tname][0])
         ctx.set_box(L)
         ctx.set_dispatch(0, 0)
-        ctx.set_jsplit(2, ch)
+        ctx.set_jsplit(2)
         assert "_w8_" in ctx.kernel_name, ctx.kernel_name
         dp, df = torch.from_numpy(p).cuda(), torch.from_numpy(f).cuda()
         out = []
@@ -82,21 +81,19 @@ def test_dense_clouds_all_rows(gpu, ch, prec_name, tname, boxed):
             continue  # Eq. (4) at overlapping centres through a face: fp32 displacement error, B6
         want = orc.apply(p64, f64, wl.A, wl.ETA, TENSOR[tname][1], box=float(np.float32(L)),
                          image=orc.IMAGE_F32 if boxed else orc.IMAGE_DEFINITION)
-        assert rel_err(out[0][:, :3].astype(np.float64), want) <= TOL[prec_name], (n, ch)
+        assert rel_err(out[0][:, :3].astype(np.float64), want) <= TOL[prec_name], n
         ctx.close()
 
 
-@pytest.mark.parametrize("ch", [0, 32, 128])
-@pytest.mark.parametrize("n", [4096, 70001])
-def test_config5_cloud_sampled_rows(gpu, ch, n):
+@pytest.mark.parametrize("n", [4096, 70001, 300007])
+def test_config5_cloud_sampled_rows(gpu, n):
     """The sweep cloud (phi = 0.01, overlaps allowed): default dispatch at N = 4096 is this kernel;
     N = 70001 forced (several i-blocks per CTA, ragged tail), 4096 seeded rows."""
     torch, sd = gpu
     pos, force = wl.sweep(n)
     p, f = wl.to_xyzw(pos, np.float32), wl.to_xyzw(force, np.float32)
     ctx = sd.Context(n, wl.A, wl.ETA)
-    if ch or n > 6000:
-        ctx.set_jsplit(2, ch)
+    ctx.set_jsplit(2)
     assert "_w8_" in ctx.kernel_name, ctx.kernel_name
     dp, df = torch.from_numpy(p).cuda(), torch.from_numpy(f).cuda()
     dv = torch.full_like(dp, float("nan"))
@@ -126,7 +123,7 @@ def test_step_through_the_one_launch_kernel(gpu, n, integ, boxed, forces):
     steps, dt = 3, 0.01
     ctx = sd.Context(n, wl.A, wl.ETA)
     ctx.set_box(L)
-    ctx.set_jsplit(2, 0)
+    ctx.set_jsplit(2)
     assert "_w8_" in ctx.kernel_name
     dp, df = torch.from_numpy(p).cuda(), torch.from_numpy(f).cuda()
     gi = sd.INT_EULER if integ == "euler" else sd.INT_MIDPOINT
@@ -159,9 +156,9 @@ def test_jsplit_argument_validation(gpu):
     assert "_w8_" in ctx.kernel_name               # default at this N
     ctx.set_jsplit(1)
     assert "_w8_" not in ctx.kernel_name
-    for bad in ((3, 0), (-1, 0), (2, 12), (2, 256)):
+    for bad in (3, -1):
         with pytest.raises(sd.SdError):
-            ctx.set_jsplit(*bad)
+            ctx.set_jsplit(bad)
     ctx.set_precision(sd.PREC_F64)                 # fp64 has no warp-split kernel: classic path
     ctx.set_jsplit(2)
     assert "f64" in ctx.kernel_name
