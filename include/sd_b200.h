@@ -22,7 +22,14 @@
  *    written as 0 on output.  Records must be 16-byte aligned (32 bytes for double).
  *  - Unless the name ends in `_host`, data pointers are DEVICE pointers owned by the caller.
  *    The context owns every scratch buffer (packed particle records, partial sums, midpoint
- *    positions, position low words); nothing is allocated on the hot path.
+ *    positions, position low words), allocated by sd_create and by the setters that change the
+ *    kernel variant.  Two lazily allocated exceptions, both on first use and never inside a
+ *    stream capture: the device staging of sd_mobility_apply_host (3 N records) and the cell
+ *    grid of the lubrication step above 2560 particles.  Nothing else is allocated by
+ *    sd_mobility_apply / sd_step / sd_lubrication_apply.
+ *  - Calls must be made with the CUDA device the context was created on as the current device
+ *    (SD_ERR_INVALID_ARG otherwise).  After a setter failed with SD_ERR_ALLOC / SD_ERR_CUDA the
+ *    context refuses work until a setter succeeds again; its settings are kept.
  *  - `stream` is a cudaStream_t passed as void* (NULL = default stream).  Calls only enqueue
  *    work; they do not synchronise the host, except sd_create, sd_destroy and the `_host`
  *    variants (which return after their result has landed in host memory).
@@ -57,7 +64,10 @@ typedef enum {
 
 typedef enum {
     SD_PREC_F32_KAHAN = 0, /* fp32 terms, compensated accumulation; default */
-    SD_PREC_F64 = 1,       /* everything in fp64 */
+    SD_PREC_F64 = 1,       /* fp64 terms and sums.  1/r is a 22-bit MUFU.RSQ seed on the fp32 copy of r^2
+                            * plus one Newton step in fp64: relative error <= 8.6e-14 per pair (not
+                            * correctly rounded; 1e-11 on the row sums is the tested bound), and r^2
+                            * must lie in the fp32 range (|r| between 1e-19 and 1e19) */
     SD_PREC_F32_PLAIN = 2  /* fp32 terms, plain fp32 accumulation: ablation of PAPER.md:253-263 */
 } sd_precision;
 
@@ -77,49 +87,6 @@ sd_status sd_create(sd_ctx** out, long long N, double a, double eta);
  * last product; every other setter keeps them (the lubrication correction reads them). */
 sd_status sd_set_tensor(sd_ctx* ctx, sd_tensor tensor);
 sd_status sd_set_precision(sd_ctx* ctx, sd_precision precision);
-
-/* The static work schedule of the tiled kernels, as a pure host function (no GPU needed; the
- * library builds its own schedules with the same code).  The (i-block, j-tile) units u = b T + t,
- * B = ceil(N / particles_per_block) blocks x T = ceil(N / tile_j) tiles, are cut into
- * G = min(B T, max_ctas) contiguous pieces of equal size +-1: piece g owns units
- * [cta_u0[g], cta_u0[g+1]).  Block b collects the partial sums of pieces blk_first[b] ...
- * blk_first[b] + blk_nslots[b] - 1.  CTA x works on piece cta_piece[x]; the CTAs x, x + num_sms,
- * x + 2 num_sms, ... (which share an SM) own consecutive pieces.  dims receives {B, T, G,
- * max slots per block}; the arrays (host; sizes G+1, G, B, B) may be NULL, call once with NULL
- * arrays to learn the sizes. */
-sd_status sd_schedule_plan(long long N, int particles_per_block, int tile_j, long long max_ctas,
-                           int num_sms, long long* cta_u0, int* cta_piece, int* blk_first,
-                           int* blk_nslots, int* dims);
-
-/* Dispatch knobs of the small-N path (PAPER.md:239: below a few thousand particles the device is
- * under-filled), for ablations and tests; the defaults are the measured crossovers.
- *   small_apply_max     : N up to which one product is ONE launch of the warp-per-particle kernel
- *                         (no pack / partial sums / finalize); < 0 restores the default.
- *   particles_per_thread: 2, 4 or 8 particles i per thread in the tiled kernels (fp64: half of
- *                         it); 0 = automatic (by N).
- * Reallocates the scratch buffers; synchronises the device. */
-sd_status sd_set_dispatch(sd_ctx* ctx, long long small_apply_max, int particles_per_thread);
-
-/* How the j sum of one particle is split (north_star: "splits j across warps"), fp32 modes, above
- * the small-N path:
- *   mode 0  automatic: the warp-split one-launch kernel up to a measured N, the classic kernels above
- *   mode 1  classic only: the 8 warps of a CTA own different particles and share every j tile; j is
- *           split across CTAs; pack / pair / finalize kernels
- *   mode 2  warp-split wherever it exists: the 8 warps of a CTA own the same 256 particles and take
- *           an eighth of the CTA's j range each (their own bulk-copy pipelines), sums combined
- *           through shared memory, the last CTA of an i-block finishes its rows: one launch
- * Reallocates the scratch buffers; synchronises the device. */
-sd_status sd_set_jsplit(sd_ctx* ctx, int mode);
-
-/* Ablation of the memory-access schemes the paper compares (PAPER.md:111-241 and Appendix A): how
- * the j records reach the threads of the tiled kernel.
- *   0  bulk asynchronous copies into a ring of shared-memory tiles (default, the product path)
- *   1  "naive" (Alg. 1): every thread loads each record from global memory, one address per warp
- *   2  "tiling" (Alg. 2): the block copies a tile into shared memory between two barriers
- * Modes 1 and 2 exist for SD_TENSOR_RPY + SD_PREC_F32_KAHAN in free space only; otherwise, and
- * for any later change away from that combination, SD_ERR_UNSUPPORTED is returned and the context
- * is left unchanged.  Results are bit-identical across modes. */
-sd_status sd_set_staging(sd_ctx* ctx, int mode);
 
 /* Boundary conditions (footnote 1: "a simulation box with periodic boundaries and
  * include only hydrodynamic interactions from the nearest image of each particle").
@@ -167,9 +134,10 @@ sd_status sd_step(sd_ctx* ctx, void* pos, sd_force_fn fn, void* user, const void
  * paper never lets spheres touch); coincident centres contribute nothing.  F^ext is f_ext[N][4]
  * or, when f_ext is NULL, the uniform force gravity[3] (NULL: zero).  pos, vel, f_ext, force_out
  * are device arrays of the context's element type; force_out may be f_ext, not pos or vel.  The
- * neighbour search is a hashed cell grid rebuilt on every call (context-owned, allocated on first
- * use); results do not depend on thread scheduling.  With sd_set_box the nearest image is used
- * and the box side must be at least 9a (SD_ERR_UNSUPPORTED otherwise).  The cut-off is decided in
+ * neighbour search tests all pairs in one launch up to 2560 particles and uses a hashed cell grid
+ * rebuilt on every call above that (context-owned, allocated on first use); results do not
+ * depend on thread scheduling.  With sd_set_box the nearest image is used and the box side must
+ * exceed 6a (9a for the cell grid), SD_ERR_UNSUPPORTED otherwise.  The cut-off is decided in
  * the context's arithmetic, the accepted pairs are evaluated in fp64. */
 sd_status sd_lubrication_apply(sd_ctx* ctx, const void* pos, const void* vel, const void* f_ext,
                                const double gravity[3], void* force_out, void* stream);
@@ -186,13 +154,6 @@ sd_status sd_set_velocity(sd_ctx* ctx, const void* vel, void* stream);
 /* Copy the velocities of the last product into vel_out[N][4] (device). */
 sd_status sd_get_velocity(sd_ctx* ctx, void* vel_out, void* stream);
 
-/* Ablation of PAPER.md:253-263 ("single or double-single precision for ... (b) positions in the
- * Euler integration"): on = 1 (default) carries positions as (hi, lo) float pairs in the fp32
- * modes; on = 0 keeps them in plain fp32, r <- fl32(r + h v), low words held at zero.  No effect
- * in SD_PREC_F64.  The accumulation of the velocities, (a) in the paper, is selected by
- * sd_set_precision (SD_PREC_F32_KAHAN / SD_PREC_F32_PLAIN). */
-sd_status sd_set_position_compensation(sd_ctx* ctx, int on);
-
 /* Forget the position low words (call after editing pos between sd_step calls). */
 sd_status sd_reset_compensation(sd_ctx* ctx, void* stream);
 
@@ -200,6 +161,65 @@ sd_status sd_reset_compensation(sd_ctx* ctx, void* stream);
 long long sd_num_particles(const sd_ctx* ctx);
 double sd_self_mobility(const sd_ctx* ctx); /* mu0 = 1/(6 pi eta a) */
 double sd_box(const sd_ctx* ctx);           /* side of the periodic cube, 0 in free space */
+
+const char* sd_last_error(const sd_ctx* ctx);
+void sd_destroy(sd_ctx* ctx);
+
+/* =====================================================================================
+ * Diagnostics, ablations and tuning knobs.  NOT needed to use the library: the calls above are
+ * the product ABI.  What follows serves the tests, bench.py and the paper's
+ * ablation experiments; defaults are the measured optima.
+ * ===================================================================================== */
+
+/* The static work schedule of the tiled kernels, as a pure host function (no GPU needed; the
+ * library builds its own schedules with the same code).  The (i-block, j-tile) units u = b T + t,
+ * B = ceil(N / particles_per_block) blocks x T = ceil(N / tile_j) tiles, are cut into
+ * G = min(B T, max_ctas) contiguous pieces of equal size +-1: piece g owns units
+ * [cta_u0[g], cta_u0[g+1]).  Block b collects the partial sums of pieces blk_first[b] ...
+ * blk_first[b] + blk_nslots[b] - 1.  CTA x works on piece cta_piece[x]; the CTAs x, x + num_sms,
+ * x + 2 num_sms, ... (which share an SM) own consecutive pieces.  dims receives {B, T, G,
+ * max slots per block}; the arrays (host; sizes G+1, G, B, B) may be NULL, call once with NULL
+ * arrays to learn the sizes. */
+sd_status sd_schedule_plan(long long N, int particles_per_block, int tile_j, long long max_ctas,
+                           int num_sms, long long* cta_u0, int* cta_piece, int* blk_first,
+                           int* blk_nslots, int* dims);
+
+/* Dispatch knobs of the small-N path (PAPER.md:239: below a few thousand particles the device is
+ * under-filled), for ablations and tests; the defaults are the measured crossovers.
+ *   small_apply_max     : N up to which one product is ONE launch of the warp-per-particle kernel
+ *                         (no pack / partial sums / finalize); < 0 restores the default.
+ *   particles_per_thread: 2, 4 or 8 particles i per thread in the tiled kernels (fp64: half of
+ *                         it); 0 = automatic (by N).
+ * Reallocates the scratch buffers; synchronises the device. */
+sd_status sd_set_dispatch(sd_ctx* ctx, long long small_apply_max, int particles_per_thread);
+
+/* How the j sum of one particle is split (north_star: "splits j across warps"), fp32 modes, above
+ * the small-N path:
+ *   mode 0  automatic: the warp-split one-launch kernel up to a measured N, the classic kernels above
+ *   mode 1  classic only: the 8 warps of a CTA own different particles and share every j tile; j is
+ *           split across CTAs; pack / pair / finalize kernels
+ *   mode 2  warp-split wherever it exists: the 8 warps of a CTA own the same 256 particles and take
+ *           an eighth of the CTA's j range each (their own bulk-copy pipelines), sums combined
+ *           through shared memory, the last CTA of an i-block finishes its rows: one launch
+ * Reallocates the scratch buffers; synchronises the device. */
+sd_status sd_set_jsplit(sd_ctx* ctx, int mode);
+
+/* Ablation of the memory-access schemes the paper compares (PAPER.md:111-241 and Appendix A): how
+ * the j records reach the threads of the tiled kernel.
+ *   0  bulk asynchronous copies into a ring of shared-memory tiles (default, the product path)
+ *   1  "naive" (Alg. 1): every thread loads each record from global memory, one address per warp
+ *   2  "tiling" (Alg. 2): the block copies a tile into shared memory between two barriers
+ * Modes 1 and 2 exist for SD_TENSOR_RPY + SD_PREC_F32_KAHAN in free space only; otherwise, and
+ * for any later change away from that combination, SD_ERR_UNSUPPORTED is returned and the context
+ * is left unchanged.  Results are bit-identical across modes. */
+sd_status sd_set_staging(sd_ctx* ctx, int mode);
+
+/* Ablation of PAPER.md:253-263 ("single or double-single precision for ... (b) positions in the
+ * Euler integration"): on = 1 (default) carries positions as (hi, lo) float pairs in the fp32
+ * modes; on = 0 keeps them in plain fp32, r <- fl32(r + h v), low words held at zero.  No effect
+ * in SD_PREC_F64.  The accumulation of the velocities, (a) in the paper, is selected by
+ * sd_set_precision (SD_PREC_F32_KAHAN / SD_PREC_F32_PLAIN). */
+sd_status sd_set_position_compensation(sd_ctx* ctx, int on);
 
 /* Number of kernel launches enqueued by this context since creation (bench bookkeeping). */
 long long sd_launch_count(const sd_ctx* ctx);
@@ -235,8 +255,6 @@ sd_status sd_fma_peak_probe(sd_ctx* ctx, sd_precision precision, double* tflops_
 sd_status sd_access_bench(int elem_floats, int pattern, int scheme, long long N, int reps,
                           const void* in, void* out, double* ms_per_launch, void* stream);
 
-const char* sd_last_error(const sd_ctx* ctx);
-void sd_destroy(sd_ctx* ctx);
 
 #ifdef __cplusplus
 }

@@ -75,7 +75,7 @@ struct sd_ctx {
     void* lub_spos = nullptr;        // [N] positions, velocities, cells in bucket order
     void* lub_svel = nullptr;
     int4* lub_scell = nullptr;
-    void* lub_tmp = nullptr;         // cub scan scratch
+    void* lub_tmp = nullptr;         // block totals of the bucket scan
     size_t lub_tmp_bytes = 0;
     unsigned lub_H = 0;
     // CUDA graph of kGraphSteps steps of the full loop (constant forces + lubrication)
@@ -141,6 +141,24 @@ sd_status fail(sd_ctx* ctx, sd_status code, const std::string& msg) {
         if (e_ != cudaSuccess)                                                             \
             return fail(ctx, e_ == cudaErrorMemoryAllocation ? SD_ERR_ALLOC : SD_ERR_CUDA, \
                         std::string(#call) + ": " + cudaGetErrorString(e_));               \
+    } while (0)
+
+// Every entry point that touches the device: the context must be usable and the caller's current
+// device must be the one the context was created on (its buffers and streams live there).
+sd_status enter(sd_ctx* c, const char* who) {
+    if (!c->valid)
+        return fail(c, SD_ERR_INVALID_ARG, std::string(who) + ": the context is unusable after a failed "
+                    "reconfiguration (" + c->err + "); call a setter that succeeds, or destroy it");
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != c->device)
+        return fail(c, SD_ERR_INVALID_ARG, std::string(who) + ": the current CUDA device is not the one the "
+                    "context was created on (cudaSetDevice first)");
+    return SD_OK;
+}
+#define SD_ENTER(ctx, who)                      \
+    do {                                        \
+        sd_status e_ = enter(ctx, who);         \
+        if (e_ != SD_OK) return e_;             \
     } while (0)
 
 template <int I2, int TENSOR, int ACC, bool PBC, int TJ = sd::kTJ>
@@ -245,20 +263,49 @@ HostSchedule build_schedule(long long N, int IB, int TJ, long long max_ctas, int
 
 sd_status configure_w(sd_ctx* c);
 
+// The packed one-launch kernel keeps all N records in dynamic shared memory (up to 72 KiB): the
+// opt-in is per device and per function, so every context sets it for the instantiation it will
+// launch, outside any stream capture, and checks the result.
+sd_status set_packed_attr(sd_ctx* c) {
+    if (c->precision == SD_PREC_F64 || c->N < sd::kPackedMinN || c->N > sd::kPackedMaxN) return SD_OK;
+    const bool rpy = c->tensor == SD_TENSOR_RPY, kahan = c->precision != SD_PREC_F32_PLAIN, pbc = c->box > 0.0;
+    const void* f = nullptr;
+#define SD_PKF(T, K, P) reinterpret_cast<const void*>(&sd::small_apply_packed_kernel<T, K, P>)
+    if (rpy) f = kahan ? (pbc ? SD_PKF(0, true, true) : SD_PKF(0, true, false))
+                       : (pbc ? SD_PKF(0, false, true) : SD_PKF(0, false, false));
+    else f = kahan ? (pbc ? SD_PKF(1, true, true) : SD_PKF(1, true, false))
+                   : (pbc ? SD_PKF(1, false, true) : SD_PKF(1, false, false));
+#undef SD_PKF
+    SD_CUDA(c, cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, sd::kPackedMaxN * 32));
+    return SD_OK;
+}
+
 // Pick the kernel variant for (N, precision, tensor), build the static schedule and
 // (re)allocate every scratch buffer.
 sd_status configure(sd_ctx* c) {
     // the velocities of the last product survive a reconfiguration that keeps their element type
     // (sd_set_box, sd_set_tensor, sd_set_dispatch, ...): the lubrication correction needs them
+    {
+        int dev = -1;
+        if (cudaGetDevice(&dev) != cudaSuccess || dev != c->device)
+            return fail(c, SD_ERR_INVALID_ARG, "the current CUDA device is not the one the context was created on");
+    }
+    // ... and so do the low words of the positions (a change of tensor, box or dispatch in the
+    // middle of a run must not drop them)
     void* keep_vel = nullptr;
+    void* keep_lo = nullptr;
     const size_t vel_bytes = static_cast<size_t>(c->Nrec) * 4 * elem_size(c->precision);
     if (c->vel && c->vel_bytes == vel_bytes) {
         keep_vel = c->vel;
         c->vel = nullptr;
+        keep_lo = c->pos_lo;
+        c->pos_lo = nullptr;
     }
+    const bool lo_was_valid = c->lo_valid;
     free_buffers(c);
     c->valid = false;  // until every buffer below exists again
     c->vel = keep_vel;
+    c->pos_lo = keep_lo;
     Config cfg;
     const bool f64 = c->precision == SD_PREC_F64;
     const bool rpy = c->tensor == SD_TENSOR_RPY;
@@ -358,11 +405,12 @@ sd_status configure(sd_ctx* c) {
         SD_CUDA(c, cudaMemset(c->vel, 0, nrec * v4));
         c->vel_bytes = nrec * v4;
     }
-    SD_CUDA(c, cudaMalloc(&c->pos_lo, nrec * v4));
+    const bool fresh_lo = c->pos_lo == nullptr;
+    if (fresh_lo) SD_CUDA(c, cudaMalloc(&c->pos_lo, nrec * v4));
     SD_CUDA(c, cudaMalloc(&c->pos_half, nrec * v4));
     SD_CUDA(c, cudaMalloc(&c->pos_alt, nrec * v4));
     SD_CUDA(c, cudaMalloc(&c->force_buf, nrec * v4));
-    SD_CUDA(c, cudaMemset(c->pos_lo, 0, nrec * v4));
+    if (fresh_lo) SD_CUDA(c, cudaMemset(c->pos_lo, 0, nrec * v4));
     SD_CUDA(c, cudaMalloc(&c->d_cta_u0, sizeof(long long) * (cfg.G + 1)));
     SD_CUDA(c, cudaMalloc(&c->d_blk_first, sizeof(int) * cfg.B));
     SD_CUDA(c, cudaMalloc(&c->d_blk_nslots, sizeof(int) * cfg.B));
@@ -371,12 +419,16 @@ sd_status configure(sd_ctx* c) {
     SD_CUDA(c, cudaMemcpy(c->d_cta_u0, u0.data(), sizeof(long long) * (cfg.G + 1), cudaMemcpyHostToDevice));
     SD_CUDA(c, cudaMemcpy(c->d_blk_first, first.data(), sizeof(int) * cfg.B, cudaMemcpyHostToDevice));
     SD_CUDA(c, cudaMemcpy(c->d_blk_nslots, nslots.data(), sizeof(int) * cfg.B, cudaMemcpyHostToDevice));
-    c->lo_valid = true;  // zeroed
+    c->lo_valid = fresh_lo ? true : lo_was_valid;  // fresh words are zero; kept ones keep their state
     // mid N in the fp32 modes: the whole product in one launch of the warp-split kernel
     if (!f64 && c->staging == sd::STAGE_BULK && c->N > c->small_apply_max &&
         (c->jsplit == 2 || (c->jsplit == 0 && c->N <= (pbc ? sd::kWMaxNBox : sd::kWMaxN)))) {
         sd_status ws = configure_w(c);
         if (ws != SD_OK) return ws;
+    }
+    {
+        sd_status ps = set_packed_attr(c);
+        if (ps != SD_OK) return ps;
     }
     c->valid = true;
     return SD_OK;
@@ -658,13 +710,7 @@ void launch_small_packed_k(sd_ctx* c, const void* posx, const void* force, const
     const int per_cta = (sd::kPackedThreads / 32) * 2;
     const int blocks = (n + per_cta - 1) / per_cta;
     const double gx = g ? g[0] : 0.0, gy = g ? g[1] : 0.0, gz = g ? g[2] : 0.0;
-    const size_t smem = static_cast<size_t>(n) * 32;
-    static bool attr_set = false;  // once per instantiation: up to 80 KiB of dynamic shared memory
-    if (!attr_set) {
-        cudaFuncSetAttribute(sd::small_apply_packed_kernel<TENSOR, KAHAN, PBC>,
-                             cudaFuncAttributeMaxDynamicSharedMemorySize, sd::kPackedMaxN * 32);
-        attr_set = true;
-    }
+    const size_t smem = static_cast<size_t>(n) * 32;  // opt-in above 48 KiB: set_packed_attr, at configure time
     sd::small_apply_packed_kernel<TENSOR, KAHAN, PBC><<<blocks, sd::kPackedThreads, smem, st>>>(
         static_cast<const float4*>(posx), static_cast<const float4*>(force), gx, gy, gz,
         static_cast<float4*>(vel), static_cast<const float4*>(pos_base), static_cast<float4*>(c->pos_lo),
@@ -741,22 +787,21 @@ sd_status launch_stepper(sd_ctx* c, void* pos, const void* force, const double g
 
 // cell-grid scratch of the lubrication step (allocated on first use, never inside a stream capture)
 sd_status ensure_lub_buffers(sd_ctx* c) {
-    if (!c->lub_cell) {
-        const int n = static_cast<int>(c->N);
-        cudaStream_t st = nullptr;
-        unsigned H = 512;  // 2^(3 bits) buckets, at least one per particle
-        while (H < static_cast<unsigned>(n)) H <<= 3;
-        c->lub_H = H;
-        SD_CUDA(c, cudaMalloc(&c->lub_spos, 4 * elem_size(c->precision) * n));
-        SD_CUDA(c, cudaMalloc(&c->lub_svel, 4 * elem_size(c->precision) * n));
-        SD_CUDA(c, cudaMalloc(&c->lub_scell, sizeof(int4) * n));
-        SD_CUDA(c, cudaMalloc(&c->lub_cell, sizeof(int4) * n));
-        SD_CUDA(c, cudaMalloc(&c->lub_count, sizeof(unsigned) * (H + 1)));
-        SD_CUDA(c, cudaMalloc(&c->lub_start, sizeof(unsigned) * (H + 1)));
-        SD_CUDA(c, cudaMalloc(&c->lub_cursor, sizeof(unsigned) * H));
-        SD_CUDA(c, cudaMalloc(&c->lub_order, sizeof(int) * n));
-        SD_CUDA(c, cub::DeviceScan::ExclusiveSum(nullptr, c->lub_tmp_bytes, c->lub_count, c->lub_start,
-                                                 static_cast<int>(H + 1), st));
+    const int n = static_cast<int>(c->N);
+    unsigned H = 512;  // 2^(3 bits) buckets, at least one per particle
+    while (H < static_cast<unsigned>(n)) H <<= 3;
+    c->lub_H = H;
+    // every buffer on its own: after a failed allocation the next call allocates what is missing
+    if (!c->lub_spos) SD_CUDA(c, cudaMalloc(&c->lub_spos, 4 * elem_size(c->precision) * n));
+    if (!c->lub_svel) SD_CUDA(c, cudaMalloc(&c->lub_svel, 4 * elem_size(c->precision) * n));
+    if (!c->lub_scell) SD_CUDA(c, cudaMalloc(&c->lub_scell, sizeof(int4) * n));
+    if (!c->lub_cell) SD_CUDA(c, cudaMalloc(&c->lub_cell, sizeof(int4) * n));
+    if (!c->lub_count) SD_CUDA(c, cudaMalloc(&c->lub_count, sizeof(unsigned) * (H + 1)));
+    if (!c->lub_start) SD_CUDA(c, cudaMalloc(&c->lub_start, sizeof(unsigned) * (H + 1)));
+    if (!c->lub_cursor) SD_CUDA(c, cudaMalloc(&c->lub_cursor, sizeof(unsigned) * H));
+    if (!c->lub_order) SD_CUDA(c, cudaMalloc(&c->lub_order, sizeof(int) * n));
+    if (!c->lub_tmp) {  // block totals of the two-launch scan
+        c->lub_tmp_bytes = sizeof(unsigned) * ((H + 1 + sd::kScanBlock - 1) / sd::kScanBlock);
         SD_CUDA(c, cudaMalloc(&c->lub_tmp, c->lub_tmp_bytes));
     }
     return SD_OK;
@@ -778,8 +823,13 @@ sd_status launch_lubrication(sd_ctx* c, const void* pos, const void* vel, const 
             grid.invL = 1.0 / grid.L;
         }
         grid.nc = static_cast<int>(std::floor(grid.L / (3.0 * c->a)));
-        if (grid.nc < 3)
-            return fail(c, SD_ERR_UNSUPPORTED, "lubrication in a periodic box needs a box side of at least 9 a");
+        // a pair inside 3a must have ONE nearest image: L > 6a; the cell grid probes 27 distinct
+        // cells and needs three of them per edge: L >= 9a
+        if (grid.nc < 2 || !(grid.L > 6.0 * c->a))
+            return fail(c, SD_ERR_UNSUPPORTED, "lubrication in a periodic box needs a box side above 6 a");
+        if (grid.nc < 3 && n > sd::kLubSmallMax)
+            return fail(c, SD_ERR_UNSUPPORTED,
+                        "lubrication in a periodic box needs a box side of at least 9 a above 2560 particles (cell grid)");
         grid.nc = std::min(grid.nc, 1024);
     }
     if (n <= sd::kLubSmallMax) {  // small systems: all pairs in one launch, no cell grid
@@ -809,6 +859,7 @@ sd_status launch_lubrication(sd_ctx* c, const void* pos, const void* vel, const 
     SD_CUDA(c, cudaMemsetAsync(c->lub_count, 0, sizeof(unsigned) * (H + 1), st));
     SD_CUDA(c, cudaMemsetAsync(c->lub_cursor, 0, sizeof(unsigned) * H, st));
     const int nb = (n + 255) / 256;
+    const unsigned nscan = (H + 1 + sd::kScanBlock - 1) / sd::kScanBlock;
     const double gx = g ? g[0] : 0.0, gy = g ? g[1] : 0.0, gz = g ? g[2] : 0.0;
     sd_status s;
 #define SD_LUB_FORCE_ARGS(T4)                                                                       \
@@ -819,8 +870,11 @@ sd_status launch_lubrication(sd_ctx* c, const void* pos, const void* vel, const 
     sd::lub_count_kernel<T4><<<nb, 256, 0, st>>>(static_cast<const T4*>(pos), c->lub_cell,          \
                                                  c->lub_count, grid, n);                           \
     if ((s = check_launch(c, "lub_count_kernel")) != SD_OK) return s;                               \
-    SD_CUDA(c, cub::DeviceScan::ExclusiveSum(c->lub_tmp, c->lub_tmp_bytes, c->lub_count,            \
-                                             c->lub_start, static_cast<int>(H + 1), st));          \
+    sd::lub_scan_totals_kernel<<<nscan, 256, 0, st>>>(c->lub_count, static_cast<unsigned*>(c->lub_tmp), H + 1); \
+    if ((s = check_launch(c, "lub_scan_totals_kernel")) != SD_OK) return s;                         \
+    sd::lub_scan_apply_kernel<<<nscan, 256, 0, st>>>(c->lub_count, static_cast<const unsigned*>(c->lub_tmp), \
+                                                     c->lub_start, H + 1);                         \
+    if ((s = check_launch(c, "lub_scan_apply_kernel")) != SD_OK) return s;                          \
     sd::lub_scatter_kernel<<<nb, 256, 0, st>>>(c->lub_cell, c->lub_start, c->lub_cursor,            \
                                                c->lub_order, n);                                   \
     if ((s = check_launch(c, "lub_scatter_kernel")) != SD_OK) return s;                             \
@@ -1015,6 +1069,7 @@ sd_status sd_set_box(sd_ctx* ctx, double box_side) {
 
 sd_status sd_mobility_apply(sd_ctx* ctx, const void* pos, const void* force, void* vel, void* stream) {
     if (!ctx) return fail(nullptr, SD_ERR_INVALID_ARG, "sd_mobility_apply: ctx is NULL");
+    SD_ENTER(ctx, "sd_mobility_apply");
     if (!pos || !force || !vel) return fail(ctx, SD_ERR_INVALID_ARG, "sd_mobility_apply: NULL pointer");
     const size_t al = 4 * elem_size(ctx->precision);
     if (misaligned(pos, al) || misaligned(force, al) || misaligned(vel, al))
@@ -1033,6 +1088,7 @@ sd_status sd_mobility_apply(sd_ctx* ctx, const void* pos, const void* force, voi
 sd_status sd_mobility_apply_host(sd_ctx* ctx, const void* pos_host, const void* force_host,
                                  void* vel_host, void* stream) {
     if (!ctx) return fail(nullptr, SD_ERR_INVALID_ARG, "sd_mobility_apply_host: ctx is NULL");
+    SD_ENTER(ctx, "sd_mobility_apply_host");
     if (!pos_host || !force_host || !vel_host)
         return fail(ctx, SD_ERR_INVALID_ARG, "sd_mobility_apply_host: NULL pointer");
     const size_t bytes = static_cast<size_t>(ctx->N) * 4 * elem_size(ctx->precision);
@@ -1055,6 +1111,7 @@ sd_status sd_step(sd_ctx* ctx, void* pos, sd_force_fn fn, void* user, const void
                   const double gravity[3], double dt, long long n_steps, sd_integrator integrator,
                   void* stream) {
     if (!ctx) return fail(nullptr, SD_ERR_INVALID_ARG, "sd_step: ctx is NULL");
+    SD_ENTER(ctx, "sd_step");
     if (!pos) return fail(ctx, SD_ERR_INVALID_ARG, "sd_step: pos is NULL");
     if (!fn && !force && !gravity) return fail(ctx, SD_ERR_INVALID_ARG, "sd_step: no force given");
     if (!std::isfinite(dt)) return fail(ctx, SD_ERR_INVALID_ARG, "sd_step: dt is not finite");
@@ -1207,6 +1264,7 @@ sd_status sd_set_lubrication(sd_ctx* ctx, int on) {
 
 sd_status sd_set_velocity(sd_ctx* ctx, const void* vel, void* stream) {
     if (!ctx) return fail(nullptr, SD_ERR_INVALID_ARG, "sd_set_velocity: ctx is NULL");
+    SD_ENTER(ctx, "sd_set_velocity");
     const size_t bytes = static_cast<size_t>(ctx->N) * 4 * elem_size(ctx->precision);
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     if (vel) SD_CUDA(ctx, cudaMemcpyAsync(ctx->vel, vel, bytes, cudaMemcpyDeviceToDevice, st));
@@ -1217,6 +1275,7 @@ sd_status sd_set_velocity(sd_ctx* ctx, const void* vel, void* stream) {
 sd_status sd_lubrication_apply(sd_ctx* ctx, const void* pos, const void* vel, const void* f_ext,
                                const double gravity[3], void* force_out, void* stream) {
     if (!ctx) return fail(nullptr, SD_ERR_INVALID_ARG, "sd_lubrication_apply: ctx is NULL");
+    SD_ENTER(ctx, "sd_lubrication_apply");
     if (!pos || !vel || !force_out) return fail(ctx, SD_ERR_INVALID_ARG, "sd_lubrication_apply: NULL pointer");
     const size_t al = 4 * elem_size(ctx->precision);
     if (misaligned(pos, al) || misaligned(vel, al) || misaligned(force_out, al) || (f_ext && misaligned(f_ext, al)))
@@ -1229,6 +1288,7 @@ sd_status sd_lubrication_apply(sd_ctx* ctx, const void* pos, const void* vel, co
 
 sd_status sd_get_velocity(sd_ctx* ctx, void* vel_out, void* stream) {
     if (!ctx) return fail(nullptr, SD_ERR_INVALID_ARG, "sd_get_velocity: ctx is NULL");
+    SD_ENTER(ctx, "sd_get_velocity");
     if (!vel_out) return fail(ctx, SD_ERR_INVALID_ARG, "sd_get_velocity: vel_out is NULL");
     const size_t bytes = static_cast<size_t>(ctx->N) * 4 * elem_size(ctx->precision);
     SD_CUDA(ctx, cudaMemcpyAsync(vel_out, ctx->vel, bytes, cudaMemcpyDeviceToDevice,
@@ -1238,6 +1298,7 @@ sd_status sd_get_velocity(sd_ctx* ctx, void* vel_out, void* stream) {
 
 sd_status sd_reset_compensation(sd_ctx* ctx, void* stream) {
     if (!ctx) return fail(nullptr, SD_ERR_INVALID_ARG, "sd_reset_compensation: ctx is NULL");
+    SD_ENTER(ctx, "sd_reset_compensation");
     const size_t bytes = static_cast<size_t>(ctx->Nrec) * 4 * elem_size(ctx->precision);
     SD_CUDA(ctx, cudaMemsetAsync(ctx->pos_lo, 0, bytes, static_cast<cudaStream_t>(stream)));
     ctx->lo_valid = true;
@@ -1284,6 +1345,7 @@ sd_status sd_profile_read(sd_ctx* ctx, double* pair_kernel_ms, long long* pair_k
 
 sd_status sd_fma_peak_probe(sd_ctx* ctx, sd_precision precision, double* tflops_out, void* stream) {
     if (!ctx) return fail(nullptr, SD_ERR_INVALID_ARG, "sd_fma_peak_probe: ctx is NULL");
+    SD_ENTER(ctx, "sd_fma_peak_probe");
     if (!tflops_out) return fail(ctx, SD_ERR_INVALID_ARG, "sd_fma_peak_probe: tflops_out is NULL");
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     const int threads = 512, blocks = ctx->num_sms * 4, iters = 4096;

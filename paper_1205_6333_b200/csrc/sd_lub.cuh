@@ -9,7 +9,8 @@
 // call, no host synchronisation, deterministic:
 //   lub_count_kernel    cell (3 ints, side >= 3a) and bucket (Morton code of the cell's low bits,
 //                       H = 8^k >= N buckets) of every particle; bucket histogram by atomicAdd
-//   exclusive scan      cub::DeviceScan over the H counters (library primitive, plumbing)
+//   lub_scan_*_kernel   exclusive scan of the H counters in two launches (block totals, then every
+//                       block adds the totals before it to its own scan)
 //   lub_scatter_kernel  particle indices into their buckets (atomic cursor), then
 //   lub_sort_kernel     each bucket sorted by particle index: the summation order below, and
 //                       with it every bit of the result, does not depend on the atomics
@@ -28,8 +29,6 @@
 // required), neighbour cells wrap, displacements take the nearest image by the rule of the pair
 // kernels.
 #pragma once
-#include <cub/device/device_scan.cuh>
-
 #include "sd_common.cuh"
 #include "sd_stream.cuh"
 
@@ -90,6 +89,72 @@ lub_scatter_kernel(const int4* __restrict__ cell, const unsigned* __restrict__ s
     if (i >= N) return;
     const unsigned h = static_cast<unsigned>(cell[i].w);
     order[start[h] + atomicAdd(&cursor[h], 1u)] = i;
+}
+
+// Exclusive scan of n counters, two launches, blocks of kScanBlock elements (256 threads x 8):
+// A writes every block's total; B sums the totals of the blocks before it (at most n / 2048
+// values, read by all threads of the block) and scans its own elements on top of that.
+constexpr int kScanBlock = 2048;
+
+__device__ __forceinline__ unsigned lub_block_exclusive(unsigned v, unsigned* warp_sums, unsigned& total) {
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    unsigned inc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const unsigned t = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += t;
+    }
+    if (lane == 31) warp_sums[w] = inc;
+    __syncthreads();
+    unsigned base = 0;
+    total = 0;
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {
+        const unsigned ws = warp_sums[q];
+        if (q < w) base += ws;
+        total += ws;
+    }
+    __syncthreads();
+    return base + inc - v;
+}
+
+__global__ void __launch_bounds__(256)
+lub_scan_totals_kernel(const unsigned* __restrict__ count, unsigned* __restrict__ totals, const unsigned n) {
+    __shared__ unsigned warp_sums[8];
+    const unsigned b0 = blockIdx.x * kScanBlock + threadIdx.x * 8;
+    unsigned v = 0;
+#pragma unroll
+    for (int q = 0; q < 8; ++q) v += (b0 + q < n) ? count[b0 + q] : 0u;
+    unsigned total;
+    lub_block_exclusive(v, warp_sums, total);
+    if (threadIdx.x == 0) totals[blockIdx.x] = total;
+}
+
+__global__ void __launch_bounds__(256)
+lub_scan_apply_kernel(const unsigned* __restrict__ count, const unsigned* __restrict__ totals,
+                      unsigned* __restrict__ start, const unsigned n) {
+    __shared__ unsigned warp_sums[8];
+    __shared__ unsigned s_prefix;
+    unsigned pre = 0;
+    for (unsigned k = threadIdx.x; k < blockIdx.x; k += 256) pre += totals[k];
+    unsigned dummy;
+    const unsigned ex = lub_block_exclusive(pre, warp_sums, dummy);
+    if (threadIdx.x == 255) s_prefix = ex + pre;
+    __syncthreads();
+    const unsigned prefix = s_prefix;
+    const unsigned b0 = blockIdx.x * kScanBlock + threadIdx.x * 8;
+    unsigned c[8], v = 0;
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {
+        c[q] = (b0 + q < n) ? count[b0 + q] : 0u;
+        v += c[q];
+    }
+    unsigned run = prefix + lub_block_exclusive(v, warp_sums, dummy);
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {
+        if (b0 + q < n) start[b0 + q] = run;
+        run += c[q];
+    }
 }
 
 // one thread per bucket: insertion sort by particle index (buckets hold a handful of particles)

@@ -82,3 +82,4 @@ def test_gpu_access_kernels_bit_exact(elem, n):
             want = orc.access_sums(d, pattern, scheme)
             assert want.max() < 2 ** 24                       # every partial sum is exact in fp32
             np.testing.assert_array_equal(out.cpu().numpy().astype(np.float64), want)
+

@@ -133,17 +133,35 @@ def test_lubrication_apply_against_the_plain_definition(gpu, prec_name, tol, box
     ctx.close()
 
 
-def test_lubrication_needs_a_box_of_nine_radii(gpu):
+@pytest.mark.parametrize("prec_name,tol", [("PREC_F32_KAHAN", 2e-7), ("PREC_F64", 1e-12)])
+def test_lubrication_box_side_limits(gpu, prec_name, tol):
+    """A pair inside 3a must have one nearest image: the box side has to exceed 6a.  The all-pairs
+    kernel (N <= 2560) works from there on -- checked against the plain definition in a box of 7a,
+    where most pairs interact through a face -- the cell grid above that size needs 9a."""
     torch, sd = gpu
-    ctx = sd.Context(8, wl.A, wl.ETA)
-    ctx.set_box(8.5)
-    z = torch.zeros((8, 4), device="cuda")
-    with pytest.raises(sd.SdError) as e:
-        ctx.lubrication_apply(z, z.clone(), z.clone())
-    assert e.value.status == sd.ERR_UNSUPPORTED
-    ctx.set_box(9.5)
-    ctx.lubrication_apply(z, z.clone(), z.clone())
+    dt = _dt(prec_name)
+    n = 40
+    ctx = sd.Context(n, wl.A, wl.ETA)
+    ctx.set_precision(getattr(sd, prec_name))
+    z = torch.zeros((n, 4), device="cuda", dtype=torch.float64 if dt == np.float64 else torch.float32)
+    for bad in (5.5, 6.0):
+        ctx.set_box(bad)
+        with pytest.raises(sd.SdError) as e:
+            ctx.lubrication_apply(z, z.clone(), z.clone())
+        assert e.value.status == sd.ERR_UNSUPPORTED
+    L = 7.0
+    ctx.set_box(L)
+    pos = wl.rsa_cube(n, 4.0 / 3.0 * np.pi * n / L ** 3, wl.SEED_BASE + 340)   # fills the box of side L
+    near = guards.pairs_in_shell(pos, 3.0 - GUARD, 3.0 + GUARD, L)
+    assert near.shape[0] == 0
+    vel = wl.normal_forces(n, wl.SEED_BASE + 341)
+    p, v = wl.to_xyzw(pos, dt), wl.to_xyzw(vel, dt)
+    out = torch.empty_like(z)
+    ctx.lubrication_apply(torch.from_numpy(p).cuda(), torch.from_numpy(v).cuda(), out, gravity=(0.0, 0.0, -1.0))
     torch.cuda.synchronize()
+    corr = orc.lubrication(p[:, :3].astype(np.float64), v[:, :3].astype(np.float64), wl.A, wl.ETA, box=L)
+    assert np.count_nonzero(np.abs(corr).sum(axis=1)) > n // 2
+    assert _row_err(out.cpu().numpy()[:, :3].astype(np.float64), np.array([0.0, 0.0, -1.0]) - corr) <= tol
     ctx.close()
 
 
