@@ -19,6 +19,7 @@
 #include "sd_pairs_f32.cuh"
 #include "sd_pairs_f64.cuh"
 #include "sd_pairs_f32w.cuh"
+#include "sd_pairs_f64w.cuh"
 #include "sd_access.cuh"
 #include "sd_lub.cuh"
 #include "sd_small.cuh"
@@ -161,9 +162,15 @@ sd_status enter(sd_ctx* c, const char* who) {
         if (e_ != SD_OK) return e_;             \
     } while (0)
 
-template <int I2, int TENSOR, int ACC, bool PBC, int TJ = sd::kTJ>
+template <int I2, int TENSOR, int ACC, bool PBC, int TJ = sd::kTJ, int REPAIR = 1>
 const void* f32_kernel() {
-    return reinterpret_cast<const void*>(&sd::pairs_f32_kernel<I2, TENSOR, ACC, PBC, sd::STAGE_BULK, TJ>);
+    return reinterpret_cast<const void*>(&sd::pairs_f32_kernel<I2, TENSOR, ACC, PBC, sd::STAGE_BULK, TJ, REPAIR>);
+}
+// 8 particles per thread at N >= kRepairMaxN: the round-1 careful pass (see sd_pairs_f32.cuh)
+template <bool PBC>
+const void* f32_pick_large(bool rpy, bool plain) {
+    return rpy ? (plain ? f32_kernel<4, 0, 1, PBC, sd::kTJ, 0>() : f32_kernel<4, 0, 0, PBC, sd::kTJ, 0>())
+               : (plain ? f32_kernel<4, 1, 1, PBC, sd::kTJ, 0>() : f32_kernel<4, 1, 0, PBC, sd::kTJ, 0>());
 }
 template <int I, int TENSOR, bool PBC>
 const void* f64_kernel() {
@@ -336,7 +343,9 @@ sd_status configure(sd_ctx* c) {
              {{"pairs_f32x2_i8_oseen_kahan", "pairs_f32x2_i8_oseen_kahan_pbc"},
               {"pairs_f32x2_i8_oseen_plain", "pairs_f32x2_i8_oseen_plain_pbc"}}}};
         cfg.name = names[i2 == 4 ? 2 : (i2 == 2 ? 1 : 0)][rpy ? 0 : 1][plain ? 1 : 0][pbc ? 1 : 0];
-        if (i2 == 4)
+        if (i2 == 4 && c->N >= sd::kRepairMaxN)
+            cfg.kernel = pbc ? f32_pick_large<true>(rpy, plain) : f32_pick_large<false>(rpy, plain);
+        else if (i2 == 4)
             cfg.kernel = pbc ? f32_pick<4, true>(rpy, plain) : f32_pick<4, false>(rpy, plain);
         else if (i2 == 2)
             cfg.kernel = pbc ? f32_pick<2, true>(rpy, plain) : f32_pick<2, false>(rpy, plain);
@@ -349,13 +358,16 @@ sd_status configure(sd_ctx* c) {
                 return fail(c, SD_ERR_UNSUPPORTED,
                             "staging ablation exists for RPY, fp32-Kahan, free space only: call sd_set_staging(ctx, 0) first");
             const bool naive = c->staging == sd::STAGE_NAIVE;
-#define SD_STAGED_T(I2V, TJV)                                                                       \
-    (naive ? reinterpret_cast<const void*>(&sd::pairs_f32_kernel<I2V, 0, 0, false, sd::STAGE_NAIVE, TJV>) \
-           : reinterpret_cast<const void*>(&sd::pairs_f32_kernel<I2V, 0, 0, false, sd::STAGE_SYNC, TJV>))
+#define SD_STAGED_R(I2V, TJV, RV)                                                                   \
+    (naive ? reinterpret_cast<const void*>(&sd::pairs_f32_kernel<I2V, 0, 0, false, sd::STAGE_NAIVE, TJV, RV>) \
+           : reinterpret_cast<const void*>(&sd::pairs_f32_kernel<I2V, 0, 0, false, sd::STAGE_SYNC, TJV, RV>))
+#define SD_STAGED_T(I2V, TJV) SD_STAGED_R(I2V, TJV, 1)
 #define SD_STAGED(I2V) SD_STAGED_T(I2V, sd::kTJ)
-            cfg.kernel = (i2 == 4) ? SD_STAGED(4)
+            // same repair variant as the bulk-copy kernel of this size: the modes stay bit-identical
+            cfg.kernel = (i2 == 4) ? (c->N >= sd::kRepairMaxN ? SD_STAGED_R(4, sd::kTJ, 0) : SD_STAGED(4))
                                    : ((i2 == 2) ? SD_STAGED(2)
                                                 : (small_tiles ? SD_STAGED_T(1, sd::kTJSmall) : SD_STAGED(1)));
+#undef SD_STAGED_R
 #undef SD_STAGED_T
 #undef SD_STAGED
             static const char* snames[2][3] = {
@@ -421,8 +433,9 @@ sd_status configure(sd_ctx* c) {
     SD_CUDA(c, cudaMemcpy(c->d_blk_nslots, nslots.data(), sizeof(int) * cfg.B, cudaMemcpyHostToDevice));
     c->lo_valid = fresh_lo ? true : lo_was_valid;  // fresh words are zero; kept ones keep their state
     // mid N in the fp32 modes: the whole product in one launch of the warp-split kernel
-    if (!f64 && c->staging == sd::STAGE_BULK && c->N > c->small_apply_max &&
-        (c->jsplit == 2 || (c->jsplit == 0 && c->N <= (pbc ? sd::kWMaxNBox : sd::kWMaxN)))) {
+    const long long wmax = f64 ? sd::kW64MaxN : (pbc ? sd::kWMaxNBox : sd::kWMaxN);
+    if (c->staging == sd::STAGE_BULK && c->N > c->small_apply_max &&
+        (c->jsplit == 2 || (c->jsplit == 0 && c->N <= wmax))) {
         sd_status ws = configure_w(c);
         if (ws != SD_OK) return ws;
     }
@@ -449,18 +462,30 @@ const void* w_pick(bool rpy, bool plain, bool pbc) {
 
 sd_status configure_w(sd_ctx* c) {
     const bool rpy = c->tensor == SD_TENSOR_RPY, plain = c->precision == SD_PREC_F32_PLAIN, pbc = c->box > 0.0;
+    const bool f64 = c->precision == SD_PREC_F64;
     Config w;
-    const int i2 = 4;
-    w.ipt = 2 * i2;
-    w.IB = 64 * i2;
+    size_t smem = 0;
     w.TJ = sd::kWQ;  // the schedule is cut at 4-record granularity; tiles are private to the warps
-    w.kernel = w_pick<4>(rpy, plain, pbc);
-    const size_t smem = sd::WShape<4>::smem_bytes;
+    if (f64) {
+        w.ipt = 4;
+        w.IB = 32 * 4;
+#define SD_W64(T, P) reinterpret_cast<const void*>(&sd::pairs_f64w_kernel<4, T, P>)
+        w.kernel = rpy ? (pbc ? SD_W64(0, true) : SD_W64(0, false)) : (pbc ? SD_W64(1, true) : SD_W64(1, false));
+#undef SD_W64
+        smem = sd::W64Shape<4>::smem_bytes;
+    } else {
+        w.ipt = 8;
+        w.IB = 64 * 4;
+        w.kernel = w_pick<4>(rpy, plain, pbc);
+        smem = sd::WShape<4>::smem_bytes;
+    }
     static const char* wn[2][2][2] = {{{"pairs_f32x2_w8_rpy_kahan", "pairs_f32x2_w8_rpy_kahan_pbc"},
                                        {"pairs_f32x2_w8_rpy_plain", "pairs_f32x2_w8_rpy_plain_pbc"}},
                                       {{"pairs_f32x2_w8_oseen_kahan", "pairs_f32x2_w8_oseen_kahan_pbc"},
                                        {"pairs_f32x2_w8_oseen_plain", "pairs_f32x2_w8_oseen_plain_pbc"}}};
     w.name = wn[rpy ? 0 : 1][plain ? 1 : 0][pbc ? 1 : 0];
+    static const char* wn64[2][2] = {{"pairs_f64_w4_rpy", "pairs_f64_w4_rpy_pbc"}, {"pairs_f64_w4_oseen", "pairs_f64_w4_oseen_pbc"}};
+    if (f64) w.name = wn64[rpy ? 0 : 1][pbc ? 1 : 0];
     SD_CUDA(c, cudaFuncSetAttribute(w.kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem)));
     int occ = 0;
     SD_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, w.kernel, sd::kThreads, smem));
@@ -471,7 +496,7 @@ sd_status configure_w(sd_ctx* c) {
     c->wcfg = w;
     c->w_smem = smem;
     const size_t nrec = static_cast<size_t>(c->Nrec);
-    SD_CUDA(c, cudaMalloc(&c->w_part, nrec * 2 * sizeof(float4) * w.max_slots));
+    SD_CUDA(c, cudaMalloc(&c->w_part, nrec * (f64 ? sizeof(double4) : 2 * sizeof(float4)) * w.max_slots));
     SD_CUDA(c, cudaMalloc(&c->w_blk_done, sizeof(int) * w.B));
     SD_CUDA(c, cudaMemset(c->w_blk_done, 0, sizeof(int) * w.B));
     SD_CUDA(c, cudaMalloc(&c->w_cta_u0, sizeof(long long) * (w.G + 1)));
@@ -482,11 +507,18 @@ sd_status configure_w(sd_ctx* c) {
     SD_CUDA(c, cudaMemcpy(c->w_blk_first, hs.first.data(), sizeof(int) * w.B, cudaMemcpyHostToDevice));
     SD_CUDA(c, cudaMemcpy(c->w_blk_nslots, hs.nslots.data(), sizeof(int) * w.B, cudaMemcpyHostToDevice));
     SD_CUDA(c, cudaMemcpy(c->w_cta_piece, hs.piece.data(), sizeof(int) * w.G, cudaMemcpyHostToDevice));
-    std::vector<float4> pad(2 * sd::kWSJ, make_float4(0.f, 0.f, 0.f, 0.f));
-    for (int q = 0; q < sd::kWSJ; ++q) pad[q] = make_float4(SD_PAD_POS, SD_PAD_POS, SD_PAD_POS, 0.f);
-    SD_CUDA(c, cudaMalloc(&c->w_pad, pad.size() * sizeof(float4)));
-    SD_CUDA(c, cudaMemcpy(c->w_pad, pad.data(), pad.size() * sizeof(float4), cudaMemcpyHostToDevice));
-    SD_CUDA(c, cudaMalloc(&c->grav_buf, nrec * sizeof(float4)));
+    if (f64) {
+        std::vector<double4> pad(2 * sd::kW64SJ, make_double4(0.0, 0.0, 0.0, 0.0));
+        for (int q = 0; q < sd::kW64SJ; ++q) pad[q] = make_double4(SD_PAD_POS, SD_PAD_POS, SD_PAD_POS, 0.0);
+        SD_CUDA(c, cudaMalloc(&c->w_pad, pad.size() * sizeof(double4)));
+        SD_CUDA(c, cudaMemcpy(c->w_pad, pad.data(), pad.size() * sizeof(double4), cudaMemcpyHostToDevice));
+    } else {
+        std::vector<float4> pad(2 * sd::kWSJ, make_float4(0.f, 0.f, 0.f, 0.f));
+        for (int q = 0; q < sd::kWSJ; ++q) pad[q] = make_float4(SD_PAD_POS, SD_PAD_POS, SD_PAD_POS, 0.f);
+        SD_CUDA(c, cudaMalloc(&c->w_pad, pad.size() * sizeof(float4)));
+        SD_CUDA(c, cudaMemcpy(c->w_pad, pad.data(), pad.size() * sizeof(float4), cudaMemcpyHostToDevice));
+    }
+    SD_CUDA(c, cudaMalloc(&c->grav_buf, nrec * 4 * elem_size(c->precision)));
     c->w_on = true;
     return SD_OK;
 }
@@ -585,6 +617,29 @@ sd_status launch_pairs(sd_ctx* c, cudaStream_t st) {
 sd_status launch_w(sd_ctx* c, const void* posx, const void* force, void* vel, const void* pos_base,
                    void* pos_out, double dt, int mode, cudaStream_t st) {
     return profiled(c, st, [&]() -> sd_status {
+        if (c->precision == SD_PREC_F64) {
+            sd::Schedule sch;
+            sch.cta_u0 = c->w_cta_u0, sch.blk_first_cta = c->w_blk_first, sch.blk_nslots = c->w_blk_nslots;
+            sch.cta_piece = c->w_cta_piece;
+            sch.T = c->wcfg.T, sch.B = c->wcfg.B, sch.G = c->wcfg.G;
+            sd::PairCoef64 k = folded_coef<double>(c);
+            float thr = (c->tensor == SD_TENSOR_RPY) ? static_cast<float>(4.0 * c->a * c->a * (1.0 + 1e-6)) : 1e-30f;
+            sd::FinArgs64 fin;
+            fin.vel = static_cast<double4*>(vel);
+            fin.pos_base = static_cast<const double4*>(pos_base);
+            fin.pos_out = static_cast<double4*>(pos_out);
+            fin.dt = dt, fin.c1 = c->mu0 * 0.75 * c->a, fin.mu0 = c->mu0, fin.mode = mode;
+            const double4* pp = static_cast<const double4*>(posx);
+            const double4* ff = static_cast<const double4*>(force);
+            const double4* pad = static_cast<const double4*>(c->w_pad);
+            double4* part = static_cast<double4*>(c->w_part);
+            int n = static_cast<int>(c->N);
+            long long stride = c->Nrec;
+            void* args[] = {&pp, &ff, &pad, &part, &c->w_blk_done, &sch, &k, &thr, &fin, &n, &stride};
+            cudaError_t e = cudaLaunchKernel(c->wcfg.kernel, dim3(c->wcfg.G), dim3(sd::kThreads), args, c->w_smem, st);
+            if (e != cudaSuccess) return fail(c, SD_ERR_CUDA, std::string("pairs_f64w: ") + cudaGetErrorString(e));
+            return check_launch(c, c->wcfg.name);
+        }
         sd::Schedule sch;
         sch.cta_u0 = c->w_cta_u0;
         sch.blk_first_cta = c->w_blk_first;
@@ -1131,9 +1186,12 @@ sd_status sd_step(sd_ctx* ctx, void* pos, sd_force_fn fn, void* user, const void
     const bool lub = ctx->lubrication != 0;
     if (ctx->w_on && !fn && !lub && !force) {  // the warp-split kernel reads a force array
         const int n = static_cast<int>(ctx->N);
-        sd::fill4_kernel<<<(n + 255) / 256, 256, 0, st>>>(static_cast<float4*>(ctx->grav_buf),
-                                                         static_cast<float>(gravity[0]), static_cast<float>(gravity[1]),
-                                                         static_cast<float>(gravity[2]), n);
+        if (ctx->precision == SD_PREC_F64)
+            sd::fill4_kernel<double4><<<(n + 255) / 256, 256, 0, st>>>(static_cast<double4*>(ctx->grav_buf), gravity[0],
+                                                                      gravity[1], gravity[2], n);
+        else
+            sd::fill4_kernel<float4><<<(n + 255) / 256, 256, 0, st>>>(static_cast<float4*>(ctx->grav_buf), gravity[0],
+                                                                     gravity[1], gravity[2], n);
         if ((s = check_launch(ctx, "fill4_kernel")) != SD_OK) return s;
     }
     if (!fn && !lub && ctx->N <= sd::kStepperMax)  // all steps in one launch

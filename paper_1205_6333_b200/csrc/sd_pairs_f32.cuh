@@ -307,7 +307,8 @@ __device__ __forceinline__ float self_clamped_coef(const int tensor, const float
 // Repair of one chunk whose packed pass met a pair below the clamp (overlapping spheres,
 // coincident centres).  The unclamped body has then added a far-field term of enormous size to the
 // sum of ONE particle; the other packed groups of the lane are fine.  Only the groups flagged in
-// `groups` (bit m) are redone: their chunk sum restarts from its base, every pair goes through the
+// kernel's `groups` mask are redone, one call of chunk_fix_group each: the chunk sum restarts from
+// its base (0, or the running sum at chunk start without compensation), every pair goes through the
 // clamped packed body for that one group (finite terms of ordinary size), and the pairs below the
 // clamp are put right one by one -- clamped term out, exact term in.  About a quarter of an
 // ordinary chunk pass per flagged group, where redoing the chunk for all groups with per-pair
@@ -316,53 +317,48 @@ __device__ __forceinline__ float self_clamped_coef(const int tensor, const float
 //   cp / cf : positions / forces of the chunk's records, JS float4 apart from one j to the next
 //   ISTEP   : index distance between the particles of consecutive slots (m, half) of a lane
 // Convention kept for the epilogue: a self pair leaves the clamped term A_c F'_i in the sum.
-template <int I2, int TENSOR, int ACC, bool PBC, int JS, int ISTEP>
-__device__ __forceinline__ void chunk_fix(const f32x2 (&xi)[I2], const f32x2 (&yi)[I2], const f32x2 (&zi)[I2],
-                                          const float4* cp, const float4* cf, const int j0, const int len,
-                                          const int N, const int i_first, const PairCoef& k,
-                                          const unsigned groups, f32x2 (&px)[I2], f32x2 (&py)[I2],
-                                          f32x2 (&pz)[I2], const f32x2 (&qx)[I2], const f32x2 (&qy)[I2],
-                                          const f32x2 (&qz)[I2]) {
-#pragma unroll
-    for (int m = 0; m < I2; ++m) {
-        if (!((groups >> m) & 1u)) continue;
-        f32x2 x1[1] = {xi[m]}, y1[1] = {yi[m]}, z1[1] = {zi[m]};
-        f32x2 p1x[1], p1y[1], p1z[1];
-        p1x[0] = ACC == ACC_KAHAN ? bc2(0.f) : qx[m];
-        p1y[0] = ACC == ACC_KAHAN ? bc2(0.f) : qy[m];
-        p1z[0] = ACC == ACC_KAHAN ? bc2(0.f) : qz[m];
-        const int i0 = i_first + (2 * m) * ISTEP;
-        const float xa = lo2(xi[m]), ya = lo2(yi[m]), za = lo2(zi[m]);
-        const float xb = hi2(xi[m]), yb = hi2(yi[m]), zb = hi2(zi[m]);
-        float mnd = 0.f, r2p[2];
+// It is a real call (__noinline__, operands by value): inlined into the kernel it took part in the
+// register allocation of the hot loop (22 accumulator copies per 4 j in the warp-split kernel,
+// -2 % in the classic one); as a call the hot loop does not know it exists.
+struct P3 {
+    f32x2 x, y, z;
+};
+template <int TENSOR, bool PBC, int JS, int ISTEP>
+__device__ __noinline__ P3 chunk_fix_group(const f32x2 x, const f32x2 y, const f32x2 z, const float4* cp,
+                                           const float4* cf, const int j0, const int len, const int N,
+                                           const int i0, const PairCoef k, const P3 base) {
+    f32x2 x1[1] = {x}, y1[1] = {y}, z1[1] = {z};
+    f32x2 p1x[1] = {base.x}, p1y[1] = {base.y}, p1z[1] = {base.z};
+    const float xa = lo2(x), ya = lo2(y), za = lo2(z);
+    const float xb = hi2(x), yb = hi2(y), zb = hi2(z);
+    float mnd = 0.f, r2p[2];
 #pragma unroll 2
-        for (int jj = 0; jj < len; ++jj) {
-            const float4 pj = cp[jj * JS];
-            const float4 fj = cf[jj * JS];
-            const int j = j0 + jj;
-            pair_fast_staged<1, TENSOR, PBC, true>(x1, y1, z1, pj, fj, k, p1x, p1y, p1z, mnd, r2p);
-            const bool fix0 = r2p[0] < k.clampv && j != i0;
-            const bool fix1 = r2p[1] < k.clampv && j != i0 + ISTEP;
-            if ((fix0 || fix1) && j < N) {
-                float ax = lo2(p1x[0]), ay = lo2(p1y[0]), az = lo2(p1z[0]);
-                float bx = hi2(p1x[0]), by = hi2(p1y[0]), bz = hi2(p1z[0]);
-                if (fix0) {
-                    pair_clamped_sub<TENSOR, PBC>(xa, ya, za, pj, fj, k, ax, ay, az);
-                    pair_exact<TENSOR, PBC>(xa, ya, za, false, pj, fj, k, ax, ay, az);
-                }
-                if (fix1) {
-                    pair_clamped_sub<TENSOR, PBC>(xb, yb, zb, pj, fj, k, bx, by, bz);
-                    pair_exact<TENSOR, PBC>(xb, yb, zb, false, pj, fj, k, bx, by, bz);
-                }
-                p1x[0] = pk2(ax, bx);
-                p1y[0] = pk2(ay, by);
-                p1z[0] = pk2(az, bz);
+    for (int jj = 0; jj < len; ++jj) {
+        const float4 pj = cp[jj * JS];
+        const float4 fj = cf[jj * JS];
+        const int j = j0 + jj;
+        pair_fast_staged<1, TENSOR, PBC, true>(x1, y1, z1, pj, fj, k, p1x, p1y, p1z, mnd, r2p);
+        const bool fix0 = r2p[0] < k.clampv && j != i0;
+        const bool fix1 = r2p[1] < k.clampv && j != i0 + ISTEP;
+        if ((fix0 || fix1) && j < N) {
+            float ax = lo2(p1x[0]), ay = lo2(p1y[0]), az = lo2(p1z[0]);
+            float bx = hi2(p1x[0]), by = hi2(p1y[0]), bz = hi2(p1z[0]);
+            if (fix0) {
+                pair_clamped_sub<TENSOR, PBC>(xa, ya, za, pj, fj, k, ax, ay, az);
+                pair_exact<TENSOR, PBC>(xa, ya, za, false, pj, fj, k, ax, ay, az);
             }
+            if (fix1) {
+                pair_clamped_sub<TENSOR, PBC>(xb, yb, zb, pj, fj, k, bx, by, bz);
+                pair_exact<TENSOR, PBC>(xb, yb, zb, false, pj, fj, k, bx, by, bz);
+            }
+            p1x[0] = pk2(ax, bx);
+            p1y[0] = pk2(ay, by);
+            p1z[0] = pk2(az, bz);
         }
-        px[m] = p1x[0];
-        py[m] = p1y[0];
-        pz[m] = p1z[0];
     }
+    P3 r;
+    r.x = p1x[0], r.y = p1y[0], r.z = p1z[0];
+    return r;
 }
 
 __device__ __forceinline__ void kahan_merge2(f32x2& s, f32x2& c, const f32x2 p) {
@@ -372,7 +368,15 @@ __device__ __forceinline__ void kahan_merge2(f32x2& s, f32x2& c, const f32x2 p) 
     s = t;
 }
 
-template <int I2, int TENSOR, int ACC, bool PBC, int STAGE = STAGE_BULK, int TJ = kTJ>
+// REPAIR: what happens to a chunk that holds a pair below the clamp (or the warp's self pairs).
+//   0  round-1 careful pass: the whole chunk again through the clamped body with per-pair checks
+//      (six to eight chunk passes; its code shares the kernel's register allocation)
+//   1  diagonal chunks branch-free, flagged packed groups repaired by a call of chunk_fix_group
+// Measured (profiles/r02_mid_n.md): 1 is 5 % faster at N = 32 768, 1.6 % at 65 536, equal at 131 072
+// and 0.9 % SLOWER at N = 1 048 576 (the FFMA2 loop is the same text, its registers are not), so the
+// dispatcher takes 1 below kRepairMaxN and 0 above.
+constexpr int kRepairMaxN = 200000;
+template <int I2, int TENSOR, int ACC, bool PBC, int STAGE = STAGE_BULK, int TJ = kTJ, int REPAIR = 1>
 __global__ void __launch_bounds__(kThreads, (I2 == 1) ? 3 : ((I2 == 2) ? 2 : 1))
 pairs_f32_kernel(const float4* __restrict__ rec, float4* __restrict__ part, const Schedule sch,
                  const PairCoef k, const int N, const long long slot_stride) {
@@ -481,72 +485,127 @@ pairs_f32_kernel(const float4* __restrict__ rec, float4* __restrict__ part, cons
                         qz[m] = pz[m];
                     }
                 }
-                float mn = 3.0e38f;
-                float r2v[2 * I2];
-                const int j0 = jbase + ch * kChunk;
-                // the chunk that holds this warp's own particles (self pairs, r = 0)
-                const int rel = j0 - (i_first - lane);
-                const bool diag = rel >= 0 && (rel % kThreads) == 0 && rel < I * kThreads;
-                if (!diag) {
-#pragma unroll kUnrollJ
-                    for (int jj = 0; jj < kChunk; ++jj) {
-                        const float4 pj = cj[2 * jj];
-                        const float4 fj = cj[2 * jj + 1];
-                        pair_fast_staged<I2, TENSOR, PBC, false>(xi, yi, zi, pj, fj, k, px, py, pz,
-                                                                 mn, r2v);
-                    }
-                }
-                if (diag || mn < k.thr) {
-                    // careful pass: self pairs, overlapping pairs or coincident centres sit in this
-                    // chunk.  Every pair goes through the clamped packed body (finite terms of
-                    // ordinary size, so nothing cancels); the pairs below the clamp are then put
-                    // right one by one: clamped term out, exact term (none for the self pair) in.
-                    // (The cheaper repair of the warp-split kernel, chunk_fix, was measured here too:
-                    // it moves the register allocation of the hot loop, -2.0 % at N = 1 M, -1.4 % at
-                    // 65 536, +0.9 % at 32 768; profiles/r02_mid_n.md.)
-#pragma unroll
-                    for (int m = 0; m < I2; ++m) {
-                        if (ACC == ACC_KAHAN) {
-                            px[m] = py[m] = pz[m] = bc2(0.f);
-                        } else {
-                            px[m] = qx[m];
-                            py[m] = qy[m];
-                            pz[m] = qz[m];
+                if (REPAIR == 0) {
+                    float mn = 3.0e38f;
+                    float r2v[2 * I2];
+                    const int j0 = jbase + ch * kChunk;
+                    // the chunk that holds this warp's own particles (self pairs, r = 0)
+                    const int rel = j0 - (i_first - lane);
+                    const bool diag = rel >= 0 && (rel % kThreads) == 0 && rel < I * kThreads;
+                    if (!diag) {
+    #pragma unroll kUnrollJ
+                        for (int jj = 0; jj < kChunk; ++jj) {
+                            const float4 pj = cj[2 * jj];
+                            const float4 fj = cj[2 * jj + 1];
+                            pair_fast_staged<I2, TENSOR, PBC, false>(xi, yi, zi, pj, fj, k, px, py, pz,
+                                                                     mn, r2v);
                         }
                     }
-#pragma unroll 2
-                    for (int jj = 0; jj < kChunk; ++jj) {
-                        const float4 pj = cj[2 * jj];
-                        const float4 fj = cj[2 * jj + 1];
-                        const int j = j0 + jj;
-                        pair_fast_staged<I2, TENSOR, PBC, true>(xi, yi, zi, pj, fj, k, px, py, pz,
-                                                                mn, r2v);
-#pragma unroll
+                    if (diag || mn < k.thr) {
+                        // careful pass: self pairs, overlapping pairs or coincident centres sit in this
+                        // chunk.  Every pair goes through the clamped packed body (finite terms of
+                        // ordinary size, so nothing cancels); the pairs below the clamp are then put
+                        // right one by one: clamped term out, exact term (none for the self pair) in.
+                        // (The cheaper repair of the warp-split kernel, chunk_fix, was measured here too:
+                        // it moves the register allocation of the hot loop, -2.0 % at N = 1 M, -1.4 % at
+                        // 65 536, +0.9 % at 32 768; profiles/r02_mid_n.md.)
+    #pragma unroll
                         for (int m = 0; m < I2; ++m) {
-                            // the self pair keeps its clamped term A_c F'_i: the finalize kernel
-                            // takes it out again (self_clamped_coef), all rows at once, instead of
-                            // 32 lanes walking through this branch one after the other
-                            const int i0 = i_first + (2 * m) * kThreads;
-                            const bool fix0 = r2v[2 * m] < k.clampv && j != i0;
-                            const bool fix1 = r2v[2 * m + 1] < k.clampv && j != i0 + kThreads;
-                            if ((fix0 || fix1) && j < N) {
-                                float ax = lo2(px[m]), ay = lo2(py[m]), az = lo2(pz[m]);
-                                float bx = hi2(px[m]), by = hi2(py[m]), bz = hi2(pz[m]);
-                                if (fix0) {
-                                    pair_clamped_sub<TENSOR, PBC>(lo2(xi[m]), lo2(yi[m]), lo2(zi[m]),
-                                                                  pj, fj, k, ax, ay, az);
-                                    pair_exact<TENSOR, PBC>(lo2(xi[m]), lo2(yi[m]), lo2(zi[m]),
-                                                            false, pj, fj, k, ax, ay, az);
+                            if (ACC == ACC_KAHAN) {
+                                px[m] = py[m] = pz[m] = bc2(0.f);
+                            } else {
+                                px[m] = qx[m];
+                                py[m] = qy[m];
+                                pz[m] = qz[m];
+                            }
+                        }
+    #pragma unroll 2
+                        for (int jj = 0; jj < kChunk; ++jj) {
+                            const float4 pj = cj[2 * jj];
+                            const float4 fj = cj[2 * jj + 1];
+                            const int j = j0 + jj;
+                            pair_fast_staged<I2, TENSOR, PBC, true>(xi, yi, zi, pj, fj, k, px, py, pz,
+                                                                    mn, r2v);
+    #pragma unroll
+                            for (int m = 0; m < I2; ++m) {
+                                // the self pair keeps its clamped term A_c F'_i: the finalize kernel
+                                // takes it out again (self_clamped_coef), all rows at once, instead of
+                                // 32 lanes walking through this branch one after the other
+                                const int i0 = i_first + (2 * m) * kThreads;
+                                const bool fix0 = r2v[2 * m] < k.clampv && j != i0;
+                                const bool fix1 = r2v[2 * m + 1] < k.clampv && j != i0 + kThreads;
+                                if ((fix0 || fix1) && j < N) {
+                                    float ax = lo2(px[m]), ay = lo2(py[m]), az = lo2(pz[m]);
+                                    float bx = hi2(px[m]), by = hi2(py[m]), bz = hi2(pz[m]);
+                                    if (fix0) {
+                                        pair_clamped_sub<TENSOR, PBC>(lo2(xi[m]), lo2(yi[m]), lo2(zi[m]),
+                                                                      pj, fj, k, ax, ay, az);
+                                        pair_exact<TENSOR, PBC>(lo2(xi[m]), lo2(yi[m]), lo2(zi[m]),
+                                                                false, pj, fj, k, ax, ay, az);
+                                    }
+                                    if (fix1) {
+                                        pair_clamped_sub<TENSOR, PBC>(hi2(xi[m]), hi2(yi[m]), hi2(zi[m]),
+                                                                      pj, fj, k, bx, by, bz);
+                                        pair_exact<TENSOR, PBC>(hi2(xi[m]), hi2(yi[m]), hi2(zi[m]),
+                                                                false, pj, fj, k, bx, by, bz);
+                                    }
+                                    px[m] = pk2(ax, bx);
+                                    py[m] = pk2(ay, by);
+                                    pz[m] = pk2(az, bz);
                                 }
-                                if (fix1) {
-                                    pair_clamped_sub<TENSOR, PBC>(hi2(xi[m]), hi2(yi[m]), hi2(zi[m]),
-                                                                  pj, fj, k, bx, by, bz);
-                                    pair_exact<TENSOR, PBC>(hi2(xi[m]), hi2(yi[m]), hi2(zi[m]),
-                                                            false, pj, fj, k, bx, by, bz);
-                                }
-                                px[m] = pk2(ax, bx);
-                                py[m] = pk2(ay, by);
-                                pz[m] = pk2(az, bz);
+                            }
+                        }
+                    }
+                } else {
+                    float mn = 3.0e38f;
+                    float mng[I2];
+    #pragma unroll
+                    for (int m = 0; m < I2; ++m) mng[m] = 3.0e38f;
+                    float r2v[2 * I2];
+                    const int j0 = jbase + ch * kChunk;
+                    // the chunk that holds this warp's own particles (self pairs, r = 0)
+                    const int rel = j0 - (i_first - lane);
+                    const bool diag = rel >= 0 && (rel % kThreads) == 0 && rel < I * kThreads;
+                    unsigned groups = 0u;
+                    if (!diag) {
+    #pragma unroll kUnrollJ
+                        for (int jj = 0; jj < kChunk; ++jj) {
+                            const float4 pj = cj[2 * jj];
+                            const float4 fj = cj[2 * jj + 1];
+                            pair_fast_staged<I2, TENSOR, PBC, false, true>(xi, yi, zi, pj, fj, k, px, py, pz,
+                                                                           mn, r2v, mng);
+                        }
+    #pragma unroll
+                        for (int m = 0; m < I2; ++m) groups |= (mng[m] < k.thr ? 1u : 0u) << m;
+                    } else {
+                        int zeros = 0;
+    #pragma unroll kUnrollJ
+                        for (int jj = 0; jj < kChunk; ++jj) {
+                            const float4 pj = cj[2 * jj];
+                            const float4 fj = cj[2 * jj + 1];
+                            pair_fast_staged<I2, TENSOR, PBC, true>(xi, yi, zi, pj, fj, k, px, py, pz, mn, r2v);
+    #pragma unroll
+                            for (int q = 0; q < I; ++q) {
+                                const bool z = r2v[q] == 0.f;
+                                zeros += z ? 1 : 0;
+                                mng[q / 2] = fminf(mng[q / 2], z ? 3.0e38f : r2v[q]);
+                            }
+                        }
+    #pragma unroll
+                        for (int m = 0; m < I2; ++m) groups |= (mng[m] < k.clampv ? 1u : 0u) << m;
+                        if (zeros != ((j0 + lane < N) ? 1 : 0)) groups = (1u << I2) - 1u;
+                    }
+                    if (groups) {
+    #pragma unroll
+                        for (int m = 0; m < I2; ++m) {
+                            if ((groups >> m) & 1u) {
+                                P3 base;
+                                base.x = ACC == ACC_KAHAN ? bc2(0.f) : qx[m];
+                                base.y = ACC == ACC_KAHAN ? bc2(0.f) : qy[m];
+                                base.z = ACC == ACC_KAHAN ? bc2(0.f) : qz[m];
+                                const P3 r = chunk_fix_group<TENSOR, PBC, 2, kThreads>(
+                                    xi[m], yi[m], zi[m], cj, cj + 1, j0, kChunk, N, i_first + (2 * m) * kThreads, k, base);
+                                px[m] = r.x, py[m] = r.y, pz[m] = r.z;
                             }
                         }
                     }

@@ -35,12 +35,12 @@
 
 namespace sd {
 
-// Up to here the warp-split kernel runs by default (measured against the classic kernels, both
-// tensors, profiles/r02_mid_n.md: free space 17 % faster at N = 3000 and 4096, 7 % at 8192, 1-2 % up
-// to 20480, equal at 24576, 4 % slower at 32768; periodic box 17 % at 4096, 4 % at 8192, equal from
-// 12288 to 16384, 2-4 % slower above).
-constexpr int kWMaxN = 20480;
-constexpr int kWMaxNBox = 12288;
+// Up to here the warp-split kernel runs by default (measured against the classic kernels with
+// `python bench.py --n N --jsplit classic|warp`, profiles/r02_mid_n.md: free space 18 % faster at
+// N = 4096, 10 % at 8192, 8 % at 16 384 and 20 480, 3 % at 24 576, 2 % slower at 32 768; periodic box
+// 20 % at 4096, 6 % at 8192, 3 % at 12 288, equal at 16 384, 2 % at 24 576).
+constexpr int kWMaxN = 28000;
+constexpr int kWMaxNBox = 28000;
 
 // everything the fused epilogue needs
 struct FinArgs {
@@ -267,9 +267,20 @@ pairs_f32w_kernel(const float4* __restrict__ pos, const float4* __restrict__ frc
                 for (int m = 0; m < I2; ++m) groups |= (mng[m] < k.clampv ? 1u : 0u) << m;
                 if (zeros != (mine ? 1 : 0)) groups = (1u << I2) - 1u;  // coincident centres: all groups
             }
-            if (groups)  // rare: repair the chunk sums of the groups that met a pair below the clamp
-                chunk_fix<I2, TENSOR, ACC, PBC, 1, 32>(xi, yi, zi, cp, cf, j0, len, N, i_first, k, groups, px,
-                                                       py, pz, qx, qy, qz);
+            if (groups) {  // rare: repair the chunk sums of the groups that met a pair below the clamp
+#pragma unroll
+                for (int m = 0; m < I2; ++m) {
+                    if ((groups >> m) & 1u) {
+                        P3 base;
+                        base.x = ACC == ACC_KAHAN ? bc2(0.f) : qx[m];
+                        base.y = ACC == ACC_KAHAN ? bc2(0.f) : qy[m];
+                        base.z = ACC == ACC_KAHAN ? bc2(0.f) : qz[m];
+                        const P3 r = chunk_fix_group<TENSOR, PBC, 1, 32>(xi[m], yi[m], zi[m], cp, cf, j0, len, N,
+                                                                         i_first + 64 * m, k, base);
+                        px[m] = r.x, py[m] = r.y, pz[m] = r.z;
+                    }
+                }
+            }
             if (ACC == ACC_KAHAN) {
 #pragma unroll
                 for (int m = 0; m < I2; ++m) {

@@ -162,44 +162,61 @@ __device__ __forceinline__ void pair_clamped_sub_f64(const double xi, const doub
 // chunk (self pair and pad records excluded); the chunk sums of the particles that have a pair
 // below `thr` are recomputed with the exact branching body.  A self pair keeps the clamped term
 // A_c F'_i (removed by finalize_f64_kernel).
-template <int I, int TENSOR, bool PBC>
+//   cp / cf : positions / forces of the chunk's records, JS double4 apart from one j to the next
+//   ISTEP   : index distance between consecutive particles of a lane
+// The work per particle is a real call (__noinline__, operands by value) so that it takes no part
+// in the register allocation of the hot loop (sd_pairs_f32.cuh, chunk_fix_group).
+struct D3 {
+    double x, y, z;
+};
+template <int TENSOR, bool PBC, int JS>
+__device__ __noinline__ D3 chunk_fix_one_f64(const double x, const double y, const double z, const double4* cp,
+                                             const double4* cf, const int nj, const int jself, const PairCoef64 k,
+                                             const double thr, const D3 base, const D3 cur) {
+    double mnq = 1.0e300;
+#pragma unroll 4
+    for (int jj = 0; jj < nj; ++jj) {
+        const double4 pj = cp[jj * JS];
+        const double dx = min_image_f64<PBC>(x - pj.x, k), dy = min_image_f64<PBC>(y - pj.y, k),
+                     dz = min_image_f64<PBC>(z - pj.z, k);
+        const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+        mnq = fmin(mnq, jj == jself ? 1.0e300 : r2);
+    }
+    if (!(mnq < thr)) return cur;
+    double nx = 0.0, ny = 0.0, nz = 0.0;
+#pragma unroll 1
+    for (int jj = 0; jj < nj; ++jj) {
+        const double4 pj = cp[jj * JS];
+        const double4 fj = cf[jj * JS];
+        if (jj == jself) {
+            const double ac = self_clamped_coef_f64(TENSOR, k.clampv, k.k2);
+            nx = fma(ac, fj.x, nx);
+            ny = fma(ac, fj.y, ny);
+            nz = fma(ac, fj.z, nz);
+        } else {
+            pair_exact_f64<TENSOR, PBC>(x, y, z, false, pj, fj, k, nx, ny, nz);
+        }
+    }
+    D3 r;
+    r.x = base.x + nx, r.y = base.y + ny, r.z = base.z + nz;
+    return r;
+}
+
+template <int I, int TENSOR, bool PBC, int JS, int ISTEP>
 __device__ __forceinline__ void chunk_fix_f64(const double (&xi)[I], const double (&yi)[I], const double (&zi)[I],
-                                              const double4* cj, const int j0, const int N, const int i_first,
-                                              const PairCoef64& k, const double thr, double (&px)[I],
-                                              double (&py)[I], double (&pz)[I], const double (&qx)[I],
-                                              const double (&qy)[I], const double (&qz)[I]) {
-    const int nj = min(kChunk, N - j0);
+                                              const double4* cp, const double4* cf, const int j0, const int len,
+                                              const int N, const int i_first, const PairCoef64& k, const double thr,
+                                              double (&px)[I], double (&py)[I], double (&pz)[I],
+                                              const double (&qx)[I], const double (&qy)[I], const double (&qz)[I]) {
+    const int nj = min(len, N - j0);
 #pragma unroll
     for (int m = 0; m < I; ++m) {
-        const int jself = i_first + m * kThreads - j0;
-        double mnq = 1.0e300;
-#pragma unroll 4
-        for (int jj = 0; jj < nj; ++jj) {
-            const double4 pj = cj[2 * jj];
-            const double dx = min_image_f64<PBC>(xi[m] - pj.x, k), dy = min_image_f64<PBC>(yi[m] - pj.y, k),
-                         dz = min_image_f64<PBC>(zi[m] - pj.z, k);
-            const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
-            mnq = fmin(mnq, jj == jself ? 1.0e300 : r2);
-        }
-        if (mnq < thr) {
-            double nx = 0.0, ny = 0.0, nz = 0.0;
-#pragma unroll 1
-            for (int jj = 0; jj < nj; ++jj) {
-                const double4 pj = cj[2 * jj];
-                const double4 fj = cj[2 * jj + 1];
-                if (jj == jself) {
-                    const double ac = self_clamped_coef_f64(TENSOR, k.clampv, k.k2);
-                    nx = fma(ac, fj.x, nx);
-                    ny = fma(ac, fj.y, ny);
-                    nz = fma(ac, fj.z, nz);
-                } else {
-                    pair_exact_f64<TENSOR, PBC>(xi[m], yi[m], zi[m], false, pj, fj, k, nx, ny, nz);
-                }
-            }
-            px[m] = qx[m] + nx;
-            py[m] = qy[m] + ny;
-            pz[m] = qz[m] + nz;
-        }
+        D3 base, cur;
+        base.x = qx[m], base.y = qy[m], base.z = qz[m];
+        cur.x = px[m], cur.y = py[m], cur.z = pz[m];
+        const D3 r = chunk_fix_one_f64<TENSOR, PBC, JS>(xi[m], yi[m], zi[m], cp, cf, nj, i_first + m * ISTEP - j0, k,
+                                                        thr, base, cur);
+        px[m] = r.x, py[m] = r.y, pz[m] = r.z;
     }
 }
 
@@ -320,8 +337,8 @@ pairs_f64_kernel(const double4* __restrict__ rec, double4* __restrict__ part, co
                     fix = mn < static_cast<float>(k.clampv) * 1.000001f || zeros != ((j0 + lane < N) ? 1 : 0);
                 }
                 if (fix)  // rare: repair the sums of the particles that have a pair below the clamp
-                    chunk_fix_f64<I, TENSOR, PBC>(xi, yi, zi, cj, j0, N, i_first, k, diag ? k.clampv : k.thr, px,
-                                                  py, pz, qx, qy, qz);
+                    chunk_fix_f64<I, TENSOR, PBC, 2, kThreads>(xi, yi, zi, cj, cj + 1, j0, kChunk, N, i_first, k,
+                                                               diag ? k.clampv : k.thr, px, py, pz, qx, qy, qz);
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(&empty_bar[s]);

@@ -63,10 +63,12 @@ pack_kernel(const T4* __restrict__ pos, const T4* __restrict__ force, T4* __rest
 }
 
 // uniform force written out per particle (sd_step with gravity on the paths that read a force array)
+template <typename T4>
 __global__ void __launch_bounds__(256)
-fill4_kernel(float4* __restrict__ out, const float x, const float y, const float z, const int n) {
+fill4_kernel(T4* __restrict__ out, const double x, const double y, const double z, const int n) {
+    typedef typename Vec4<T4>::S S;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n) out[i] = make_float4(x, y, z, 0.f);
+    if (i < n) out[i] = Vec4<T4>::make(S(x), S(y), S(z), S(0));
 }
 
 constexpr int kFinThreads = 128;
