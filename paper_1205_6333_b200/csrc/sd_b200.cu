@@ -62,7 +62,8 @@ struct sd_ctx {
     int tensor = SD_TENSOR_RPY;
     int precision = SD_PREC_F32_KAHAN;
     double box = 0.0;  // side of the periodic cube; 0 = free space
-    long long small_apply_max = sd::kSmallApplyMax;  // N up to which the one-launch kernel runs
+    long long small_apply_max = sd::kSmallApplyMax;  // N up to which the one-launch warp-per-particle kernel runs
+    long long small_user = -1;                       // sd_set_dispatch override (< 0: automatic, see configure)
     int ipt_override = 0;                            // particles per thread; 0 = automatic
     int staging = 0;                                 // sd::STAGE_* (ablation, fp32 RPY Kahan only)
     int pos_comp = 1;                                // 0: plain fp32 positions (ablation)
@@ -317,6 +318,12 @@ sd_status configure(sd_ctx* c) {
     const bool f64 = c->precision == SD_PREC_F64;
     const bool rpy = c->tensor == SD_TENSOR_RPY;
     const bool pbc = c->box > 0.0;
+    // where the warp-per-particle one-launch kernels stop (measured, profiles/r02_mid_n.md): with the
+    // warp-split kernel behind them at the end of the packed fp32 window (2304) resp. at 1000 in fp64;
+    // 2560 when only the classic tiled kernels follow
+    if (c->small_user >= 0) c->small_apply_max = c->small_user;
+    else if (c->jsplit == 1 || c->staging != sd::STAGE_BULK) c->small_apply_max = sd::kSmallApplyMax;
+    else c->small_apply_max = f64 ? sd::kW64MinN : sd::kPackedMaxN;
     if (!f64) {
         const bool plain = c->precision == SD_PREC_F32_PLAIN;
         // particles per thread: 8 once there is enough work to balance 2048-particle i-blocks
@@ -1068,7 +1075,7 @@ sd_status sd_set_dispatch(sd_ctx* ctx, long long small_apply_max, int particles_
         particles_per_thread != 8)
         return fail(ctx, SD_ERR_INVALID_ARG, "sd_set_dispatch: particles_per_thread must be 0, 2, 4 or 8");
     cudaDeviceSynchronize();
-    ctx->small_apply_max = small_apply_max < 0 ? sd::kSmallApplyMax : small_apply_max;
+    ctx->small_user = small_apply_max < 0 ? -1 : small_apply_max;
     ctx->ipt_override = particles_per_thread;
     return configure(ctx);
 }

@@ -17,10 +17,14 @@
 namespace sd {
 
 constexpr int kW64SJ = 32;     // j records (2 x 32 bytes each) per warp-private sub-tile
-// Measured against the classic fp64 kernels (1 - 2 particles per thread, 2 - 3 CTAs per SM), profiles/r02_mid_n.md:
-// 69.9 / 167.5 / 537 us at N = 4096 / 8192 / 16384 against 61.7 / 162 / 517: slower everywhere (two warps per
-// scheduler do not hide the DFMA latency that 24 resident warps hide), so it never runs by default (mode 2 only).
-constexpr int kW64MaxN = 0;
+// Measured (profiles/r02_mid_n.md): against the one-launch warp-per-particle kernel it wins from N = 1024 on
+// (14.6 / 20.9 / 28.1 / 35.0 us at N = 1024 / 1536 / 2048 / 2560 against 16.6 / 24.9 / 33.0 / 59.6), against the classic
+// fp64 kernels (1 - 2 particles per thread, 2 - 3 CTAs per SM) per product up to N = 3000 (43.3 against 47.3 us) but not per
+// Euler step there (41.9 against 39.6 us: sd_step never runs the pack kernel); from N = 4096 on it
+// loses (69.9 / 167.5 / 537 us at 4096 / 8192 / 16384 against 61.7 / 162 / 517: two warps per scheduler do not hide the
+// DFMA latency that 24 resident warps hide).  Default range: kW64MinN < N <= kW64MaxN.
+constexpr int kW64MinN = 1000;
+constexpr int kW64MaxN = 2800;
 
 struct FinArgs64 {
     double4* vel;
