@@ -56,7 +56,7 @@ struct FinArgs {
 };
 
 constexpr int kWQ = 4;        // schedule granule: j records per "quad" (= the unrolled loop body)
-constexpr int kWSJ = 64;      // j records per warp-private sub-tile (two compensation chunks)
+constexpr int kWSJ = 64;      // j records per warp-private sub-tile (two compensation chunks; 128: +0.5 % at N >= 16384, -1 % at 4096)
 constexpr int kWStages = 3;   // sub-tiles per warp in flight / in use
 
 template <int I2>
