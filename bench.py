@@ -475,10 +475,47 @@ def extra_measurements(torch, sd, wl, sm_count, probes):
                           "pairs_per_s_median": (2 if iname == "midpoint" else 1) * n * n * nsteps
                           / float(np.median(t))})
             ctx.close()
+    # ---- periodic box at the headline size, the paper's own benchmark shape, lubrication
+    n = 1048576
+    pos, force = wl.sweep(n)
+    dp = torch.from_numpy(wl.to_xyzw(pos, np.float32)).cuda()
+    df = torch.from_numpy(wl.to_xyzw(force, np.float32)).cuda()
+    dv = torch.empty_like(dp)
+    ctx = sd.Context(n, wl.A, wl.ETA)
+    ctx.set_box(wl.cube_side(n, 0.01))
+    t = _sample_times(torch, lambda: ctx.mobility_apply(dp, df, dv), 1, 3, 1)
+    flb = (FLOPS_PER_PAIR["rpy"] + FLOPS_NEAREST_IMAGE) / 1e12
+    box = {"workload": "sd_mobility_apply N=1048576 uniform cube phi=0.01 in its periodic box (nearest image), RPY, "
+                       "fp32-Kahan", "kernel": ctx.kernel_name, "pairs_per_s_median": n * n / float(np.median(t)),
+           "flops_per_pair": FLOPS_PER_PAIR["rpy"] + FLOPS_NEAREST_IMAGE,
+           "frac_of_derived_peak_median": n * n / float(np.median(t)) * flb / peaks["f32"]}
+    ctx.close()
+    del dp, df, dv
+    fcc = []
+    cells = 10
+    lat = wl.fcc_lattice(cells, 0.1, jitter_seed=wl.SEED_BASE + 31 + cells)
+    d0 = torch.from_numpy(wl.to_xyzw(lat, np.float32)).cuda()
+    for full in (False, True):
+        ctx = sd.Context(lat.shape[0], wl.A, wl.ETA)
+        ctx.set_box(wl.fcc_box(cells, 0.1))
+        ctx.set_lubrication(full)
+        dq = d0.clone()
+
+        def run():
+            dq.copy_(d0)
+            ctx.reset_compensation()
+            ctx.set_velocity(None)
+            ctx.step(dq, 0.001, 100, sd.INT_EULER, gravity=(0.0, 0.0, -1.0))
+        t = _sample_times(torch, run, 2, 5, 1)
+        fcc.append({"workload": f"sd_step N={lat.shape[0]} fcc lattice n=0.1/a^3 in its periodic box, gravity, Euler "
+                                "dt=0.001, 100 steps per call" + (", lubrication correction on" if full else ""),
+                    "kernel": ctx.kernel_name, "steps_per_s_median": 100 / float(np.median(t)),
+                    "us_per_step_median": 1e4 * float(np.median(t))})
+        ctx.close()
     return {"what": "BASELINE.json metric beyond the headline point, same process, CUDA events on the "
                     "launching stream; fractions = pairs/s x (34 RPY | 29 Oseen) flops / FMA peak",
             "fma_probe_tflops": probes, "derived_peak_tflops": peaks,
-            "config5_sweep": sweep, "sd_step": steps}
+            "config5_sweep": sweep, "sd_step": steps, "periodic_box": box, "paper_benchmark_shape": fcc}
 
 
 def main():
