@@ -405,18 +405,36 @@ def fma_peaks(sm_count):
             "f64": sm_count * FP64_LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12}, sm_max_mhz
 
 
+def graph_of(torch, fn, count):
+    """`count` calls of fn captured into one CUDA graph (below N ~ 10^4 a product is shorter than the
+    13 us a Python / ctypes call costs on the host: a loop of calls measures the interpreter).
+    Returns a callable that replays the graph on the current stream."""
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        fn()
+    torch.cuda.current_stream().wait_stream(side)
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=side):
+        for _ in range(count):
+            fn()
+    return g.replay
+
+
 def _sample_times(torch, fn, warm, samples, per_sample):
     """`samples` timings of `per_sample` back-to-back calls of fn between one pair of CUDA events on
-    the current (launching) stream, after `warm` untimed calls; seconds per call."""
+    the current (launching) stream, after `warm` untimed calls; seconds per call.  per_sample > 1:
+    the calls are replayed from one CUDA graph (graph_of)."""
     for _ in range(warm):
         fn()
     torch.cuda.synchronize()
+    run = graph_of(torch, fn, per_sample) if per_sample > 1 else fn
     out = []
     for _ in range(samples):
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record()
-        for _ in range(per_sample):
-            fn()
+        run()
         e1.record()
         torch.cuda.synchronize()
         out.append(e0.elapsed_time(e1) * 1e-3 / per_sample)
@@ -428,8 +446,9 @@ def extra_measurements(torch, sd, wl, sm_count, probes):
     configuration 5 (sd_mobility_apply at six sizes x {fp32-Kahan, fp64} x {RPY, Oseen}; best and
     median of 10 samples after 3 warm-ups, warm L2 -- the inputs are at most 67 MB) and sd_step
     steps/s on configurations 1, 3 and 4.  Small products are launch-bound when timed one by one
-    (an event pair costs more than the kernel), so a sample is `launches_per_sample` back-to-back
-    launches on one stream, as a simulation issues them."""
+    (an event pair, and the Python call itself, cost more than the kernel), so a sample is
+    `launches_per_sample` back-to-back launches replayed from one CUDA graph, as sd_step issues its
+    step loops."""
     peaks, _ = fma_peaks(sm_count)
     sweep = []
     for n in CFG5_NS:
@@ -577,7 +596,12 @@ def main():
     for _ in range(args.warmup):
         ctx.mobility_apply(d_pos, d_force, d_vel)
     barrier()
-    ctx.profile_enable(True)
+    # several products per timed step: replayed from one CUDA graph (no per-kernel events then: the
+    # roofline below is computed from the whole step)
+    c0 = ctx.launch_count
+    step_fn = graph_of(torch, lambda: ctx.mobility_apply(d_pos, d_force, d_vel), lps) if lps > 1 else None
+    launches_per_product = (ctx.launch_count - c0) // (lps + 1)  # graph_of: one warm call + lps captured ones
+    ctx.profile_enable(lps == 1)
     ctx.profile_read()
     launches0 = ctx.launch_count
     sampler = benchutil.ClockSampler(local_rank)
@@ -588,7 +612,9 @@ def main():
         flush.zero_()  # L2 flush between timed iterations (outside the event pair)
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record()
-        for _ in range(lps):
+        if step_fn is not None:
+            step_fn()
+        else:
             ctx.mobility_apply(d_pos, d_force, d_vel)
         e1.record()
         evs.append((e0, e1))
@@ -597,6 +623,9 @@ def main():
     local_s = sum(a.elapsed_time(b) for a, b in evs) * 1e-3
     gpu_launches = ctx.launch_count - launches0
     pair_ms, pair_launches = ctx.profile_read()
+    if step_fn is not None:  # no per-kernel events inside a graph: whole products stand in
+        gpu_launches = launches_per_product * lps * args.steps
+        pair_ms, pair_launches = local_s * 1e3, args.steps * lps
     ctx.profile_enable(False)
     units, t_max = benchutil.aggregate_over_ranks(local_s, float(args.steps) * lps * n * n)
     value = units / t_max

@@ -36,9 +36,10 @@
 namespace sd {
 
 // Up to here the warp-split kernel runs by default (measured against the classic kernels with
-// `python bench.py --n N --jsplit classic|warp`, profiles/r02_mid_n.md: free space 18 % faster at
-// N = 4096, 10 % at 8192, 8 % at 16 384 and 20 480, 3 % at 24 576, 2 % slower at 32 768; periodic box
-// 20 % at 4096, 6 % at 8192, 3 % at 12 288, equal at 16 384, 2 % at 24 576).
+// `python bench.py --n N --jsplit classic|warp --launches-per-step K`, CUDA-graph replay,
+// profiles/r02_mid_n.md: free space 11 % faster at N = 4096, 5 % at 8192, 6 % at 16 384 and 20 480,
+// 2 % at 24 576, 2 % slower at 32 768; periodic box 10 % at 4096, 2 % at 8192, within 1.6 % of each
+// other from 12 288 to 24 576).
 constexpr int kWMaxN = 28000;
 constexpr int kWMaxNBox = 28000;
 
