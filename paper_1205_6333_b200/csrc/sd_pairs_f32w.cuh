@@ -41,7 +41,7 @@ namespace sd {
 // 2 % at 24 576, 2 % slower at 32 768; periodic box 10 % at 4096, 2 % at 8192, within 1.6 % of each
 // other from 12 288 to 24 576).
 constexpr int kWMaxN = 28000;
-constexpr int kWMaxNBox = 28000;
+constexpr int kWMaxNBox = 14000;
 
 // everything the fused epilogue needs
 struct FinArgs {
