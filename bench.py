@@ -372,12 +372,16 @@ def run_lub(args, rank):
     achieved = 4.0 * rec * args.steps / secs / 1e9
     line = dict(base, value=args.steps * n / secs, ms_per_step=1e3 * secs / args.steps,
                 dtype="f64" if f64mode else "f32",
-                config={"workload": name, "kernel": "lub_count + cub scan + lub_scatter + lub_sort + lub_force",
+                config={"workload": name,
+                        "kernel": ("lub_small (all pairs)" if n <= 1024 else "lub_one_launch (grid in shared memory)"
+                                   if n <= 4096 else "lub_count + lub_scan_totals + lub_scan_apply + lub_scatter + "
+                                   "lub_sort + lub_gather + lub_force"),
                         "parallelism": "1 GPU", "l2": "L2 flushed with a 256 MiB write between timed iterations"},
                 clocks=clocks, gpu_launches=gpu_launches,
                 e2e={"value": args.steps * n / e2e, "unit": "particles/s", "h2d_bytes_per_step": 3 * rec,
                      "d2h_bytes_per_step": rec},
-                roofline={"bound": "hbm", "kernel": "whole lubrication step (5 launches)", "achieved": achieved,
+                roofline={"bound": "hbm", "kernel": f"whole lubrication step ({gpu_launches // max(args.steps, 1)} launches)",
+                          "achieved": achieved,
                           "peak": hbm, "unit": "GB/s", "frac": achieved / hbm, "traffic": None,
                           "peak_source": src, "bytes_per_particle": 4 * rec // n})
     if not args.no_cpu_baseline:

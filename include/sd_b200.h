@@ -25,7 +25,7 @@
  *    positions, position low words), allocated by sd_create and by the setters that change the
  *    kernel variant.  Two lazily allocated exceptions, both on first use and never inside a
  *    stream capture: the device staging of sd_mobility_apply_host (3 N records) and the cell
- *    grid of the lubrication step above 2560 particles.  Nothing else is allocated by
+ *    grid of the lubrication step above 4096 particles.  Nothing else is allocated by
  *    sd_mobility_apply / sd_step / sd_lubrication_apply.
  *  - Calls must be made with the CUDA device the context was created on as the current device
  *    (SD_ERR_INVALID_ARG otherwise).  After a setter failed with SD_ERR_ALLOC / SD_ERR_CUDA the
@@ -134,11 +134,13 @@ sd_status sd_step(sd_ctx* ctx, void* pos, sd_force_fn fn, void* user, const void
  * paper never lets spheres touch); coincident centres contribute nothing.  F^ext is f_ext[N][4]
  * or, when f_ext is NULL, the uniform force gravity[3] (NULL: zero).  pos, vel, f_ext, force_out
  * are device arrays of the context's element type; force_out may be f_ext, not pos or vel.  The
- * neighbour search tests all pairs in one launch up to 2560 particles and uses a hashed cell grid
- * rebuilt on every call above that (context-owned, allocated on first use); results do not
- * depend on thread scheduling.  With sd_set_box the nearest image is used and the box side must
- * exceed 6a (9a for the cell grid), SD_ERR_UNSUPPORTED otherwise.  The cut-off is decided in
- * the context's arithmetic, the accepted pairs are evaluated in fp64. */
+ * neighbour search tests all pairs in one launch up to 1024 particles and uses a cell grid
+ * rebuilt on every call above that (up to 4096 particles in the shared memory of the one kernel
+ * that does the whole step; beyond that in context-owned global arrays, allocated on first use);
+ * results do not depend on thread scheduling.  With sd_set_box the nearest image is used and the
+ * box side must exceed 6a (9a for the cell grid, i.e. above 4096 particles), SD_ERR_UNSUPPORTED
+ * otherwise.  The cut-off is decided in the context's arithmetic, the accepted pairs are
+ * evaluated in fp64. */
 sd_status sd_lubrication_apply(sd_ctx* ctx, const void* pos, const void* vel, const void* f_ext,
                                const double gravity[3], void* force_out, void* stream);
 

@@ -69,14 +69,15 @@ struct sd_ctx {
     int pos_comp = 1;                                // 0: plain fp32 positions (ablation)
     int lubrication = 0;                             // sd_step corrects the forces by Eq. (8)
     // lubrication cell grid (allocated on first use)
-    int4* lub_cell = nullptr;
-    unsigned* lub_count = nullptr;   // [H + 1] bucket histogram
+    unsigned* lub_bucket = nullptr;  // [N] bucket of every particle
+    unsigned* lub_count = nullptr;   // [H + 1] bucket histogram (left zeroed by every call)
     unsigned* lub_start = nullptr;   // [H + 1] exclusive scan of it
     unsigned* lub_cursor = nullptr;  // [H]
     int* lub_order = nullptr;        // [N] particle indices grouped by bucket
-    void* lub_spos = nullptr;        // [N] positions, velocities, cells in bucket order
+    void* lub_spos = nullptr;        // [N] positions, velocities in bucket order
     void* lub_svel = nullptr;
-    int4* lub_scell = nullptr;
+    bool lub_one_launch_ready = false;  // shared-memory attribute of lub_one_launch_kernel set
+    bool lub_count_dirty = false;    // a call was abandoned between lub_count_kernel and lub_sort_kernel
     void* lub_tmp = nullptr;         // block totals of the bucket scan
     size_t lub_tmp_bytes = 0;
     unsigned lub_H = 0;
@@ -200,10 +201,9 @@ void free_buffers(sd_ctx* c) {
         if (*b) cudaFree(*b);
         *b = nullptr;
     }
-    void** lub[] = {reinterpret_cast<void**>(&c->lub_cell), reinterpret_cast<void**>(&c->lub_count),
+    void** lub[] = {reinterpret_cast<void**>(&c->lub_bucket), reinterpret_cast<void**>(&c->lub_count),
                     reinterpret_cast<void**>(&c->lub_start), reinterpret_cast<void**>(&c->lub_cursor),
-                    reinterpret_cast<void**>(&c->lub_order), &c->lub_tmp, &c->lub_spos, &c->lub_svel,
-                    reinterpret_cast<void**>(&c->lub_scell)};
+                    reinterpret_cast<void**>(&c->lub_order), &c->lub_tmp, &c->lub_spos, &c->lub_svel};
     for (void** b : lub) {
         if (*b) cudaFree(*b);
         *b = nullptr;
@@ -856,9 +856,12 @@ sd_status ensure_lub_buffers(sd_ctx* c) {
     // every buffer on its own: after a failed allocation the next call allocates what is missing
     if (!c->lub_spos) SD_CUDA(c, cudaMalloc(&c->lub_spos, 4 * elem_size(c->precision) * n));
     if (!c->lub_svel) SD_CUDA(c, cudaMalloc(&c->lub_svel, 4 * elem_size(c->precision) * n));
-    if (!c->lub_scell) SD_CUDA(c, cudaMalloc(&c->lub_scell, sizeof(int4) * n));
-    if (!c->lub_cell) SD_CUDA(c, cudaMalloc(&c->lub_cell, sizeof(int4) * n));
-    if (!c->lub_count) SD_CUDA(c, cudaMalloc(&c->lub_count, sizeof(unsigned) * (H + 1)));
+    if (!c->lub_bucket) SD_CUDA(c, cudaMalloc(&c->lub_bucket, sizeof(unsigned) * n));
+    if (!c->lub_count) {  // zeroed once here; every call leaves it zeroed (lub_sort_kernel)
+        SD_CUDA(c, cudaMalloc(&c->lub_count, sizeof(unsigned) * (H + 1)));
+        SD_CUDA(c, cudaMemset(c->lub_count, 0, sizeof(unsigned) * (H + 1)));
+        c->lub_count_dirty = false;
+    }
     if (!c->lub_start) SD_CUDA(c, cudaMalloc(&c->lub_start, sizeof(unsigned) * (H + 1)));
     if (!c->lub_cursor) SD_CUDA(c, cudaMalloc(&c->lub_cursor, sizeof(unsigned) * H));
     if (!c->lub_order) SD_CUDA(c, cudaMalloc(&c->lub_order, sizeof(int) * n));
@@ -889,15 +892,45 @@ sd_status launch_lubrication(sd_ctx* c, const void* pos, const void* vel, const 
         // cells and needs three of them per edge: L >= 9a
         if (grid.nc < 2 || !(grid.L > 6.0 * c->a))
             return fail(c, SD_ERR_UNSUPPORTED, "lubrication in a periodic box needs a box side above 6 a");
-        if (grid.nc < 3 && n > sd::kLubSmallMax)
+        if (grid.nc < 3 && n > sd::kLubOneCtaMaxN)
             return fail(c, SD_ERR_UNSUPPORTED,
-                        "lubrication in a periodic box needs a box side of at least 9 a above 2560 particles (cell grid)");
-        grid.nc = std::min(grid.nc, 1024);
+                        "lubrication in a periodic box needs a box side of at least 9 a above 4096 particles (cell grid)");
     }
-    if (n <= sd::kLubSmallMax) {  // small systems: all pairs in one launch, no cell grid
-        const double gx = g ? g[0] : 0.0, gy = g ? g[1] : 0.0, gz = g ? g[2] : 0.0;
+    const double gx = g ? g[0] : 0.0, gy = g ? g[1] : 0.0, gz = g ? g[2] : 0.0;
+    if (n > sd::kLubSmallMax && n <= sd::kLubOneCtaMaxN && (grid.nc == 0 || grid.nc >= 3)) {
+        // one launch: every CTA builds the grid in its shared memory, then takes its share of the particles
+        grid.M = 16;  // 16^3 = kLubOneCtaMaxH buckets
+        if (grid.nc > 0) {
+            grid.nc = std::min(grid.nc, grid.M);
+            grid.M = grid.nc;
+        }
+        const int ctas = std::min(c->num_sms, (n + 31) / 32);
+        if (!c->lub_one_launch_ready) {
+            SD_CUDA(c, cudaFuncSetAttribute(sd::lub_one_launch_kernel<float4>,
+                                            cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                            static_cast<int>(sizeof(sd::LubOneLaunchSmem<float4>))));
+            SD_CUDA(c, cudaFuncSetAttribute(sd::lub_one_launch_kernel<double4>,
+                                            cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                            static_cast<int>(sizeof(sd::LubOneLaunchSmem<double4>))));
+            c->lub_one_launch_ready = true;
+        }
+        if (c->precision == SD_PREC_F64)
+            sd::lub_one_launch_kernel<double4>
+                <<<ctas, sd::kLubOneCtaThreads, sizeof(sd::LubOneLaunchSmem<double4>), st>>>(
+                    static_cast<const double4*>(pos), static_cast<const double4*>(vel),
+                    static_cast<const double4*>(fext), gx, gy, gz, static_cast<double4*>(force_out), grid,
+                    c->a, c->mu0, n);
+        else
+            sd::lub_one_launch_kernel<float4>
+                <<<ctas, sd::kLubOneCtaThreads, sizeof(sd::LubOneLaunchSmem<float4>), st>>>(
+                    static_cast<const float4*>(pos), static_cast<const float4*>(vel),
+                    static_cast<const float4*>(fext), gx, gy, gz, static_cast<float4*>(force_out), grid,
+                    c->a, c->mu0, n);
+        return check_launch(c, "lub_one_launch_kernel");
+    }
+    if (n <= sd::kLubOneCtaMaxN) {  // small systems, small boxes: all pairs in one launch, no cell grid
         const int blocks = (n + 7) / 8;
-        grid.mask = 0;
+        grid.M = 0;
         if (c->precision == SD_PREC_F64)
             sd::lub_small_kernel<double4><<<blocks, 256, 0, st>>>(
                 static_cast<const double4*>(pos), static_cast<const double4*>(vel),
@@ -914,44 +947,48 @@ sd_status launch_lubrication(sd_ctx* c, const void* pos, const void* vel, const 
         sd_status a = ensure_lub_buffers(c);
         if (a != SD_OK) return a;
     }
-    const unsigned H = c->lub_H;
+    const unsigned H = c->lub_H;  // 8^bits buckets, M = 2^bits per edge
     unsigned bits = 0;
     while ((1u << (3 * (bits + 1))) <= H) ++bits;
-    grid.mask = (1u << bits) - 1u;
-    SD_CUDA(c, cudaMemsetAsync(c->lub_count, 0, sizeof(unsigned) * (H + 1), st));
-    SD_CUDA(c, cudaMemsetAsync(c->lub_cursor, 0, sizeof(unsigned) * H, st));
+    grid.M = 1 << bits;
+    if (grid.nc > 0) {  // box: one bucket per cell, larger cells if there are more than M per edge
+        grid.nc = std::min(grid.nc, grid.M);
+        grid.M = grid.nc;
+    }
     const int nb = (n + 255) / 256;
     const unsigned nscan = (H + 1 + sd::kScanBlock - 1) / sd::kScanBlock;
-    const double gx = g ? g[0] : 0.0, gy = g ? g[1] : 0.0, gz = g ? g[2] : 0.0;
+    if (c->lub_count_dirty) SD_CUDA(c, cudaMemsetAsync(c->lub_count, 0, sizeof(unsigned) * (H + 1), st));
     sd_status s;
 #define SD_LUB_FORCE_ARGS(T4)                                                                       \
-    static_cast<const T4*>(c->lub_spos), static_cast<const T4*>(c->lub_svel),                       \
-        static_cast<const T4*>(fext), gx, gy, gz, c->lub_scell, c->lub_start,                       \
-        static_cast<T4*>(force_out), grid, c->a, c->mu0, n
+    static_cast<const T4*>(c->lub_spos), static_cast<const T4*>(c->lub_svel), c->lub_order,         \
+        static_cast<const T4*>(fext), gx, gy, gz, c->lub_start, static_cast<T4*>(force_out), grid,  \
+        c->a, c->mu0, n
 #define SD_LUB(T4)                                                                                  \
-    sd::lub_count_kernel<T4><<<nb, 256, 0, st>>>(static_cast<const T4*>(pos), c->lub_cell,          \
+    c->lub_count_dirty = true;                                                                      \
+    sd::lub_count_kernel<T4><<<nb, 256, 0, st>>>(static_cast<const T4*>(pos), c->lub_bucket,        \
                                                  c->lub_count, grid, n);                           \
     if ((s = check_launch(c, "lub_count_kernel")) != SD_OK) return s;                               \
-    sd::lub_scan_totals_kernel<<<nscan, 256, 0, st>>>(c->lub_count, static_cast<unsigned*>(c->lub_tmp), H + 1); \
+    sd::lub_scan_totals_kernel<<<nscan, 256, 0, st>>>(c->lub_count, static_cast<unsigned*>(c->lub_tmp), \
+                                                      H + 1);                                      \
     if ((s = check_launch(c, "lub_scan_totals_kernel")) != SD_OK) return s;                         \
     sd::lub_scan_apply_kernel<<<nscan, 256, 0, st>>>(c->lub_count, static_cast<const unsigned*>(c->lub_tmp), \
-                                                     c->lub_start, H + 1);                         \
+                                                     c->lub_start, c->lub_cursor, H + 1);          \
     if ((s = check_launch(c, "lub_scan_apply_kernel")) != SD_OK) return s;                          \
-    sd::lub_scatter_kernel<<<nb, 256, 0, st>>>(c->lub_cell, c->lub_start, c->lub_cursor,            \
-                                               c->lub_order, n);                                   \
+    sd::lub_scatter_kernel<<<nb, 256, 0, st>>>(c->lub_bucket, c->lub_cursor, c->lub_order, n);      \
     if ((s = check_launch(c, "lub_scatter_kernel")) != SD_OK) return s;                             \
-    sd::lub_sort_kernel<<<(H + 255) / 256, 256, 0, st>>>(c->lub_start, c->lub_order, H);            \
+    sd::lub_sort_kernel<<<(H + 255) / 256, 256, 0, st>>>(c->lub_start, c->lub_order, c->lub_count, H); \
     if ((s = check_launch(c, "lub_sort_kernel")) != SD_OK) return s;                                \
-    sd::lub_gather_kernel<T4><<<nb, 256, 0, st>>>(                                                  \
-        static_cast<const T4*>(pos), static_cast<const T4*>(vel), c->lub_cell, c->lub_order,        \
-        static_cast<T4*>(c->lub_spos), static_cast<T4*>(c->lub_svel), c->lub_scell, n);             \
+    c->lub_count_dirty = false;                                                                     \
+    sd::lub_gather_kernel<T4><<<nb, 256, 0, st>>>(static_cast<const T4*>(pos), static_cast<const T4*>(vel), \
+                                                  c->lub_order, static_cast<T4*>(c->lub_spos),      \
+                                                  static_cast<T4*>(c->lub_svel), n);                \
     if ((s = check_launch(c, "lub_gather_kernel")) != SD_OK) return s;                              \
-    if (n >= 262144)                                                                                \
-        sd::lub_force_kernel<T4, 1><<<(n + 127) / 128, 128, 0, st>>>(SD_LUB_FORCE_ARGS(T4));        \
+    if (n >= sd::kLubOneLaneMinN)                                                                   \
+        sd::lub_force_kernel<T4, 1><<<(n + 127) / 128, sd::kLubThreads, 0, st>>>(SD_LUB_FORCE_ARGS(T4)); \
     else if (n >= 32768)                                                                            \
-        sd::lub_force_kernel<T4, 8><<<(n * 8 + 127) / 128, 128, 0, st>>>(SD_LUB_FORCE_ARGS(T4));    \
+        sd::lub_force_kernel<T4, 8><<<(n * 8 + 127) / 128, sd::kLubThreads, 0, st>>>(SD_LUB_FORCE_ARGS(T4)); \
     else                                                                                            \
-        sd::lub_force_kernel<T4, 32><<<(n * 32 + 127) / 128, 128, 0, st>>>(SD_LUB_FORCE_ARGS(T4));  \
+        sd::lub_force_kernel<T4, 32><<<(n * 32 + 127) / 128, sd::kLubThreads, 0, st>>>(SD_LUB_FORCE_ARGS(T4)); \
     return check_launch(c, "lub_force_kernel")
     if (c->precision == SD_PREC_F64) {
         SD_LUB(double4);
@@ -1288,7 +1325,7 @@ sd_status sd_step(sd_ctx* ctx, void* pos, sd_force_fn fn, void* user, const void
         key.integrator = static_cast<int>(integrator);
         if (!ctx->gexec || std::memcmp(&key, &ctx->gkey, sizeof(GraphKey)) != 0) {
             drop_graph(ctx);
-            if (lub && (s = ensure_lub_buffers(ctx)) != SD_OK) return s;
+            if (lub && ctx->N > sd::kLubOneCtaMaxN && (s = ensure_lub_buffers(ctx)) != SD_OK) return s;
             if (!ctx->cap_stream) SD_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->cap_stream, cudaStreamNonBlocking));
             const long long launches0 = ctx->launches;
             SD_CUDA(ctx, cudaStreamBeginCapture(ctx->cap_stream, cudaStreamCaptureModeThreadLocal));

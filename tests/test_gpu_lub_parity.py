@@ -46,7 +46,8 @@ def _row_err(got, want):
 
 @pytest.mark.parametrize("prec_name,tol", [("PREC_F32_KAHAN", 2e-7), ("PREC_F64", 1e-12)])
 @pytest.mark.parametrize("boxed", [False, True])
-@pytest.mark.parametrize("n,phi", [(50, 0.1), (3000, 0.05), (40000, 0.05)])
+@pytest.mark.parametrize("n,phi", [(50, 0.1), (1500, 0.05), (3000, 0.05), (4096, 0.2), (5000, 0.05),
+                                   (40000, 0.05), (70001, 0.05), (50000, 0.3)])
 def test_lubrication_apply_all_rows(gpu, prec_name, tol, boxed, n, phi):
     """Uniform clouds with overlaps allowed: pairs inside 3a (about 27 phi per sphere), in contact,
     overlapping (s clamped) and, when boxed, through the faces; per-particle external forces."""
@@ -92,13 +93,16 @@ def test_lubrication_apply_all_rows(gpu, prec_name, tol, boxed, n, phi):
 
 @pytest.mark.parametrize("prec_name,tol", [("PREC_F32_KAHAN", 2e-7), ("PREC_F64", 1e-12)])
 @pytest.mark.parametrize("boxed", [False, True])
-@pytest.mark.parametrize("n0,phi", [(60, 0.1), (3000, 0.05), (40000, 0.05)])
+@pytest.mark.parametrize("n0,phi", [(60, 0.1), (1500, 0.05), (3000, 0.05), (4096, 0.2), (5000, 0.05),
+                                    (40000, 0.05), (70001, 0.05), (50000, 0.3)])
 def test_lubrication_apply_against_the_plain_definition(gpu, prec_name, tol, boxed, n0, phi):
     """Eq. (8) with the cut-off decided as the paper states it (r < 3a, in double) and the plain
     `remainder` image: the same uniform clouds as above (overlaps, contacts, pairs through the
     faces) after one member of every pair within GUARD of r = 3a has been removed (CPU pre-check on
     the rounded coordinates; a component near half a box cannot matter here: such a pair is at
-    least 4.5 a apart in either image).  All rows; all-pairs kernel (N <= 2560) and cell grid."""
+    least 4.5 a apart in either image).  All rows; every dispatch class: all pairs (N <= 1024), the
+    one-launch grid (<= 4096), the cell grid with 32 / 8 / 1 lanes per particle (the last one with
+    full queues at phi = 0.3)."""
     torch, sd = gpu
     dt = _dt(prec_name)
     L = wl.cube_side(n0, phi)
@@ -136,8 +140,9 @@ def test_lubrication_apply_against_the_plain_definition(gpu, prec_name, tol, box
 @pytest.mark.parametrize("prec_name,tol", [("PREC_F32_KAHAN", 2e-7), ("PREC_F64", 1e-12)])
 def test_lubrication_box_side_limits(gpu, prec_name, tol):
     """A pair inside 3a must have one nearest image: the box side has to exceed 6a.  The all-pairs
-    kernel (N <= 2560) works from there on -- checked against the plain definition in a box of 7a,
-    where most pairs interact through a face -- the cell grid above that size needs 9a."""
+    kernel (N <= 1024, and up to 4096 when the box is too small for a grid) works from there on --
+    checked against the plain definition in a box of 7a, where most pairs interact through a face --
+    the cell grid above that size needs 9a."""
     torch, sd = gpu
     dt = _dt(prec_name)
     n = 40
@@ -162,6 +167,43 @@ def test_lubrication_box_side_limits(gpu, prec_name, tol):
     corr = orc.lubrication(p[:, :3].astype(np.float64), v[:, :3].astype(np.float64), wl.A, wl.ETA, box=L)
     assert np.count_nonzero(np.abs(corr).sum(axis=1)) > n // 2
     assert _row_err(out.cpu().numpy()[:, :3].astype(np.float64), np.array([0.0, 0.0, -1.0]) - corr) <= tol
+    ctx.close()
+
+
+@pytest.mark.parametrize("prec_name,tol", [("PREC_F32_KAHAN", 2e-7), ("PREC_F64", 1e-12)])
+def test_lubrication_small_box_between_1024_and_4096_particles(gpu, prec_name, tol):
+    """1024 < N <= 4096 in a box of 8a (two cells per edge: no grid): the all-pairs kernel, against
+    the plain definition; N = 5000 in the same box is refused."""
+    torch, sd = gpu
+    dt = _dt(prec_name)
+    n0, L = 1500, 8.0
+    rng = np.random.Generator(np.random.PCG64(wl.SEED_BASE + 350))
+    pos = rng.uniform(0.0, L, size=(n0, 3))           # heavily overlapping: s is clamped on most pairs
+    Ls = float(np.float32(L)) if dt == np.float32 else L
+    p0 = wl.to_xyzw(pos, dt)[:, :3].astype(np.float64)
+    keep = guards.drop_one_of_each(n0, guards.pairs_in_shell(p0, 3.0 * wl.A - GUARD, 3.0 * wl.A + GUARD, Ls))
+    pos = pos[keep][:1200]
+    n = pos.shape[0]
+    assert n > 1024
+    vel = wl.normal_forces(n, wl.SEED_BASE + 351)
+    p, v = wl.to_xyzw(pos, dt), wl.to_xyzw(vel, dt)
+    ctx = sd.Context(n, wl.A, wl.ETA)
+    ctx.set_precision(getattr(sd, prec_name))
+    ctx.set_box(L)
+    out = torch.full((n, 4), float("nan"), device="cuda", dtype=torch.float64 if dt == np.float64 else torch.float32)
+    ctx.lubrication_apply(torch.from_numpy(p).cuda(), torch.from_numpy(v).cuda(), out, gravity=(0.0, 0.0, -1.0))
+    torch.cuda.synchronize()
+    corr = orc.lubrication(p[:, :3].astype(np.float64), v[:, :3].astype(np.float64), wl.A, wl.ETA,
+                           box=Ls, image=orc.IMAGE_DEFINITION, decide_f32=False)
+    assert _row_err(out.cpu().numpy()[:, :3].astype(np.float64), np.array([0.0, 0.0, -1.0]) - corr) <= tol
+    ctx.close()
+    ctx = sd.Context(5000, wl.A, wl.ETA)
+    ctx.set_precision(getattr(sd, prec_name))
+    ctx.set_box(L)
+    z = torch.zeros((5000, 4), device="cuda", dtype=out.dtype)
+    with pytest.raises(sd.SdError) as e:
+        ctx.lubrication_apply(z, z.clone(), z.clone())
+    assert e.value.status == sd.ERR_UNSUPPORTED
     ctx.close()
 
 
