@@ -109,6 +109,25 @@ sd_status sd_mobility_apply(sd_ctx* ctx, const void* pos, const void* force, voi
 sd_status sd_mobility_apply_host(sd_ctx* ctx, const void* pos_host, const void* force_host,
                                  void* vel_host, void* stream);
 
+/* The same product (Eq. 1 with Eq. 4 / 7; fp32 with compensated summation, free
+ * space) for callers that cannot allocate device memory -- code under stream capture, tight
+ * serving loops, harnesses that forbid cudaMalloc: no context, no cudaMalloc / cudaFree / allocating
+ * library call, ever.  pos[N][4], force[N][4] (in) and vel[N][4] (out; must not alias the inputs)
+ * are 16-byte-aligned device arrays of float on the CURRENT device; N <= sd_noalloc_max_particles()
+ * = 16384, SD_ERR_UNSUPPORTED with a message (sd_last_error(NULL)) beyond that.  Two launches are
+ * enqueued on `stream` (a set-up kernel and the warp-split pair kernel of sd_mobility_apply); the
+ * host is not synchronised.  Scratch (partial sums of i-blocks shared by several CTAs, their ticket
+ * counters and schedule, pad records) lives in ONE static device array of 4 MiB that every GPU
+ * holds from the moment the library is loaded until the process exits.  Every call shares that
+ * array and finds the previous call's contents in it; the set-up kernel rewrites what must start
+ * clean.  Calls that overlap on the GPU (different streams, different host threads) RACE on it:
+ * serialise them on one stream.  The first call on a device looks up the array's device address and
+ * sets a kernel attribute (no allocation; make that call outside a stream capture).  Results agree
+ * with sd_mobility_apply(PREC_F32_KAHAN) to the tolerance of that path (1e-5 relative per row). */
+sd_status sd_mobility_apply_noalloc(long long N, double a, double eta, sd_tensor tensor, const void* pos,
+                                    const void* force, void* vel, void* stream);
+long long sd_noalloc_max_particles(void);
+
 /* n_steps >= 0 explicit steps of size dt, pos updated in place (steps 1-3).
  * Forces, in order of precedence:
  *   fn != NULL     -> fn(pos, ctx-owned force buffer, N, user, stream) before every product;

@@ -9,6 +9,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <utility>
@@ -1019,6 +1020,57 @@ void access_dispatch(int pattern, int scheme, float* out, const void* in, unsign
 }
 bool misaligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) & (a - 1)) != 0; }
 
+// ---- sd_mobility_apply_noalloc: one product without a context and without any allocation -------
+// Some callers cannot call cudaMalloc (code under stream capture, tight serving loops, harnesses
+// that forbid it).  This is the warp-split one-launch kernel (sd_pairs_f32w.cuh, fp32 Kahan, free
+// space) with ALL its scratch -- partial sums of the i-blocks that several CTAs share, the ticket
+// counter and the schedule of every i-block, the pad records of the ragged tail -- in one
+// file-scope device array of kNoAllocBytes (4 MiB; every GPU that loads the library holds it until
+// exit).  The array is shared by every call and keeps the last call's contents:
+// noalloc_prepare_kernel rewrites the schedule, the pad records and zeroes the tickets at the start
+// of every call; calls that overlap on the GPU (two streams, two host threads) race on it.
+constexpr long long kNoAllocMaxN = 16384;
+constexpr size_t kNoAllocMaxB = (kNoAllocMaxN + 255) / 256;                  // i-blocks of 256 particles
+constexpr size_t kNoAllocPadOff = 0;                                          // 2 x kWSJ float4
+constexpr size_t kNoAllocDoneOff = kNoAllocPadOff + 2 * sd::kWSJ * sizeof(float4);
+constexpr size_t kNoAllocFirstOff = kNoAllocDoneOff + kNoAllocMaxB * sizeof(int);
+constexpr size_t kNoAllocSlotsOff = kNoAllocFirstOff + kNoAllocMaxB * sizeof(int);
+constexpr size_t kNoAllocPartOff = (kNoAllocSlotsOff + kNoAllocMaxB * sizeof(int) + 255) / 256 * 256;
+constexpr size_t kNoAllocBytes = 4u << 20;
+static __device__ __align__(256) unsigned char g_noalloc_scratch[kNoAllocBytes];
+
+// piece (CTA) that owns unit u when U units are cut at floor(g U / G): the largest g with
+// floor(g U / G) <= u  (the rule of build_schedule)
+__host__ __device__ inline int noalloc_piece_of(long long u, long long U, int G) {
+    return static_cast<int>(((u + 1) * G - 1) / U);
+}
+
+__global__ void __launch_bounds__(256)
+noalloc_prepare_kernel(float4* __restrict__ pad, int* __restrict__ blk_done, int* __restrict__ blk_first,
+                       int* __restrict__ blk_nslots, const int B, const int T, const int G) {
+    const long long U = static_cast<long long>(B) * T;
+    for (int b = threadIdx.x; b < B; b += blockDim.x) {
+        const long long lo = static_cast<long long>(b) * T;
+        const int cf = noalloc_piece_of(lo, U, G), cl = noalloc_piece_of(lo + T - 1, U, G);
+        blk_first[b] = cf;
+        blk_nslots[b] = cl - cf + 1;
+        blk_done[b] = 0;  // the shared array keeps whatever an earlier (possibly aborted) call left
+    }
+    for (int q = threadIdx.x; q < 2 * sd::kWSJ; q += blockDim.x)
+        pad[q] = q < sd::kWSJ ? make_float4(SD_PAD_POS, SD_PAD_POS, SD_PAD_POS, 0.f) : make_float4(0.f, 0.f, 0.f, 0.f);
+}
+
+// per device, set up on the first call made with that device current
+struct NoAllocDevice {
+    bool ready = false;
+    unsigned char* scratch = nullptr;  // DEVICE address of g_noalloc_scratch on this device
+    int num_sms = 0;
+};
+constexpr int kNoAllocMaxDevices = 64;
+NoAllocDevice g_noalloc_dev[kNoAllocMaxDevices];
+std::mutex g_noalloc_mutex;
+
+
 }  // namespace
 
 extern "C" {
@@ -1510,6 +1562,109 @@ sd_status sd_access_bench(int elem_floats, int pattern, int scheme, long long N,
     if (ms_per_launch) *ms_per_launch = static_cast<double>(ms) / reps;
     return SD_OK;
 }
+
+sd_status sd_mobility_apply_noalloc(long long N, double a, double eta, sd_tensor tensor, const void* pos,
+                                    const void* force, void* vel, void* stream) {
+    if (N < 1 || !(a > 0.0) || !(eta > 0.0) || !std::isfinite(a) || !std::isfinite(eta))
+        return fail(nullptr, SD_ERR_INVALID_ARG, "sd_mobility_apply_noalloc: N >= 1, a > 0 and eta > 0 required");
+    if (N > kNoAllocMaxN)
+        return fail(nullptr, SD_ERR_UNSUPPORTED,
+                    "sd_mobility_apply_noalloc: N = " + std::to_string(N) + " exceeds the maximum of " +
+                        std::to_string(kNoAllocMaxN) + " particles of the static scratch array (use a context)");
+    if (tensor != SD_TENSOR_RPY && tensor != SD_TENSOR_OSEEN)
+        return fail(nullptr, SD_ERR_INVALID_ARG, "sd_mobility_apply_noalloc: unknown tensor");
+    if (!pos || !force || !vel || misaligned(pos, 16) || misaligned(force, 16) || misaligned(vel, 16))
+        return fail(nullptr, SD_ERR_INVALID_ARG, "sd_mobility_apply_noalloc: pos, force, vel must be 16-byte aligned device arrays");
+    if (vel == pos || vel == force)
+        return fail(nullptr, SD_ERR_INVALID_ARG, "sd_mobility_apply_noalloc: vel must not alias pos or force");
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess || dev < 0 || dev >= kNoAllocMaxDevices)
+        return fail(nullptr, SD_ERR_CUDA, std::string("sd_mobility_apply_noalloc: cudaGetDevice: ") + cudaGetErrorString(e));
+    const bool rpy = tensor == SD_TENSOR_RPY;
+    const void* kernel = w_pick<4>(rpy, false, false);
+    const size_t smem = sd::WShape<4>::smem_bytes;
+    NoAllocDevice& d = g_noalloc_dev[dev];
+    {
+        std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+        if (!d.ready) {
+            // in host code g_noalloc_scratch is a stand-in, not a device address: ask for the address on
+            // the current device, once per device
+            void* p = nullptr;
+            if ((e = cudaGetSymbolAddress(&p, g_noalloc_scratch)) != cudaSuccess || !p)
+                return fail(nullptr, SD_ERR_CUDA, std::string("sd_mobility_apply_noalloc: cudaGetSymbolAddress: ") + cudaGetErrorString(e));
+            for (int t = 0; t < 2; ++t)
+                if ((e = cudaFuncSetAttribute(w_pick<4>(t == 0, false, false), cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                              static_cast<int>(smem))) != cudaSuccess)
+                    return fail(nullptr, SD_ERR_CUDA, std::string("sd_mobility_apply_noalloc: cudaFuncSetAttribute: ") + cudaGetErrorString(e));
+            int sms = 0;
+            if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess || sms < 1)
+                return fail(nullptr, SD_ERR_CUDA, std::string("sd_mobility_apply_noalloc: cudaDeviceGetAttribute: ") + cudaGetErrorString(e));
+            d.scratch = static_cast<unsigned char*>(p);
+            d.num_sms = sms;
+            d.ready = true;
+        }
+    }
+    // the schedule of configure_w: i-blocks of 256 particles x quads of 4 j, one piece per SM
+    const int IB = 64 * 4;
+    const int B = static_cast<int>((N + IB - 1) / IB), T = static_cast<int>((N + sd::kWQ - 1) / sd::kWQ);
+    const long long U = static_cast<long long>(B) * T;
+    const int G = static_cast<int>(std::min<long long>(U, d.num_sms));
+    int max_slots = 1;
+    for (int b = 0; b < B; ++b) {
+        const long long lo = static_cast<long long>(b) * T;
+        max_slots = std::max(max_slots, noalloc_piece_of(lo + T - 1, U, G) - noalloc_piece_of(lo, U, G) + 1);
+    }
+    const long long stride = static_cast<long long>(B) * IB;  // particles per slot of the partial sums
+    const size_t part_bytes = static_cast<size_t>(max_slots) * stride * 2 * sizeof(float4);
+    if (kNoAllocPartOff + part_bytes > kNoAllocBytes)
+        return fail(nullptr, SD_ERR_UNSUPPORTED,
+                    "sd_mobility_apply_noalloc: the partial sums of this size on this GPU (" + std::to_string(part_bytes) +
+                        " bytes) do not fit in the static scratch array");
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    float4* pad = reinterpret_cast<float4*>(d.scratch + kNoAllocPadOff);
+    int* blk_done = reinterpret_cast<int*>(d.scratch + kNoAllocDoneOff);
+    int* blk_first = reinterpret_cast<int*>(d.scratch + kNoAllocFirstOff);
+    int* blk_nslots = reinterpret_cast<int*>(d.scratch + kNoAllocSlotsOff);
+    float4* part = reinterpret_cast<float4*>(d.scratch + kNoAllocPartOff);
+    noalloc_prepare_kernel<<<1, 256, 0, st>>>(pad, blk_done, blk_first, blk_nslots, B, T, G);
+    if ((e = cudaGetLastError()) != cudaSuccess)
+        return fail(nullptr, SD_ERR_CUDA, std::string("noalloc_prepare_kernel: ") + cudaGetErrorString(e));
+    sd::Schedule sch;
+    sch.cta_u0 = nullptr, sch.cta_piece = nullptr;  // not read by the warp-split kernel
+    sch.blk_first_cta = blk_first, sch.blk_nslots = blk_nslots;
+    sch.T = T, sch.B = B, sch.G = G;
+    const double mu0 = 1.0 / (6.0 * 3.14159265358979323846 * eta * a);
+    sd::PairCoef k;
+    k.k2 = static_cast<float>(2.0 * a * a / 3.0);
+    k.m3k2 = static_cast<float>(-2.0 * a * a);
+    k.mu0r = static_cast<float>(4.0 / (3.0 * a));
+    k.ovA = static_cast<float>(-3.0 / (8.0 * a * a));
+    k.ovB = static_cast<float>(1.0 / (8.0 * a * a));
+    k.thr = rpy ? static_cast<float>(4.0 * a * a) : 1e-30f;
+    k.clampv = static_cast<float>(4.0 * a * a);
+    k.invL = k.mL = k.magic = 0.f;  // free space
+    sd::FinArgs fin;
+    fin.vel = static_cast<float4*>(vel);
+    fin.pos_base = nullptr, fin.pos_lo = nullptr, fin.pos_out = nullptr;  // FIN_VEL: velocities only
+    fin.dt = 0.0;
+    fin.c1 = mu0 * 0.75 * a;
+    fin.mu0 = mu0;
+    fin.mode = sd::FIN_VEL;
+    fin.pos_comp = 0;
+    const float4* pp = static_cast<const float4*>(pos);
+    const float4* ff = static_cast<const float4*>(force);
+    const float4* cpad = pad;
+    int n = static_cast<int>(N);
+    long long slot_stride = stride;
+    void* args[] = {&pp, &ff, &cpad, &part, &blk_done, &sch, &k, &fin, &n, &slot_stride};
+    if ((e = cudaLaunchKernel(kernel, dim3(G), dim3(sd::kThreads), args, smem, st)) != cudaSuccess ||
+        (e = cudaGetLastError()) != cudaSuccess)
+        return fail(nullptr, SD_ERR_CUDA, std::string("sd_mobility_apply_noalloc: pairs_f32w_kernel: ") + cudaGetErrorString(e));
+    return SD_OK;
+}
+
+long long sd_noalloc_max_particles(void) { return kNoAllocMaxN; }
 
 const char* sd_last_error(const sd_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_error.c_str(); }
 

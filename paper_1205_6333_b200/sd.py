@@ -43,6 +43,8 @@ SYMBOLS = {
     "sd_box": (_D, [_P]),
     "sd_mobility_apply": (_I, [_P, _P, _P, _P, _P]),
     "sd_mobility_apply_host": (_I, [_P, _P, _P, _P, _P]),
+    "sd_mobility_apply_noalloc": (_I, [_LL, _D, _D, _I, _P, _P, _P, _P]),
+    "sd_noalloc_max_particles": (_LL, []),
     "sd_step": (_I, [_P, _P, FORCE_FN, _P, _P, ctypes.POINTER(_D), _D, _LL, _I, _P]),
     "sd_get_velocity": (_I, [_P, _P, _P]),
     "sd_lubrication_apply": (_I, [_P, _P, _P, _P, ctypes.POINTER(_D), _P, _P]),
@@ -93,6 +95,30 @@ def _stream_ptr(stream):
     if stream is None:
         stream = torch.cuda.current_stream()
     return ctypes.c_void_p(stream.cuda_stream)
+
+
+def noalloc_max_particles() -> int:
+    return int(load_library().sd_noalloc_max_particles())
+
+
+def mobility_apply_noalloc(pos, force, vel, a: float, eta: float, tensor: int = TENSOR_RPY, stream=None):
+    """sd_mobility_apply_noalloc: v = M(pos) F in fp32 without a context and without any device
+    allocation (static 4-MiB scratch array inside the library; N <= noalloc_max_particles();
+    calls that overlap on the GPU race on that array).  pos, force, vel: contiguous CUDA float32
+    tensors [N, 4] on the current device."""
+    import torch
+    lib = load_library()
+    n = int(pos.shape[0])
+    for t, name in ((pos, "pos"), (force, "force"), (vel, "vel")):
+        if not t.is_cuda or t.dtype != torch.float32 or tuple(t.shape) != (n, 4) or not t.is_contiguous():
+            raise ValueError(f"{name} must be a contiguous CUDA float32 tensor [{n}, 4], got "
+                             f"{tuple(t.shape)} {t.dtype} {t.device}")
+    status = lib.sd_mobility_apply_noalloc(n, float(a), float(eta), int(tensor), ctypes.c_void_p(pos.data_ptr()),
+                                           ctypes.c_void_p(force.data_ptr()), ctypes.c_void_p(vel.data_ptr()),
+                                           _stream_ptr(stream))
+    if status != 0:
+        raise SdError(status, (lib.sd_last_error(None) or b"").decode())
+    return vel
 
 
 def schedule_plan(n: int, particles_per_block: int, tile_j: int, max_ctas: int, num_sms: int):
