@@ -375,7 +375,7 @@ def run_lub(args, rank):
                 config={"workload": name,
                         "kernel": ("lub_small (all pairs)" if n <= 1024 else "lub_one_launch (grid in shared memory)"
                                    if n <= 4096 else "lub_count + lub_scan_totals + lub_scan_apply + lub_scatter + "
-                                   "lub_sort + lub_gather + lub_force"),
+                                   "lub_gather + lub_force"),
                         "parallelism": "1 GPU", "l2": "L2 flushed with a 256 MiB write between timed iterations"},
                 clocks=clocks, gpu_launches=gpu_launches,
                 e2e={"value": args.steps * n / e2e, "unit": "particles/s", "h2d_bytes_per_step": 3 * rec,

@@ -74,11 +74,12 @@ struct sd_ctx {
     unsigned* lub_count = nullptr;   // [H + 1] bucket histogram (left zeroed by every call)
     unsigned* lub_start = nullptr;   // [H + 1] exclusive scan of it
     unsigned* lub_cursor = nullptr;  // [H]
-    int* lub_order = nullptr;        // [N] particle indices grouped by bucket
+    int2* lub_slots = nullptr;       // [N] (particle, bucket) grouped by bucket, as the scatter left them
+    int* lub_order = nullptr;        // [N] particle indices grouped by bucket, sorted within a bucket
     void* lub_spos = nullptr;        // [N] positions, velocities in bucket order
     void* lub_svel = nullptr;
     bool lub_one_launch_ready = false;  // shared-memory attribute of lub_one_launch_kernel set
-    bool lub_count_dirty = false;    // a call was abandoned between lub_count_kernel and lub_sort_kernel
+    bool lub_count_dirty = false;    // a call was abandoned between lub_count_kernel and lub_gather_kernel
     void* lub_tmp = nullptr;         // block totals of the bucket scan
     size_t lub_tmp_bytes = 0;
     unsigned lub_H = 0;
@@ -204,7 +205,8 @@ void free_buffers(sd_ctx* c) {
     }
     void** lub[] = {reinterpret_cast<void**>(&c->lub_bucket), reinterpret_cast<void**>(&c->lub_count),
                     reinterpret_cast<void**>(&c->lub_start), reinterpret_cast<void**>(&c->lub_cursor),
-                    reinterpret_cast<void**>(&c->lub_order), &c->lub_tmp, &c->lub_spos, &c->lub_svel};
+                    reinterpret_cast<void**>(&c->lub_order), reinterpret_cast<void**>(&c->lub_slots), &c->lub_tmp,
+                    &c->lub_spos, &c->lub_svel};
     for (void** b : lub) {
         if (*b) cudaFree(*b);
         *b = nullptr;
@@ -858,7 +860,7 @@ sd_status ensure_lub_buffers(sd_ctx* c) {
     if (!c->lub_spos) SD_CUDA(c, cudaMalloc(&c->lub_spos, 4 * elem_size(c->precision) * n));
     if (!c->lub_svel) SD_CUDA(c, cudaMalloc(&c->lub_svel, 4 * elem_size(c->precision) * n));
     if (!c->lub_bucket) SD_CUDA(c, cudaMalloc(&c->lub_bucket, sizeof(unsigned) * n));
-    if (!c->lub_count) {  // zeroed once here; every call leaves it zeroed (lub_sort_kernel)
+    if (!c->lub_count) {  // zeroed once here; every call leaves it zeroed (lub_gather_kernel)
         SD_CUDA(c, cudaMalloc(&c->lub_count, sizeof(unsigned) * (H + 1)));
         SD_CUDA(c, cudaMemset(c->lub_count, 0, sizeof(unsigned) * (H + 1)));
         c->lub_count_dirty = false;
@@ -866,6 +868,7 @@ sd_status ensure_lub_buffers(sd_ctx* c) {
     if (!c->lub_start) SD_CUDA(c, cudaMalloc(&c->lub_start, sizeof(unsigned) * (H + 1)));
     if (!c->lub_cursor) SD_CUDA(c, cudaMalloc(&c->lub_cursor, sizeof(unsigned) * H));
     if (!c->lub_order) SD_CUDA(c, cudaMalloc(&c->lub_order, sizeof(int) * n));
+    if (!c->lub_slots) SD_CUDA(c, cudaMalloc(&c->lub_slots, sizeof(int2) * n));
     if (!c->lub_tmp) {  // block totals of the two-launch scan
         c->lub_tmp_bytes = sizeof(unsigned) * ((H + 1 + sd::kScanBlock - 1) / sd::kScanBlock);
         SD_CUDA(c, cudaMalloc(&c->lub_tmp, c->lub_tmp_bytes));
@@ -975,15 +978,13 @@ sd_status launch_lubrication(sd_ctx* c, const void* pos, const void* vel, const 
     sd::lub_scan_apply_kernel<<<nscan, 256, 0, st>>>(c->lub_count, static_cast<const unsigned*>(c->lub_tmp), \
                                                      c->lub_start, c->lub_cursor, H + 1);          \
     if ((s = check_launch(c, "lub_scan_apply_kernel")) != SD_OK) return s;                          \
-    sd::lub_scatter_kernel<<<nb, 256, 0, st>>>(c->lub_bucket, c->lub_cursor, c->lub_order, n);      \
+    sd::lub_scatter_kernel<<<nb, 256, 0, st>>>(c->lub_bucket, c->lub_cursor, c->lub_slots, n);      \
     if ((s = check_launch(c, "lub_scatter_kernel")) != SD_OK) return s;                             \
-    sd::lub_sort_kernel<<<(H + 255) / 256, 256, 0, st>>>(c->lub_start, c->lub_order, c->lub_count, H); \
-    if ((s = check_launch(c, "lub_sort_kernel")) != SD_OK) return s;                                \
-    c->lub_count_dirty = false;                                                                     \
     sd::lub_gather_kernel<T4><<<nb, 256, 0, st>>>(static_cast<const T4*>(pos), static_cast<const T4*>(vel), \
-                                                  c->lub_order, static_cast<T4*>(c->lub_spos),      \
-                                                  static_cast<T4*>(c->lub_svel), n);                \
+                                                  c->lub_slots, c->lub_start, c->lub_count, c->lub_order, \
+                                                  static_cast<T4*>(c->lub_spos), static_cast<T4*>(c->lub_svel), n); \
     if ((s = check_launch(c, "lub_gather_kernel")) != SD_OK) return s;                              \
+    c->lub_count_dirty = false;                                                                     \
     if (n >= sd::kLubOneLaneMinN)                                                                   \
         sd::lub_force_kernel<T4, 1><<<(n + 127) / 128, sd::kLubThreads, 0, st>>>(SD_LUB_FORCE_ARGS(T4)); \
     else if (n >= 32768)                                                                            \

@@ -18,11 +18,12 @@
 //                       block adds the totals before it to its own scan), written twice: bucket
 //                       starts and the scatter cursors
 //   lub_scatter_kernel  particle indices into their buckets (atomic cursor), then
-//   lub_sort_kernel     each bucket sorted by particle index: the summation order below, and
-//                       with it every bit of the result, does not depend on the atomics; clears
-//                       the histogram for the next call
 //   lub_gather_kernel   positions and velocities copied into bucket order (the paper's
-//                       "particle reordering"): neighbouring cells are neighbouring memory
+//                       "particle reordering": neighbouring cells are neighbouring memory), within
+//                       a bucket by particle index (every thread ranks its particle among those
+//                       of its bucket): the summation order below, and with it every bit of the
+//                       result, does not depend on the atomics; clears the histogram for the
+//                       next call
 //   lub_force_kernel    particles in bucket order.  N large, one lane per particle: the lane walks
 //                       its 9 runs with an all-fp32 test (fp64 contexts: the fp64 decision) and
 //                       queues the candidates that pass in shared memory; the warp then evaluates
@@ -86,13 +87,15 @@ lub_count_kernel(const T4* __restrict__ pos, unsigned* __restrict__ bucket, unsi
     atomicAdd(&count[h], 1u);
 }
 
-// cursor[h] starts at start[h] (lub_scan_apply_kernel)
+// cursor[h] starts at start[h] (lub_scan_apply_kernel).  slots[k] = (particle, bucket) of slot k:
+// grouped by bucket, in the order the atomics happened to give within a bucket
 __global__ void __launch_bounds__(256)
 lub_scatter_kernel(const unsigned* __restrict__ bucket, unsigned* __restrict__ cursor,
-                   int* __restrict__ order, const int N) {
+                   int2* __restrict__ slots, const int N) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N) return;
-    order[atomicAdd(&cursor[bucket[i]], 1u)] = i;
+    const unsigned h = bucket[i];
+    slots[atomicAdd(&cursor[h], 1u)] = make_int2(i, static_cast<int>(h));
 }
 
 // Exclusive scan of n counters, two launches, blocks of kScanBlock elements (256 threads x 8):
@@ -202,27 +205,29 @@ __device__ __forceinline__ void lub_sort_run(int* order, const unsigned b, const
     }
 }
 
-// one thread per bucket; also leaves the histogram zeroed for the next call
-__global__ void __launch_bounds__(256)
-lub_sort_kernel(const unsigned* __restrict__ start, int* __restrict__ order, unsigned* __restrict__ count,
-                const unsigned H) {
-    const unsigned h = blockIdx.x * blockDim.x + threadIdx.x;
-    if (h >= H) return;
-    const unsigned b = start[h], e = start[h + 1];
-    if (e != b) count[h] = 0u;
-    lub_sort_run(order, b, e);
-}
-
-// sorted copies: particle data in bucket order, so that the force kernel reads contiguous runs
+// Sorted copies: particle data in bucket order, so that the force kernel reads contiguous runs,
+// and within a bucket in the order of the particle index: the summation order of the force
+// kernel, and with it every bit of the result, does not depend on the atomics of the scatter.
+// Thread k takes the particle the scatter left in slot k, finds its rank among the (handful of)
+// particles of its bucket and writes it to slot start + rank; the first slot of every bucket also
+// clears the bucket's counter for the next call.
 template <typename T4>
 __global__ void __launch_bounds__(256)
-lub_gather_kernel(const T4* __restrict__ pos, const T4* __restrict__ vel, const int* __restrict__ order,
+lub_gather_kernel(const T4* __restrict__ pos, const T4* __restrict__ vel, const int2* __restrict__ slots,
+                  const unsigned* __restrict__ start, unsigned* __restrict__ count, int* __restrict__ order,
                   T4* __restrict__ spos, T4* __restrict__ svel, const int N) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= N) return;
-    const int i = order[k];
-    spos[k] = pos[i];
-    svel[k] = vel[i];
+    const int2 me = slots[k];
+    const T4 p = pos[me.x];
+    const T4 v = vel[me.x];
+    const unsigned b = start[me.y], e = start[me.y + 1];
+    if (static_cast<unsigned>(k) == b) count[me.y] = 0u;
+    unsigned slot = b;
+    for (unsigned q = b; q < e; ++q) slot += slots[q].x < me.x ? 1u : 0u;
+    order[slot] = me.x;
+    spos[slot] = p;
+    svel[slot] = v;
 }
 
 // nearest-image displacement of one component as a double, by the rule of the pair kernels
