@@ -173,8 +173,8 @@ const void* f32_kernel() {
 // 8 particles per thread at N >= kRepairMaxN: the round-1 careful pass (see sd_pairs_f32.cuh)
 template <bool PBC>
 const void* f32_pick_large(bool rpy, bool plain) {
-    return rpy ? (plain ? f32_kernel<4, 0, 1, PBC, sd::kTJ, 0>() : f32_kernel<4, 0, 0, PBC, sd::kTJ, 0>())
-               : (plain ? f32_kernel<4, 1, 1, PBC, sd::kTJ, 0>() : f32_kernel<4, 1, 0, PBC, sd::kTJ, 0>());
+    return rpy ? (plain ? f32_kernel<4, 0, 1, PBC, sd::kTJLarge, 0>() : f32_kernel<4, 0, 0, PBC, sd::kTJLarge, 0>())
+               : (plain ? f32_kernel<4, 1, 1, PBC, sd::kTJLarge, 0>() : f32_kernel<4, 1, 0, PBC, sd::kTJLarge, 0>());
 }
 template <int I, int TENSOR, bool PBC>
 const void* f64_kernel() {
@@ -338,7 +338,8 @@ sd_status configure(sd_ctx* c) {
         // 2 particles per thread: 32-record tiles once there are enough of them to pay for the extra
         // slots and hand-overs (four times the work units: finer balance over 444 CTAs)
         const bool small_tiles = i2 == 1 && c->N >= sd::kTJSmallMinN && c->N <= sd::kTJSmallMaxN;
-        cfg.TJ = small_tiles ? sd::kTJSmall : sd::kTJ;
+        const bool large = i2 == 4 && c->N >= sd::kRepairMaxN;  // 256-record tiles (sd_pairs_f32.cuh)
+        cfg.TJ = small_tiles ? sd::kTJSmall : (large ? sd::kTJLarge : sd::kTJ);
         static const char* names[3][2][2][2] = {
             {{{"pairs_f32x2_i2_rpy_kahan", "pairs_f32x2_i2_rpy_kahan_pbc"},
               {"pairs_f32x2_i2_rpy_plain", "pairs_f32x2_i2_rpy_plain_pbc"}},
@@ -353,7 +354,7 @@ sd_status configure(sd_ctx* c) {
              {{"pairs_f32x2_i8_oseen_kahan", "pairs_f32x2_i8_oseen_kahan_pbc"},
               {"pairs_f32x2_i8_oseen_plain", "pairs_f32x2_i8_oseen_plain_pbc"}}}};
         cfg.name = names[i2 == 4 ? 2 : (i2 == 2 ? 1 : 0)][rpy ? 0 : 1][plain ? 1 : 0][pbc ? 1 : 0];
-        if (i2 == 4 && c->N >= sd::kRepairMaxN)
+        if (large)
             cfg.kernel = pbc ? f32_pick_large<true>(rpy, plain) : f32_pick_large<false>(rpy, plain);
         else if (i2 == 4)
             cfg.kernel = pbc ? f32_pick<4, true>(rpy, plain) : f32_pick<4, false>(rpy, plain);
@@ -374,7 +375,7 @@ sd_status configure(sd_ctx* c) {
 #define SD_STAGED_T(I2V, TJV) SD_STAGED_R(I2V, TJV, 1)
 #define SD_STAGED(I2V) SD_STAGED_T(I2V, sd::kTJ)
             // same repair variant as the bulk-copy kernel of this size: the modes stay bit-identical
-            cfg.kernel = (i2 == 4) ? (c->N >= sd::kRepairMaxN ? SD_STAGED_R(4, sd::kTJ, 0) : SD_STAGED(4))
+            cfg.kernel = (i2 == 4) ? (large ? SD_STAGED_R(4, sd::kTJLarge, 0) : SD_STAGED(4))
                                    : ((i2 == 2) ? SD_STAGED(2)
                                                 : (small_tiles ? SD_STAGED_T(1, sd::kTJSmall) : SD_STAGED(1)));
 #undef SD_STAGED_R

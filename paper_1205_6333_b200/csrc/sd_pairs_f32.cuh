@@ -39,6 +39,15 @@ constexpr int kTJ = 128;     // j records per tile (4 KiB)
 // us), equal at 4000 and 12288, 20 % slower at N <= 3000 (30.8 -> 36.9 us: four times the slots to
 // reduce, a tile hand-over every 32 j), 1.6 % slower at 14000.  Used for kTJSmallMinN <= N <= kTJSmallMaxN.
 constexpr int kTJSmall = 32;
+// Third tile size, 256 records (8 KiB), for the 8-particle-per-thread kernel at N >= kRepairMaxN: a tile
+// hand-over (empty-barrier arrival, the next bulk copy issued by thread 0, full-barrier wait, restart of
+// the j pipeline) costs about 330 cycles of the CTA's slowest warp -- 1.2 % of a 128-record tile.
+// Measured (same box, same process, L2 flushed): N = 1 M 0.6602 -> 0.6647 of the roofline, 262 144
+// 0.6576 -> 0.6622; 32-record tiles: -1.1 ... -3.7 % at 32 768 ... 131 072.  Below kRepairMaxN the coarser
+// units cost in balance what the hand-overs save (65 536: -0.7 %, 131 072: +0.1 %); 512-record tiles need
+// dynamic shared memory, and addressing the ring through a pointer instead of the static array moved the
+// hot loop's register allocation (-1.7 % at every size).
+constexpr int kTJLarge = 256;
 constexpr int kTJSmallMinN = 4300;
 constexpr int kTJSmallMaxN = 12288;
 constexpr int kStages = 4;   // ring depth
@@ -382,7 +391,6 @@ pairs_f32_kernel(const float4* __restrict__ rec, float4* __restrict__ part, cons
                  const PairCoef k, const int N, const long long slot_stride) {
     constexpr int I = 2 * I2;
     constexpr int IB = kThreads * I;
-    static_assert(TJ * 2 <= kThreads, "STAGE_SYNC copies at most one float4 of the tile per thread");
     static_assert(TJ % kChunk == 0, "a tile is a whole number of compensation chunks");
     __shared__ __align__(128) float4 tiles[kStages][TJ * 2];
     __shared__ __align__(8) uint64_t full_bar[kStages];
@@ -465,7 +473,7 @@ pairs_f32_kernel(const float4* __restrict__ rec, float4* __restrict__ part, cons
                 tile = rec + static_cast<size_t>(t0 + tt) * (TJ * 2);
             } else {
                 __syncthreads();  // everybody is done with the previous tile
-                if (tid < TJ * 2) tiles[0][tid] = rec[static_cast<size_t>(t0 + tt) * (TJ * 2) + tid];
+                for (int q = tid; q < TJ * 2; q += kThreads) tiles[0][q] = rec[static_cast<size_t>(t0 + tt) * (TJ * 2) + q];
                 __syncthreads();
                 tile = &tiles[0][0];
             }

@@ -42,9 +42,9 @@ XU = ("MUFU",)
 
 # kernels of a large-N product: (label, mangled-name fragment, flops per pair, fp64?)
 KERNELS = [
-    ("fp32 Rotne-Prager  pairs_f32_kernel<4,RPY,Kahan,REPAIR=0>", "pairs_f32_kernelILi4ELi0ELi0ELb0ELi0ELi128ELi0E", 34, False),
-    ("fp32 Oseen         pairs_f32_kernel<4,Oseen,Kahan,REPAIR=0>", "pairs_f32_kernelILi4ELi1ELi0ELb0ELi0ELi128ELi0E", 29, False),
-    ("fp32 periodic box  pairs_f32_kernel<4,RPY,Kahan,PBC,REPAIR=0>", "pairs_f32_kernelILi4ELi0ELi0ELb1ELi0ELi128ELi0E", 49, False),
+    ("fp32 Rotne-Prager  pairs_f32_kernel<4,RPY,Kahan,REPAIR=0>", "pairs_f32_kernelILi4ELi0ELi0ELb0ELi0ELi256ELi0E", 34, False),
+    ("fp32 Oseen         pairs_f32_kernel<4,Oseen,Kahan,REPAIR=0>", "pairs_f32_kernelILi4ELi1ELi0ELb0ELi0ELi256ELi0E", 29, False),
+    ("fp32 periodic box  pairs_f32_kernel<4,RPY,Kahan,PBC,REPAIR=0>", "pairs_f32_kernelILi4ELi0ELi0ELb1ELi0ELi256ELi0E", 49, False),
     ("fp64 Rotne-Prager  pairs_f64_kernel<4,RPY>", "pairs_f64_kernelILi4ELi0ELb0E", 34, True),
     ("fp64 Oseen         pairs_f64_kernel<4,Oseen>", "pairs_f64_kernelILi4ELi1ELb0E", 29, True),
 ]

@@ -497,7 +497,7 @@ def test_forced_tiled_kernels_on_dense_small_clouds(gpu, prec_name, tol, tname, 
 
 # ---- memory-access ablation (Appendix A): same bits through every staging -----
 
-@pytest.mark.parametrize("n", [3000, 20000, 140000])
+@pytest.mark.parametrize("n", [3000, 20000, 140000, 204800])  # 204800: the 256-record tiles
 def test_staging_modes_are_bit_identical_and_guarded(gpu, n):
     """sd_set_staging: bulk-copy ring (default), naive global loads (Alg. 1), block tiling with
     barriers (Alg. 2).  The arithmetic and its order do not depend on how a record arrives."""
