@@ -33,9 +33,9 @@ FP32_LANES_PER_SM, FP64_LANES_PER_SM = 128, 64  # CUDA-core FMA lanes per SM (me
 # inside a timed bench): copied from the committed `ncu --set full` capture of the kernel this
 # commit ships, named beside it; a configuration without such a capture reports null.
 NCU_TRAFFIC = {
-    (1048576, "f32", "rpy", False): (42.2e6, "profiles/r02_pairs_ncu_full.md (dram__bytes_read.sum + "
-                                             "dram__bytes_write.sum of pairs_f32_kernel<4,RPY,Kahan>, 34.4 + 7.8 MB)"),
-    (1048576, "f32", "rpy", True): (43.9e6, "profiles/r02_pairs_ncu_full.md (pairs_f32_kernel<4,RPY,Kahan,PBC>, 34.7 + 9.2 MB)"),
+    (1048576, "f32", "rpy", False): (42.7e6, "profiles/r02_pairs_ncu_full.md (dram__bytes_read.sum + "
+                                             "dram__bytes_write.sum of pairs_f32_kernel<4,RPY,Kahan,TJ=256>, 34.4 + 8.3 MB)"),
+    (1048576, "f32", "rpy", True): (44.2e6, "profiles/r02_pairs_ncu_full.md (pairs_f32_kernel<4,RPY,Kahan,PBC,TJ=256>, 34.4 + 9.7 MB)"),
     (1048576, "f64", "rpy", False): (3.84e9, "profiles/r02_pairs_ncu_full.md (pairs_f64_kernel<4,RPY>, 3.77 GB + 74 MB: "
                                              "L2 misses of the 67-MB record stream)"),
 }
