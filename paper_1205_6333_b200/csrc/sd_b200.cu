@@ -176,18 +176,18 @@ const void* f32_pick_large(bool rpy, bool plain) {
     return rpy ? (plain ? f32_kernel<4, 0, 1, PBC, sd::kTJLarge, 0>() : f32_kernel<4, 0, 0, PBC, sd::kTJLarge, 0>())
                : (plain ? f32_kernel<4, 1, 1, PBC, sd::kTJLarge, 0>() : f32_kernel<4, 1, 0, PBC, sd::kTJLarge, 0>());
 }
-template <int I, int TENSOR, bool PBC>
+template <int I, int TENSOR, bool PBC, int TJ = sd::kTJ64>
 const void* f64_kernel() {
-    return reinterpret_cast<const void*>(&sd::pairs_f64_kernel<I, TENSOR, PBC>);
+    return reinterpret_cast<const void*>(&sd::pairs_f64_kernel<I, TENSOR, PBC, TJ>);
 }
 template <int I2, bool PBC, int TJ = sd::kTJ>
 const void* f32_pick(bool rpy, bool plain) {
     return rpy ? (plain ? f32_kernel<I2, 0, 1, PBC, TJ>() : f32_kernel<I2, 0, 0, PBC, TJ>())
                : (plain ? f32_kernel<I2, 1, 1, PBC, TJ>() : f32_kernel<I2, 1, 0, PBC, TJ>());
 }
-template <int I, bool PBC>
+template <int I, bool PBC, int TJ = sd::kTJ64>
 const void* f64_pick(bool rpy) {
-    return rpy ? f64_kernel<I, 0, PBC>() : f64_kernel<I, 1, PBC>();
+    return rpy ? f64_kernel<I, 0, PBC, TJ>() : f64_kernel<I, 1, PBC, TJ>();
 }
 
 void drop_graph(sd_ctx* c) {
@@ -394,13 +394,16 @@ sd_status configure(sd_ctx* c) {
                         "staging ablation exists for RPY, fp32-Kahan, free space only: call sd_set_staging(ctx, 0) first");
         cfg.ipt = (c->N > sd::kIpt4Min64) ? 4 : (c->N > sd::kIpt2Min64 ? 2 : 1);
         if (c->ipt_override) cfg.ipt = std::max(1, c->ipt_override / 2);
-        cfg.TJ = sd::kTJ64;
+        const bool large64 = cfg.ipt == 4 && c->N >= sd::kRepairMaxN;  // 128-record tiles (sd_pairs_f64.cuh)
+        cfg.TJ = large64 ? sd::kTJ64Large : sd::kTJ64;
         static const char* names64[3][2][2] = {
             {{"pairs_f64_i1_rpy", "pairs_f64_i1_rpy_pbc"}, {"pairs_f64_i1_oseen", "pairs_f64_i1_oseen_pbc"}},
             {{"pairs_f64_i2_rpy", "pairs_f64_i2_rpy_pbc"}, {"pairs_f64_i2_oseen", "pairs_f64_i2_oseen_pbc"}},
             {{"pairs_f64_i4_rpy", "pairs_f64_i4_rpy_pbc"}, {"pairs_f64_i4_oseen", "pairs_f64_i4_oseen_pbc"}}};
         cfg.name = names64[cfg.ipt == 4 ? 2 : (cfg.ipt == 2 ? 1 : 0)][rpy ? 0 : 1][pbc ? 1 : 0];
-        if (cfg.ipt == 4)
+        if (large64)
+            cfg.kernel = pbc ? f64_pick<4, true, sd::kTJ64Large>(rpy) : f64_pick<4, false, sd::kTJ64Large>(rpy);
+        else if (cfg.ipt == 4)
             cfg.kernel = pbc ? f64_pick<4, true>(rpy) : f64_pick<4, false>(rpy);
         else if (cfg.ipt == 2)
             cfg.kernel = pbc ? f64_pick<2, true>(rpy) : f64_pick<2, false>(rpy);

@@ -16,6 +16,9 @@
 namespace sd {
 
 constexpr int kTJ64 = 64;  // j records per tile (4 KiB)
+// 128-record tiles (8 KiB) for 4 particles per thread at N >= kRepairMaxN: half the tile hand-overs (see kTJLarge in
+// sd_pairs_f32.cuh); measured 0.5436 -> 0.5465 of the DFMA roofline at N = 1 M, 0.5426 -> 0.5455 at 262 144.
+constexpr int kTJ64Large = 128;
 
 // y0 = MUFU.RSQ(float(r2)) has relative error d0 <= 2^-22.4 + 2^-24 (MUFU + the rounding of r2 to
 // float) ~ 2.4e-7.  With e = 1 - r2 y0^2 ~ -2 d0 (a cancellation: fp64), one Newton step
@@ -220,12 +223,12 @@ __device__ __forceinline__ void chunk_fix_f64(const double (&xi)[I], const doubl
     }
 }
 
-template <int I, int TENSOR, bool PBC>
+template <int I, int TENSOR, bool PBC, int TJ = kTJ64>
 __global__ void __launch_bounds__(kThreads, (I == 1) ? 3 : ((I == 2) ? 2 : 1))
 pairs_f64_kernel(const double4* __restrict__ rec, double4* __restrict__ part, const Schedule sch,
                  const PairCoef64 k, const float thr, const int N, const long long slot_stride) {
     constexpr int IB = kThreads * I;
-    __shared__ __align__(128) double4 tiles[kStages][kTJ64 * 2];
+    __shared__ __align__(128) double4 tiles[kStages][TJ * 2];
     __shared__ __align__(8) uint64_t full_bar[kStages];
     __shared__ __align__(8) uint64_t empty_bar[kStages];
 
@@ -252,8 +255,8 @@ pairs_f64_kernel(const double4* __restrict__ rec, double4* __restrict__ part, co
         const int s = pf_n % kStages;
         const int q = pf_n / kStages;
         if (q > 0) mbar_wait(&empty_bar[s], (q - 1) & 1);
-        mbar_arrive_expect_tx(&full_bar[s], kTJ64 * 64);
-        bulk_load(&tiles[s][0], rec + static_cast<size_t>(pf_t) * (kTJ64 * 2), kTJ64 * 64,
+        mbar_arrive_expect_tx(&full_bar[s], TJ * 64);
+        bulk_load(&tiles[s][0], rec + static_cast<size_t>(pf_t) * (TJ * 2), TJ * 64,
                   &full_bar[s]);
         ++pf_n;
         if (++pf_t == T) pf_t = 0;
@@ -288,10 +291,10 @@ pairs_f64_kernel(const double4* __restrict__ rec, double4* __restrict__ part, co
             const int s = n % kStages;
             mbar_wait(&full_bar[s], (n / kStages) & 1);
             const double4* tile = &tiles[s][0];
-            const int jbase = (t0 + tt) * kTJ64;
+            const int jbase = (t0 + tt) * TJ;
 
 #pragma unroll 1
-            for (int ch = 0; ch < kTJ64 / kChunk; ++ch) {
+            for (int ch = 0; ch < TJ / kChunk; ++ch) {
                 const double4* cj = tile + ch * (kChunk * 2);
                 double qx[I], qy[I], qz[I];
 #pragma unroll

@@ -45,8 +45,8 @@ KERNELS = [
     ("fp32 Rotne-Prager  pairs_f32_kernel<4,RPY,Kahan,REPAIR=0>", "pairs_f32_kernelILi4ELi0ELi0ELb0ELi0ELi256ELi0E", 34, False),
     ("fp32 Oseen         pairs_f32_kernel<4,Oseen,Kahan,REPAIR=0>", "pairs_f32_kernelILi4ELi1ELi0ELb0ELi0ELi256ELi0E", 29, False),
     ("fp32 periodic box  pairs_f32_kernel<4,RPY,Kahan,PBC,REPAIR=0>", "pairs_f32_kernelILi4ELi0ELi0ELb1ELi0ELi256ELi0E", 49, False),
-    ("fp64 Rotne-Prager  pairs_f64_kernel<4,RPY>", "pairs_f64_kernelILi4ELi0ELb0E", 34, True),
-    ("fp64 Oseen         pairs_f64_kernel<4,Oseen>", "pairs_f64_kernelILi4ELi1ELb0E", 29, True),
+    ("fp64 Rotne-Prager  pairs_f64_kernel<4,RPY>", "pairs_f64_kernelILi4ELi0ELb0ELi128E", 34, True),
+    ("fp64 Oseen         pairs_f64_kernel<4,Oseen>", "pairs_f64_kernelILi4ELi1ELb0ELi128E", 29, True),
 ]
 
 _INSTR = re.compile(r"\s*/\*([0-9a-f]+)\*/\s+(@!?U?P\d\s+)?(\S+)\s*(.*?);")
