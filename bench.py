@@ -36,7 +36,7 @@ NCU_TRAFFIC = {
     (1048576, "f32", "rpy", False): (42.7e6, "profiles/r02_pairs_ncu_full.md (dram__bytes_read.sum + "
                                              "dram__bytes_write.sum of pairs_f32_kernel<4,RPY,Kahan,TJ=256>, 34.4 + 8.3 MB)"),
     (1048576, "f32", "rpy", True): (44.2e6, "profiles/r02_pairs_ncu_full.md (pairs_f32_kernel<4,RPY,Kahan,PBC,TJ=256>, 34.4 + 9.7 MB)"),
-    (1048576, "f64", "rpy", False): (3.84e9, "profiles/r02_pairs_ncu_full.md (pairs_f64_kernel<4,RPY>, 3.77 GB + 74 MB: "
+    (1048576, "f64", "rpy", False): (3.60e9, "profiles/r02_pairs_ncu_full.md (pairs_f64_kernel<4,RPY,TJ=128>, 3.54 GB + 68 MB: "
                                              "L2 misses of the 67-MB record stream)"),
 }
 CFG5_NS = [1024, 4096, 16384, 65536, 262144, 1048576]   # BASELINE.json configs[4]
