@@ -538,7 +538,31 @@ def extra_measurements(torch, sd, wl, sm_count, probes):
     return {"what": "BASELINE.json metric beyond the headline point, same process, CUDA events on the "
                     "launching stream; fractions = pairs/s x (34 RPY | 29 Oseen) flops / FMA peak",
             "fma_probe_tflops": probes, "derived_peak_tflops": peaks,
-            "config5_sweep": sweep, "sd_step": steps, "periodic_box": box, "paper_benchmark_shape": fcc}
+            "config5_sweep": sweep, "sd_step": steps, "periodic_box": box, "paper_benchmark_shape": fcc,
+            "issue_model": issue_model()}
+
+
+def issue_model():
+    """Static issue-cycle model of the hot loops of the library this process runs (paper_1205_6333_b200/
+    sassmodel.py: register-bank rule + operand-reuse cache over the SASS; host-side text processing of
+    `cuobjdump -sass`): says where the distance to the FMA roofline goes.  null when cuobjdump is missing."""
+    try:
+        from paper_1205_6333_b200 import sassmodel as sm
+        funcs = sm.disassemble()
+        out = []
+        for label, frag, flops, fp64 in sm.KERNELS:
+            names = [n for n in funcs if frag in n]
+            if not names:
+                continue
+            r = sm.analyse(funcs[names[0]], flops, fp64)
+            out.append({"kernel": " ".join(label.split()), "instructions_per_iteration": r["instructions"],
+                        "fma_class_instructions": r["wide"], "register_bank_conflicts": r["conflicts"],
+                        "model_cycles": r["cycles"], "fma_class_cycles": r["ideal_cycles"],
+                        "frac_model": r["frac_model"], "frac_without_conflicts": r["frac_no_conflicts"],
+                        "frac_fma_class_alone": r["frac_wide_only"]})
+        return {"what": "python -m paper_1205_6333_b200.sassmodel (profiles/r02_issue_model.md)", "kernels": out}
+    except Exception as e:  # diagnostics only: never fail the bench line
+        return {"unavailable": str(e)}
 
 
 def main():
