@@ -236,10 +236,10 @@ def test_uniform_20000_tiled_all_rows(gpu, prec_name, tname):
         assert rel_err(far, want[face]) > 1e-4
 
 
+@pytest.mark.parametrize("n", [131072 + 777, 200000 + 555])  # the second: 256- (fp64: 128-) record tiles, careful pass
 @pytest.mark.parametrize("prec_name", ["PREC_F32_KAHAN", "PREC_F64"])
-def test_uniform_131849_eight_per_thread_sampled_rows(gpu, prec_name):
+def test_uniform_131849_eight_per_thread_sampled_rows(gpu, prec_name, n):
     torch, sd = gpu
-    n = 131072 + 777
     L = wl.cube_side(n, 0.01)
     pos = wl.uniform_cube(n, 0.01, wl.SEED_BASE + 26)
     F = wl.normal_forces(n, wl.SEED_BASE + 27)
