@@ -208,8 +208,9 @@ sd_status sd_schedule_plan(long long N, int particles_per_block, int tile_j, lon
 /* Dispatch knobs of the small-N path (below a few thousand particles the device is
  * under-filled), for ablations and tests; the defaults are the measured crossovers.
  *   small_apply_max     : N up to which one product is ONE launch of the warp-per-particle kernel
- *                         (no pack / partial sums / finalize); < 0 restores the default (2304 in the
- *                         fp32 modes, 1000 in fp64, where the warp-split kernels take over; 2560 with
+ *                         (no pack / partial sums / finalize); < 0 restores the default (fp32 modes:
+ *                         4736 in free space, 2304 in the periodic box and with sd_set_jsplit(ctx, 2);
+ *                         fp64: 1000; the warp-split kernels take over there; 2560 with
  *                         sd_set_jsplit(ctx, 1)).
  *   particles_per_thread: 2, 4 or 8 particles i per thread in the tiled kernels (fp64: half of
  *                         it); 0 = automatic (by N).

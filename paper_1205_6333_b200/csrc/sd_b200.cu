@@ -281,7 +281,9 @@ sd_status set_packed_attr(sd_ctx* c) {
     if (c->precision == SD_PREC_F64 || c->N < sd::kPackedMinN || c->N > sd::kPackedMaxN) return SD_OK;
     const bool rpy = c->tensor == SD_TENSOR_RPY, kahan = c->precision != SD_PREC_F32_PLAIN, pbc = c->box > 0.0;
     const void* f = nullptr;
-#define SD_PKF(T, K, P) reinterpret_cast<const void*>(&sd::small_apply_packed_kernel<T, K, P>)
+#define SD_PKF(T, K, P)                                                                                   \
+    (c->N >= sd::kPackedWideMinN ? reinterpret_cast<const void*>(&sd::small_apply_packed_kernel<T, K, P, 512>) \
+                                 : reinterpret_cast<const void*>(&sd::small_apply_packed_kernel<T, K, P>))
     if (rpy) f = kahan ? (pbc ? SD_PKF(0, true, true) : SD_PKF(0, true, false))
                        : (pbc ? SD_PKF(0, false, true) : SD_PKF(0, false, false));
     else f = kahan ? (pbc ? SD_PKF(1, true, true) : SD_PKF(1, true, false))
@@ -321,12 +323,14 @@ sd_status configure(sd_ctx* c) {
     const bool f64 = c->precision == SD_PREC_F64;
     const bool rpy = c->tensor == SD_TENSOR_RPY;
     const bool pbc = c->box > 0.0;
-    // where the warp-per-particle one-launch kernels stop (measured, profiles/r02_mid_n.md): with the
-    // warp-split kernel behind them at the end of the packed fp32 window (2304) resp. at 1000 in fp64;
-    // 2560 when only the classic tiled kernels follow
+    // where the warp-per-particle one-launch kernels stop (measured, profiles/r02_mid_n.md, sd_small.cuh): with
+    // the warp-split kernel behind them at the end of the packed fp32 window (4736 in free space, 2304 in the
+    // periodic box) resp. at 1000 in fp64; 2560 when only the classic tiled kernels follow
     if (c->small_user >= 0) c->small_apply_max = c->small_user;
     else if (c->jsplit == 1 || c->staging != sd::STAGE_BULK) c->small_apply_max = sd::kSmallApplyMax;
-    else c->small_apply_max = f64 ? sd::kW64MinN : sd::kPackedMaxN;
+    else if (c->jsplit == 2)  // "warp-split wherever it exists": behind the 128-thread packed window
+        c->small_apply_max = f64 ? sd::kW64MinN : sd::kPackedWideMinN - 1;
+    else c->small_apply_max = f64 ? sd::kW64MinN : (pbc ? sd::kPackedMaxNBox : sd::kPackedMaxN);
     if (!f64) {
         const bool plain = c->precision == SD_PREC_F32_PLAIN;
         // particles per thread: 8 once there is enough work to balance 2048-particle i-blocks
@@ -776,15 +780,21 @@ template <int TENSOR, bool KAHAN, bool PBC>
 void launch_small_packed_k(sd_ctx* c, const void* posx, const void* force, const double g[3], void* vel,
                            const void* pos_base, void* pos_out, double dt, int mode, cudaStream_t st) {
     const int n = static_cast<int>(c->N);
-    const int per_cta = (sd::kPackedThreads / 32) * 2;
+    const int threads = sd::packed_threads(n);
+    const int per_cta = (threads / 32) * 2;
     const int blocks = (n + per_cta - 1) / per_cta;
     const double gx = g ? g[0] : 0.0, gy = g ? g[1] : 0.0, gz = g ? g[2] : 0.0;
     const size_t smem = static_cast<size_t>(n) * 32;  // opt-in above 48 KiB: set_packed_attr, at configure time
-    sd::small_apply_packed_kernel<TENSOR, KAHAN, PBC><<<blocks, sd::kPackedThreads, smem, st>>>(
-        static_cast<const float4*>(posx), static_cast<const float4*>(force), gx, gy, gz,
-        static_cast<float4*>(vel), static_cast<const float4*>(pos_base), static_cast<float4*>(c->pos_lo),
-        static_cast<float4*>(pos_out), dt, mode, folded_coef<float>(c), c->mu0 * 0.75 * c->a, c->mu0, n,
-        c->pos_comp);
+#define SD_PK_ARGS                                                                                        \
+    static_cast<const float4*>(posx), static_cast<const float4*>(force), gx, gy, gz,                       \
+        static_cast<float4*>(vel), static_cast<const float4*>(pos_base), static_cast<float4*>(c->pos_lo),  \
+        static_cast<float4*>(pos_out), dt, mode, folded_coef<float>(c), c->mu0 * 0.75 * c->a, c->mu0, n,   \
+        c->pos_comp
+    if (threads == 512)
+        sd::small_apply_packed_kernel<TENSOR, KAHAN, PBC, 512><<<blocks, 512, smem, st>>>(SD_PK_ARGS);
+    else
+        sd::small_apply_packed_kernel<TENSOR, KAHAN, PBC><<<blocks, sd::kPackedThreads, smem, st>>>(SD_PK_ARGS);
+#undef SD_PK_ARGS
 }
 template <bool KAHAN>
 sd_status launch_small_packed(sd_ctx* c, const void* posx, const void* force, const double g[3], void* vel,

@@ -250,16 +250,21 @@ small_apply_kernel(const T4* __restrict__ posx, const T4* __restrict__ force, co
 // merge per 128 j.  CTAs of 128 threads = 8 particles: N / 8 CTAs; the CTA keeps all N records in
 // shared memory.
 constexpr int kPackedThreads = 128;
-// Measured window (graph-replayed Euler steps on the fcc benchmark, us per step, scalar -> packed):
-// N = 108 2.99 -> 3.37, 500 5.29 -> 6.05, 864 8.09 -> 7.56, 2048 17.96 -> 13.89; N = 2560 22.6 -> 30.8
-// per product (80 KiB of shared memory per CTA).  Below the window every CTA copying all N records
-// costs more than the arithmetic saves, above it the shared-memory footprint limits the CTAs per SM.
-constexpr int kPackedMinN = 768;
-constexpr int kPackedMaxN = 2304;
-constexpr int kPackedTile = 128;
+// Measured window (products replayed from a CUDA graph, us per product, free space): against the scalar
+// warp-per-particle kernel N = 256 3.04 (3.06), 384 3.63 (4.09), 512 3.51 (4.76), 768 4.73 (5.92 before the
+// unrolling below); against the warp-split kernel (sd_pairs_f32w.cuh) with CTAs of 512 threads N = 2560 16.1
+// (19.9), 3000 18.5 (22.2), 4096 23.9 (28.0), 4736 27.4 (35.6).  Above 4736 the CTAs no longer fit one per SM
+// (32 N bytes of shared memory each); in the periodic box the warp-split kernel wins from 2304 on (N = 4000:
+// 29.5 against 30.0 us per Euler step).  Round 1 (128-record chunks, rolled loop): N = 1024 6.5, 2048 12.7 us.
+constexpr int kPackedMinN = 256;
+constexpr int kPackedMaxN = 4736;      // 148 SMs x 32 particles: one CTA of 512 threads per SM
+constexpr int kPackedMaxNBox = 2304;   // default limit in the periodic box (29 instead of 20 packed instructions per step: the warp-split kernel's 8 particles per lane win from here on)
+constexpr int kPackedWideMinN = 2305;  // above: CTAs of 512 threads (32 particles), 32 N bytes of shared memory each
+__host__ __device__ constexpr int packed_threads(int n) { return n >= kPackedWideMinN ? 512 : kPackedThreads; }
+constexpr int kPackedTile = 256;
 
-template <int TENSOR, bool KAHAN, bool PBC>
-__global__ void __launch_bounds__(kPackedThreads)
+template <int TENSOR, bool KAHAN, bool PBC, int THREADS = kPackedThreads>
+__global__ void __launch_bounds__(THREADS)
 small_apply_packed_kernel(const float4* __restrict__ posx, const float4* __restrict__ force,
                           const double gx, const double gy, const double gz,
                           float4* __restrict__ vel, const float4* __restrict__ pos_base,
@@ -273,9 +278,11 @@ small_apply_packed_kernel(const float4* __restrict__ posx, const float4* __restr
     float4* sp = s_all;
     float4* sf = s_all + N;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int i0 = (blockIdx.x * (kPackedThreads / 32) + warp) * 2;
+    const int i0 = (blockIdx.x * (THREADS / 32) + warp) * 2;
     const int ia = min(i0, N - 1), ib = min(i0 + 1, N - 1);
-    for (int j = tid; j < N; j += kPackedThreads) {
+    // (unrolled: the loads of four iterations are in flight together; the loop is pure L2 latency)
+#pragma unroll 4
+    for (int j = tid; j < N; j += THREADS) {
         sp[j] = posx[j];
         sf[j] = force ? force[j] : make_float4(float(gx), float(gy), float(gz), 0.f);
     }
@@ -288,25 +295,44 @@ small_apply_packed_kernel(const float4* __restrict__ posx, const float4* __restr
     for (int j0 = 0; j0 < N; j0 += kPackedTile) {   // compensation chunk: <= 4 terms per lane
         const int nj = min(j0 + kPackedTile, N);
         f32x2 px[1] = {zero}, py[1] = {zero}, pz[1] = {zero};
-        for (int j = j0 + lane; j < nj; j += 32) {
-            const float4 pj = sp[j];
-            const float4 fj = sf[j];
-            float mn = 0.f, r2v[2];
-            pair_fast_staged<1, TENSOR, PBC, true>(xi, yi, zi, pj, fj, k, px, py, pz, mn, r2v);
-            if (fminf(r2v[0], r2v[1]) < k.clampv) {
+        // the (at most four) j of a lane: first the clamped packed body of all of them as straight-line code, so
+        // that their address, distance, MUFU and coefficient stages overlap (one warp per scheduler: nothing else
+        // hides those latencies; N = 1024: 6.5 -> 5.9 us per product with the four bodies unrolled), then the rare
+        // pairs below the clamp are put right one by one
+        constexpr int kPerLane = kPackedTile / 32;
+        float r2q[kPerLane][2];
+        auto fast_j = [&](const int q, const int j) {
+            float mn = 0.f;
+            pair_fast_staged<1, TENSOR, PBC, true>(xi, yi, zi, sp[j], sf[j], k, px, py, pz, mn, r2q[q]);
+        };
+        auto fix_j = [&](const int q, const int j) {
+            if (fminf(r2q[q][0], r2q[q][1]) < k.clampv) {
+                const float4 pj = sp[j];
+                const float4 fj = sf[j];
                 float ax = lo2(px[0]), ay = lo2(py[0]), az = lo2(pz[0]);
                 float bx = hi2(px[0]), by = hi2(py[0]), bz = hi2(pz[0]);
-                if (r2v[0] < k.clampv) {
+                if (r2q[q][0] < k.clampv) {
                     pair_clamped_sub<TENSOR, PBC>(pa.x, pa.y, pa.z, pj, fj, k, ax, ay, az);
                     pair_exact<TENSOR, PBC>(pa.x, pa.y, pa.z, j == ia, pj, fj, k, ax, ay, az);
                 }
-                if (r2v[1] < k.clampv) {
+                if (r2q[q][1] < k.clampv) {
                     pair_clamped_sub<TENSOR, PBC>(pb.x, pb.y, pb.z, pj, fj, k, bx, by, bz);
                     pair_exact<TENSOR, PBC>(pb.x, pb.y, pb.z, j == ib, pj, fj, k, bx, by, bz);
                 }
                 px[0] = pk2(ax, bx);
                 py[0] = pk2(ay, by);
                 pz[0] = pk2(az, bz);
+            }
+        };
+        if (nj - j0 == kPackedTile) {
+#pragma unroll
+            for (int q = 0; q < kPerLane; ++q) fast_j(q, j0 + lane + 32 * q);
+#pragma unroll
+            for (int q = 0; q < kPerLane; ++q) fix_j(q, j0 + lane + 32 * q);
+        } else {
+            for (int j = j0 + lane; j < nj; j += 32) {
+                fast_j(0, j);
+                fix_j(0, j);
             }
         }
         if (KAHAN) {

@@ -680,14 +680,15 @@ def test_side_stream_and_two_contexts_give_the_same_bits(gpu):
 @pytest.mark.parametrize("tname", ["TENSOR_RPY", "TENSOR_OSEEN"])
 @pytest.mark.parametrize("boxed", [False, True])
 def test_packed_one_launch_kernel_window(gpu, prec_name, tol, tname, boxed):
-    """768 <= N <= 2304 in the fp32 modes runs small_apply_packed_kernel (two particles of a warp as
-    the halves of packed registers, clamped body + per-pair corrections, all records in shared
-    memory).  Dense clouds (phi = 0.2: overlaps in most rows, one pair of coincident centres), both
-    ends of the window and an odd N, all rows; then one step against the oracle."""
+    """256 <= N <= 4736 (periodic box: 2304 by default) in the fp32 modes runs small_apply_packed_kernel
+    (two particles of a warp as the halves of packed registers, clamped body + per-pair corrections,
+    all records in shared memory; CTAs of 128 threads up to 2304, of 512 above).  Dense clouds
+    (phi = 0.2: overlaps in most rows, one pair of coincident centres), the ends of the two windows
+    and an odd N, all rows; then one step against the oracle."""
     torch, sd = gpu
     prec, tensor = getattr(sd, prec_name), getattr(sd, tname)
     otensor = orc.TENSOR_RPY if tname == "TENSOR_RPY" else orc.TENSOR_OSEEN
-    for n in (768, 1001, 2304):
+    for n in (256, 1001, 2304, 2305, 4736):
         L = wl.cube_side(n, 0.2)
         pos = wl.uniform_cube(n, 0.2, wl.SEED_BASE + 1040 + n)
         pos[n // 2] = pos[3]
@@ -698,6 +699,8 @@ def test_packed_one_launch_kernel_window(gpu, prec_name, tol, tname, boxed):
         ctx.set_tensor(tensor)
         if boxed:
             ctx.set_box(L)
+            if n > 2304:
+                ctx.set_dispatch(n, 0)           # beyond the default window of the box: forced
         assert ctx.kernel_name == "small_apply_f32x2"
         dp, df = torch.from_numpy(p).cuda(), torch.from_numpy(f).cuda()
         dv = torch.full_like(dp, float("nan"))
