@@ -253,9 +253,9 @@ constexpr int kPackedThreads = 128;
 // Measured window (products replayed from a CUDA graph, us per product, free space): against the scalar
 // warp-per-particle kernel N = 256 3.04 (3.06), 384 3.63 (4.09), 512 3.51 (4.76), 768 4.73 (5.92 before the
 // unrolling below); against the warp-split kernel (sd_pairs_f32w.cuh) with CTAs of 512 threads N = 2560 16.1
-// (19.9), 3000 18.5 (22.2), 4096 23.9 (28.0), 4736 27.4 (35.6).  Above 4736 the CTAs no longer fit one per SM
+// (19.9), 3000 17.8 (22.2), 4096 23.0 (28.0), 4736 26.4 (35.6).  Above 4736 the CTAs no longer fit one per SM
 // (32 N bytes of shared memory each); in the periodic box the warp-split kernel wins from 2304 on (N = 4000:
-// 29.5 against 30.0 us per Euler step).  Round 1 (128-record chunks, rolled loop): N = 1024 6.5, 2048 12.7 us.
+// 29.6 against 28.1 us per Euler step with the packed kernel forced, but 20.7 against 21.6 at N = 2916: no window worth a second threshold).  Round 1 (128-record chunks, rolled loop): N = 1024 6.5, 2048 12.7 us.
 constexpr int kPackedMinN = 256;
 constexpr int kPackedMaxN = 4736;      // 148 SMs x 32 particles: one CTA of 512 threads per SM
 constexpr int kPackedMaxNBox = 2304;   // default limit in the periodic box (29 instead of 20 packed instructions per step: the warp-split kernel's 8 particles per lane win from here on)
@@ -292,14 +292,17 @@ small_apply_packed_kernel(const float4* __restrict__ posx, const float4* __restr
     f32x2 xi[1] = {add2(pk2(pa.x, pb.x), zero)}, yi[1] = {add2(pk2(pa.y, pb.y), zero)},
           zi[1] = {add2(pk2(pa.z, pb.z), zero)};
     f32x2 sx = zero, sy = zero, sz = zero, cx = zero, cy = zero, cz = zero;
-    for (int j0 = 0; j0 < N; j0 += kPackedTile) {   // compensation chunk: <= 4 terms per lane
-        const int nj = min(j0 + kPackedTile, N);
+    // 256-record chunks with 128 threads (eight j per lane in flight); 128-record chunks with 512 threads, where
+    // the 128-register cap would otherwise spill (24 ... 48 B of stack: N = 4096 23.9 -> 23.0 us without)
+    constexpr int kTile = (THREADS > kPackedThreads) ? 128 : kPackedTile;
+    for (int j0 = 0; j0 < N; j0 += kTile) {   // compensation chunk: kTile / 32 terms per lane
+        const int nj = min(j0 + kTile, N);
         f32x2 px[1] = {zero}, py[1] = {zero}, pz[1] = {zero};
         // the (at most four) j of a lane: first the clamped packed body of all of them as straight-line code, so
         // that their address, distance, MUFU and coefficient stages overlap (one warp per scheduler: nothing else
         // hides those latencies; N = 1024: 6.5 -> 5.9 us per product with the four bodies unrolled), then the rare
         // pairs below the clamp are put right one by one
-        constexpr int kPerLane = kPackedTile / 32;
+        constexpr int kPerLane = kTile / 32;
         float r2q[kPerLane][2];
         auto fast_j = [&](const int q, const int j) {
             float mn = 0.f;
@@ -324,7 +327,7 @@ small_apply_packed_kernel(const float4* __restrict__ posx, const float4* __restr
                 pz[0] = pk2(az, bz);
             }
         };
-        if (nj - j0 == kPackedTile) {
+        if (nj - j0 == kTile) {
 #pragma unroll
             for (int q = 0; q < kPerLane; ++q) fast_j(q, j0 + lane + 32 * q);
 #pragma unroll
